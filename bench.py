@@ -1,0 +1,261 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of BASELINE.json: Metropolis spin-flip attempts/s at
+L=4096, q=8, sigma=0.3, 128 replicas (configs[3]), swap event every sweep.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--variant auto|direct|field]
+
+One STEP = one sweep of every replica (L Metropolis steps each, Eq. 8) + the per-slot observables +
+one replica-exchange event (Eq. 9) = n_rep*L attempts, i.e. one pass of the whole hot path.  The
+default K = 2000 is the full configs[3] run.  Prints ONE JSON line (rank 0).  For N > 1 (torchrun)
+every rank runs its own ensemble of configs[3] (ens_base = rank: independent random streams, no
+data-path collective), so scaling is "weak" and `value` is the sum over ranks / max time.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1308_5426_b200 import inputs  # noqa: E402
+
+METRIC = "Metropolis spin-flip attempts/s at L=4096 q=8 128 replicas"
+UNIT = "attempts/s"
+# IDP.2A issue rate assumed for the ALU roofline (lanes per clock per SM on the FMA-heavy pipe:
+# B300_MICROARCH.md "Pipe rates": rt_SMSP = 2 -> 16 lanes/clk/SMSP x 4 SMSPs); DESIGN.md section 6.
+IDP_LANES_PER_CLK_PER_SM = 64
+N_SM = 148
+
+
+def workload_config(w, variant, n_gpus):
+    return {"workload": "configs[3]: L=%d q=%d sigma=%.1f, 1 ensemble x %d replicas per GPU, T geometric in "
+                        "[%.1f,%.1f], hot start, swap every sweep" % (w.L, w.q, w.sigma, w.n_rep, w.T_lo, w.T_hi),
+            "step": "1 sweep of all replicas + observables + 1 swap event = %d attempts per GPU" % (w.L * w.n_rep),
+            "variant": variant, "parallelism": "ensembles sharded over %d GPU(s), no collective" % n_gpus,
+            "l2": "not flushed: per-step state is %d KB of packed spins per GPU, resident in shared memory/L2 by "
+                  "design; the path is ALU-bound, not HBM-bound" % (w.n_rep * w.L // 2 // 1024)}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML during the timed region."""
+    REASONS = {0x2: "applications_clocks_setting", 0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x10: "sync_boost",
+               0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown",
+               0x100: "display_clock_setting"}
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.sm, self.mask, self.max_mhz, self.err = index, False, [], 0, None, None
+
+    def run(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM)
+            while not self.stop_flag:
+                self.sm.append(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
+                self.mask |= int(pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+                time.sleep(0.02)
+        except Exception as ex:  # NVML missing: report, do not fake
+            self.err = repr(ex)
+
+    def result(self):
+        self.stop_flag = True
+        self.join(timeout=2.0)
+        if not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "error": self.err}
+        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.max_mhz, "samples": len(self.sm),
+                "reasons": [n for b, n in self.REASONS.items() if self.mask & b]}
+
+
+def oracle_threads():
+    return max(1, os.cpu_count() or 1)
+
+
+def time_oracle_step(o, replicas_done_per_step, threads):
+    t0 = time.perf_counter()
+    o.sweeps(1, 1, field=False, threads=threads)
+    return time.perf_counter() - t0
+
+
+def cpu_baseline_leg(w, budget_s=12.0):
+    """The oracle as it stands (direct O(L) sum per step, the paper's way), all host cores, full configs[3]
+    ensemble, as many sweeps as fit the budget (at least 1)."""
+    from oracle import pt_oracle
+    threads = oracle_threads()
+    o = pt_oracle.Oracle(w.L, w.q, w.sigma, 1, w.n_rep, inputs.betas(w), w.seed)
+    n, t = 0, 0.0
+    while n < 1 or (t < budget_s and n < 64 and t + t / n < 2.5 * budget_s):
+        t += time_oracle_step(o, w.n_rep, threads)
+        n += 1
+    o.close()
+    return {"value": n * w.n_rep * w.L / t, "unit": UNIT, "cores": min(threads, w.n_rep), "kind": "oracle",
+            "sample": "%d sweep(s) (+swap events) of the full configs[3] ensemble (128 replicas), direct-sum mode, "
+                      "%d std::threads, g++ -O2, %.1f s" % (n, min(threads, w.n_rep), t)}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle timed on the host cores; a step = one sweep (+swap event) of a bounded
+    sample of r evenly spaced slots of configs[3]."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from oracle import pt_oracle
+    pt_oracle.build()
+    w = inputs.config(3)
+    threads = oracle_threads()
+    betas = inputs.betas(w)
+    # calibrate on one replica, then size the sample so that (K+W) steps take <= ~150 s
+    o1 = pt_oracle.Oracle(w.L, w.q, w.sigma, 1, 1, betas[:1], w.seed)
+    t1 = time_oracle_step(o1, 1, 1)
+    o1.close()
+    total_steps = args.steps + args.warmup
+    per_step_budget = 150.0 / max(1, total_steps)
+    r = int(per_step_budget / t1 * min(threads, w.n_rep) * 0.7)
+    r = max(1, min(w.n_rep, r))
+    idx = np.unique(np.linspace(0, w.n_rep - 1, r).round().astype(int))
+    r = len(idx)
+    use_threads = min(threads, r)
+    o = pt_oracle.Oracle(w.L, w.q, w.sigma, 1, r, betas[idx], w.seed)
+    for _ in range(args.warmup):
+        time_oracle_step(o, r, use_threads)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.sweeps(1, 1, field=False, threads=use_threads)
+    dt = time.perf_counter() - t0
+    o.close()
+    value = args.steps * r * w.L / dt
+    sample = ("each step = 1 sweep + swap event of %d of the 128 slots of configs[3] (evenly spaced in the ladder), "
+              "direct-sum mode, %d std::threads" % (r, use_threads))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32",
+            "data": "synthetic", "config": workload_config(w, "oracle", args.gpus),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": use_threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1308_5426_b200 import build as ptbuild
+    ptbuild.build()
+    from paper_1308_5426_b200 import pt
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libpt has no CPU path")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    w = inputs.config(3)
+    betas = inputs.betas(w)
+    K, W_ = args.steps, args.warmup
+    g = pt.PT(w.L, w.q, w.sigma, 1, w.n_rep, betas, w.seed, ens_base=rank, variant=args.variant)
+    variant = g.get_variant()
+    stream = torch.cuda.Stream()
+    g.use_torch_stream(stream)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: K steps = K sweeps, a swap event after each ----
+    with torch.cuda.stream(stream):
+        g.sweeps_async(W_, w.swap_every)
+        g.sync()
+        barrier()
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev0.record(stream)
+        launches = g.sweeps_async(K, w.swap_every)
+        ev1.record(stream)
+        g.sync()
+        barrier()
+        clocks = sampler.result()
+    ms = ev0.elapsed_time(ev1)
+    if world > 1:
+        tmax = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        ms = float(tmax.item())
+    attempts_per_gpu = K * w.n_rep * w.L
+    value = world * attempts_per_gpu / (ms * 1e-3)
+    obs = g.observables()
+    acc = float(obs["flip_accepts"].sum()) / float(obs["flip_attempts"].sum())
+
+    # ---- end to end through the C ABI with host buffers: upload a start configuration, K steps, read back ----
+    start = g.get_spins()
+    barrier()
+    t0 = time.perf_counter()
+    g.set_spins(start)                       # H2D: n_rep*L bytes
+    g.sweeps(K, w.swap_every)
+    spins = g.get_spins()                    # D2H: n_rep*L bytes
+    E = g.energy()                           # D2H: n_rep*8 bytes
+    ob = g.observables()                     # D2H: n_rep*88 bytes
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if world > 1:
+        tmax = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+        e2e_s = float(tmax.item())
+    assert spins.shape == start.shape and E.size == w.n_rep and ob["n_samples"].min() > 0
+    e2e = {"value": world * attempts_per_gpu / e2e_s, "unit": UNIT,
+           "h2d_bytes_per_step": start.nbytes / K, "d2h_bytes_per_step": (spins.nbytes + E.nbytes + w.n_rep * 88) / K,
+           "what": "pt_set_spins(host) + pt_sweeps(K) + pt_get_spins + pt_energy + pt_observables (host buffers), wall clock"}
+
+    if rank == 0:
+        f_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
+        pair_terms_per_launch = w.n_rep * w.L * w.L          # one IDP.2A lane-op pair per (i,j) term and 16-bit half
+        launch_s = ms * 1e-3 / max(1, launches)
+        achieved = pair_terms_per_launch / launch_s / 1e12
+        peak = N_SM * IDP_LANES_PER_CLK_PER_SM * 2 / 2 * f_hz / 1e12   # 2 MACs per lane-op, 2 MACs per pair term
+        roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tpair-terms/s", "frac": achieved / peak,
+                    "traffic": None, "kernel": "sweep_%s_kernel" % variant,
+                    "note": "peak = 148 SMs x 64 IDP.2A lanes/clk/SM x sampled SM clock (%.0f MHz), one lane-op per "
+                            "pair term per 16-bit half (DESIGN.md section 6); of derived ALU peak, not of "
+                            "MEASURED_PEAKS.json (HBM/tensor peaks do not bound this path); DRAM traffic per launch is "
+                            "~%d KB of packed spins" % (f_hz / 1e6, 2 * w.n_rep * w.L // 2 // 1024)}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
+                "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "int32", "data": "synthetic", "config": workload_config(w, variant, world),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+                "flip_acceptance": acc, "pair_evaluations_per_s": value * (w.L - 1)}
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline_leg(w)
+        print(json.dumps(line))
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "direct", "field"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,165 @@
+/* include/pt.h -- C ABI of libpt: the parallel-tempering Metropolis sweep of the
+ * one-dimensional q-state Potts model with periodic long-range couplings
+ * (arXiv 1308.5426; citations are PAPER.md:<line> plus the equation/section).
+ *
+ * The model (Eqs. 1-7): spins s_i in {1..q} (Eq. 1) on a ring
+ * of L sites, H = -sum_{i<j} J*(|i-j|) delta(s_i,s_j) (Eqs. 2-3, each unordered
+ * pair once -- reading A1 of DESIGN.md), J*(r) = sum_n |r+nL|^-(1+sigma)
+ * (Eqs. 4-5) evaluated through the Hurwitz-zeta closed form (Eqs. 6-7).
+ * The library quantises J* to int32 fixed point at scale 2^24,
+ * Jq[r] = round(J*(r) 2^24), so every energy below is an exact integer in
+ * units of 2^-24 and independent of summation order.
+ *
+ * The method (Eqs. 8-9; 110-128, section 4.2): n_rep replicas
+ * ("slots", one per inverse temperature) per ensemble; one sweep = L
+ * single-spin Metropolis steps (Eq. 8) in site order 0..L-1 on every replica;
+ * a swap event = replica exchange (Eq. 9) between neighbouring slots, pairs
+ * (t,t+1) with t even first, then t odd.  Randomness is
+ * Philox-4x32-10 keyed by (seed; ensemble, slot, sweep, site), so a trajectory
+ * is a pure function of the arguments of pt_create and the number of sweeps.
+ *
+ * Conventions
+ *  - All pointers are HOST pointers unless the function name ends in _dev, in
+ *    which case they are DEVICE pointers on the context's device.  The caller
+ *    owns every in/out array; the library owns all state behind pt_ctx.
+ *  - Arrays over replicas are indexed [ensemble][slot], slot = position in
+ *    `betas`; "neighbouring temperatures" = adjacent slots.
+ *  - Every function returns 0 (PT_OK) or a negative pt_status; the message of
+ *    the last failure on the calling thread is returned by pt_last_error().
+ *    No C++ exception crosses this boundary.  Calls are synchronous: results
+ *    are complete when the call returns (kernels run on the stream given to
+ *    pt_set_stream, default stream otherwise).
+ *  - A context must not be used from two threads at once.
+ */
+#ifndef PT_H_
+#define PT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pt_ctx pt_ctx; /* opaque; created by pt_create, freed by pt_destroy */
+
+typedef enum {
+    PT_OK = 0,
+    PT_EINVAL = -1,    /* bad argument (see each call) */
+    PT_EOVERFLOW = -2, /* sum_r Jq[r] >= 2^31: dE would not fit int32 (sigma too small) */
+    PT_ENOMEM = -3,    /* host or device allocation failed */
+    PT_ECUDA = -4,     /* CUDA runtime error, no device, or not an sm_100 device */
+    PT_ECAPACITY = -5  /* no sweep variant fits the shared memory of one SM for (L,q) */
+} pt_status;
+
+/* Sweep variants (pt_set_variant).  Both produce bit-identical trajectories.
+ *  PT_VARIANT_FIELD : per-colour local fields h[k][i] = sum_{j!=i} Jq[|i-j|][s_j==k]
+ *                     kept in shared memory; a proposal costs O(1), an accepted
+ *                     change updates two columns of h (north_star (3)).
+ *  PT_VARIANT_DIRECT: dE = sum_j Jq[|i-j|]([s_j==a]-[s_j==b]) summed directly
+ *                     (PAPER.md:118-124), for blocks of 32 consecutive sites at a
+ *                     time, with exact integer corrections for the changes
+ *                     accepted inside the block.  Needs L % 32 == 0 and q <= 8.
+ *  PT_VARIANT_AUTO  : DIRECT where it applies, else FIELD. */
+enum { PT_VARIANT_AUTO = 0, PT_VARIANT_FIELD = 1, PT_VARIANT_DIRECT = 2 };
+
+/* Cumulative per-slot accumulators since pt_create (the caller differences two
+ * snapshots to discard burn-in).  Sampled after every sweep, before the swap
+ * event, for the slot the configuration occupied during the sweep
+ * ("at the end of the Metropolis cycle we calculate the total
+ * energy"; Eq. 10 PAPER.md:136-140 for the magnetisation).
+ * E is the TOTAL energy in fixed point (units 2^-24).  Nmax = max_k N_k, so
+ * that M = (q Nmax/L - 1)/(q-1) (Eq. 10). */
+typedef struct {
+    int64_t n_samples;
+    int64_t sum_E;
+    uint64_t sum_E2_lo; /* sum of E^2 as a 128-bit integer: low 64 bits ... */
+    int64_t sum_E2_hi;  /* ... high 64 bits */
+    int64_t sum_Nmax;
+    int64_t sum_Nmax2;
+    int64_t flip_attempts; /* Metropolis steps, Eq. 8 */
+    int64_t flip_accepts;
+    int64_t swap_attempts; /* Eq. 9, pair (t,t+1) recorded at slot t */
+    int64_t swap_accepts;
+    int64_t near_ties;     /* -1: not counted by this library (the CPU oracle counts them) */
+} pt_obs;
+
+/* Create a context on the current CUDA device: evaluates J* (Eqs. 5-7) on the
+ * device in fp64 and quantises it, draws the hot start (spins uniform in
+ * {1..q} from the Philox stream) and computes every replica's total energy.
+ *  L      : ring length, L >= 8 and L % 8 == 0 (8 spins per 32-bit word)
+ *  q      : number of colours, 2 <= q <= 16 (4 bits per spin)
+ *  sigma  : decay exponent of Eq. 4, finite and > 0
+ *  n_ens  : independent ensembles (same model, different random streams) >= 1
+ *  n_rep  : replicas per ensemble >= 1
+ *  betas  : [n_rep] inverse temperatures (k_B = 1), finite, >= 0,
+ *           any order; shared by all ensembles
+ *  seed   : Philox key
+ * Errors: PT_EINVAL, PT_EOVERFLOW, PT_ENOMEM, PT_ECUDA, PT_ECAPACITY. *out is
+ * set to NULL on failure. */
+int pt_create(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
+              const double* betas, uint64_t seed);
+
+/* As pt_create, with the ensemble index of this context's first ensemble set
+ * to ens_base (0 <= ens_base, ens_base + n_ens <= 2^28): ensemble e of this
+ * context draws the random stream of global ensemble ens_base + e.  This is how
+ * ensembles are sharded over processes / GPUs without any communication. */
+int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
+                 const double* betas, uint64_t seed, int ens_base);
+
+void pt_destroy(pt_ctx* ctx); /* NULL is allowed */
+
+/* Advance every replica by n >= 0 sweeps.  With swap_every > 0 a swap event
+ * follows each sweep whose global index (counted from pt_create, first sweep
+ * = 1) is a multiple of swap_every, so splitting n over several calls changes
+ * nothing.  swap_every = 0: never swap.  Errors: PT_EINVAL (n < 0,
+ * swap_every < 0), PT_ECUDA. */
+int pt_sweeps(pt_ctx* ctx, int64_t n, int swap_every);
+
+/* Total energies E_out[n_ens*n_rep] (fixed point 2^-24).  recompute = 0 returns
+ * the running value (E0 + sum of accepted dE); recompute = 1 recounts
+ * E = -sum_{i<j} Jq[j-i] [s_i==s_j] from the spins (O(L^2)) and
+ * leaves the running value untouched. */
+int pt_energy(pt_ctx* ctx, int64_t* E_out, int recompute);
+int pt_energy_dev(pt_ctx* ctx, int64_t* E_out_dev, int recompute);
+
+/* out[n_ens*n_rep] accumulators, see pt_obs. */
+int pt_observables(pt_ctx* ctx, pt_obs* out);
+
+/* out[n_ens*n_rep*L] colours 1..q (Eq. 1), one byte per spin. */
+int pt_get_spins(pt_ctx* ctx, uint8_t* out);
+int pt_get_spins_dev(pt_ctx* ctx, uint8_t* out_dev);
+
+/* Replace all configurations (cold starts, resume); recomputes the energies
+ * (and local fields).  PT_EINVAL if a colour is outside 1..q (state unchanged).
+ * The sweep counter and the accumulators are kept. */
+int pt_set_spins(pt_ctx* ctx, const uint8_t* in);
+
+/* Jq[L]: Jq[0] = 0, Jq[r] = Jq[L-r] = round(J*(r) 2^24). */
+int pt_get_couplings(pt_ctx* ctx, int32_t* Jq);
+
+/* Number of sweeps done since pt_create. */
+int64_t pt_sweep_counter(pt_ctx* ctx);
+
+/* variant: PT_VARIANT_*.  PT_EINVAL if the variant cannot run this (L,q);
+ * PT_ECAPACITY if it does not fit in shared memory.  Switching rebuilds
+ * whatever the new variant needs from the spins; the trajectory is unchanged. */
+int pt_set_variant(pt_ctx* ctx, int variant);
+int pt_get_variant(pt_ctx* ctx); /* the variant that pt_sweeps runs (FIELD or DIRECT) */
+
+/* Kernels are launched on `cuda_stream` (a cudaStream_t; NULL = default stream). */
+int pt_set_stream(pt_ctx* ctx, void* cuda_stream);
+
+/* Asynchronous form of pt_sweeps for timing with CUDA events: enqueues the
+ * launches on the context's stream and returns without synchronising.
+ * *n_launches (may be NULL) receives the number of kernels enqueued. */
+int pt_sweeps_async(pt_ctx* ctx, int64_t n, int swap_every, int64_t* n_launches);
+
+/* Blocks until the context's stream is idle; returns PT_ECUDA if a kernel failed. */
+int pt_sync(pt_ctx* ctx);
+
+const char* pt_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PT_H_ */

@@ -1,0 +1,332 @@
+// pt_kernels.cuh -- set-up, energy, swap and I/O kernels of libpt (sm_100a).
+// The sweep kernels are in pt_sweep_field.cuh and pt_sweep_direct.cuh.
+#pragma once
+#include <cstdint>
+
+#include "pt.h"
+#include "pt_device.cuh"
+
+namespace ptk {
+
+using namespace ptdev;
+
+// Everything a kernel needs to know about a context (passed by value).
+struct Dev {
+    int L, W, q, n_ens, n_rep, ens_base;
+    uint32_t key0, key1;
+    const int32_t* Jq;        // [L]
+    const uint32_t* Jpair;    // direct variant: [4][L/2] packed 16-bit halves, see pack_pairs_kernel
+    const double* beta;       // [n_rep]
+    const double* thr_scale;  // [n_rep] 2^24/beta
+    uint32_t* spins;          // [n_ens*n_rep][W]   storage order
+    long long* E;             // [n_ens*n_rep]      storage order
+    int* perm;                // [n_ens][n_rep]     slot -> storage index inside the ensemble
+    pt_obs* obs;              // [n_ens][n_rep]     slot order
+    int32_t* h;               // [n_ens*n_rep][q][L] storage order (field variant)
+    unsigned* done;           // [n_ens] arrival counters of the swap event
+};
+
+// ---------------------------------------------------------------------------
+// a1. J* table (Eqs. 5-7).  With x = r/L and s = 1+sigma,
+//   J*(r) = sum_n |r+nL|^-s = L^-s [ zeta(s,x) + zeta(s,1-x) ],
+// zeta(s,y) = sum_{k>=0} (k+y)^-s the Hurwitz zeta function of Eq. 7 (Eq. 6
+// is the same expression with the k = 0 term of zeta(s,x) written as r^-s).
+// Each zeta is summed directly for k < NDIRECT and closed with the
+// Euler-Maclaurin remainder at y + NDIRECT.  One thread per r <= L/2; the
+// table is mirrored so that it is exactly symmetric (A3); Jq[0] = 0 (A2).
+// ---------------------------------------------------------------------------
+__device__ inline double zeta_tail(double s, double y) {
+    // sum_{k>=0} (y+k)^-s for y >= 16:  y^(1-s)/(s-1) + y^-s/2 + sum_m B_2m/(2m)! s^(2m-1) y^(-s-2m+1)
+    const double ys = pow(y, -s);
+    const double iy2 = 1.0 / (y * y);
+    double term = s * ys / y;  // s y^(-s-1)
+    double acc = 0.0;
+    const double b[6] = {1.0 / 12.0, -1.0 / 720.0, 1.0 / 30240.0, -1.0 / 1209600.0, 1.0 / 47900160.0,
+                         -691.0 / 1307674368000.0};
+    double corr[6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) {
+        corr[m] = b[m] * term;
+        term *= (s + (2 * m + 1)) * (s + (2 * m + 2)) * iy2;
+    }
+#pragma unroll
+    for (int m = 5; m >= 0; --m) acc += corr[m];
+    return acc + 0.5 * ys + ys * y / (s - 1.0);
+}
+
+__global__ void jstar_kernel(int L, double sigma, int32_t* __restrict__ Jq, double* __restrict__ Jreal) {
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r == 0) { Jq[0] = 0; if (Jreal) Jreal[0] = 0.0; }
+    if (r < 1 || r > L / 2) return;
+    constexpr int NDIRECT = 16;
+    const double s = 1.0 + sigma;
+    const double x = (double)r / (double)L;
+    double acc = zeta_tail(s, NDIRECT + x) + zeta_tail(s, NDIRECT + 1.0 - x);
+    for (int k = NDIRECT - 1; k >= 0; --k) acc += pow(k + x, -s) + pow(k + 1.0 - x, -s);
+    const double J = acc * pow((double)L, -s);
+    const long long v = __double2ll_rn(J * 16777216.0);  // scale 2^24 (A16), ties to even
+    Jq[r] = (int32_t)v;
+    Jq[L - r] = (int32_t)v;
+    if (Jreal) { Jreal[r] = J; Jreal[L - r] = J; }
+}
+
+// Direct variant tables.  For parity p in {0,1} and m in [0, L/2): r = 2m+p,
+//   lo[p][m] = (Jq[r] & 0xffff) | (Jq[r-1] & 0xffff) << 16
+//   hi[p][m] = (Jq[r] >> 16)    | (Jq[r-1] >> 16)    << 16       (indices mod L)
+// laid out as Jpair[0]=lo[0], [1]=hi[0], [2]=lo[1], [3]=hi[1], each L/2 words.
+__global__ void pack_pairs_kernel(int L, const int32_t* __restrict__ Jq, uint32_t* __restrict__ Jpair) {
+    const int m = blockIdx.x * blockDim.x + threadIdx.x;
+    const int H = L / 2;
+    if (m >= H) return;
+    for (int p = 0; p < 2; ++p) {
+        const int r = 2 * m + p;
+        const uint32_t j0 = (uint32_t)Jq[r], j1 = (uint32_t)Jq[(r + L - 1) % L];
+        Jpair[(2 * p + 0) * H + m] = (j0 & 0xffffu) | ((j1 & 0xffffu) << 16);
+        Jpair[(2 * p + 1) * H + m] = (j0 >> 16) | ((j1 >> 16) << 16);
+    }
+}
+
+// ---------------------------------------------------------------------------
+// a2. Hot start (configs; not in the paper): colour of site i of slot t of
+// ensemble e = mulhi32(Philox(i, 0, t, e<<4|INIT).w0, q).  One thread per word.
+// ---------------------------------------------------------------------------
+__global__ void init_spins_kernel(Dev d) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)d.n_ens * d.n_rep * d.W;
+    if (gid >= total) return;
+    const int w = (int)(gid % d.W);
+    const int x = (int)(gid / d.W);
+    const int e = x / d.n_rep, t = x % d.n_rep;
+    const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_INIT;
+    uint32_t word = 0;
+#pragma unroll
+    for (int n = 0; n < 8; ++n) {
+        const Philox4 p = philox4x32_10((uint32_t)(8 * w + n), 0u, (uint32_t)t, c3, d.key0, d.key1);
+        word |= __umulhi(p.w0, (uint32_t)d.q) << (4 * n);
+    }
+    d.spins[gid] = word;  // storage index == slot at creation (perm = identity)
+}
+
+__global__ void init_perm_kernel(Dev d) {
+    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid < d.n_ens * d.n_rep) d.perm[gid] = gid % d.n_rep;
+}
+
+// ---------------------------------------------------------------------------
+// a6. Total energy (Eq. 2 in reading A1):
+//   E = -sum_{i<j} Jq[j-i] [c_i==c_j] = -(1/2) sum_i sum_{j!=i} Jq[|i-j|] [c_j==c_i].
+// One CTA per replica (storage order), one site per thread and pass; spins and
+// couplings staged in shared memory; SWAR match of 8 sites per word.
+// dynamic smem: (L + W) * 4 bytes.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) energy_kernel(Dev d, long long* __restrict__ E_out) {
+    extern __shared__ uint32_t smem_e[];
+    int32_t* J = (int32_t*)smem_e;
+    uint32_t* sp = smem_e + d.L;
+    __shared__ long long s_part[8];
+    const int x = blockIdx.x;
+    for (int r = threadIdx.x; r < d.L; r += blockDim.x) J[r] = d.Jq[r];
+    for (int w = threadIdx.x; w < d.W; w += blockDim.x) sp[w] = d.spins[(size_t)x * d.W + w];
+    __syncthreads();
+    long long acc = 0;
+    for (int i = threadIdx.x; i < d.L; i += blockDim.x) {
+        const uint32_t a = (uint32_t)get_nibble(sp, i);
+        long long row = 0;
+        for (int w = 0; w < d.W; ++w) {
+            uint32_t m = match_nibbles(sp[w], a);
+            while (m) {
+                const int bit = __ffs(m) - 1;
+                m &= m - 1;
+                const int j = 8 * w + (bit >> 2);
+                const int dist = j > i ? j - i : i - j;
+                row += J[dist];  // J[0] = 0 removes j == i
+            }
+        }
+        acc += row;
+    }
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        long long tot = 0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) tot += s_part[k];
+        E_out[x] = -(tot / 2);  // the ordered-pair sum is even
+    }
+}
+
+// ---------------------------------------------------------------------------
+// Local fields of the field variant (north_star (3)):
+//   h[x][k][i] = sum_{j!=i} Jq[|i-j|] [c_j==k].   One CTA per replica.
+// dynamic smem: (L + W) * 4 bytes.
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) build_fields_kernel(Dev d) {
+    extern __shared__ uint32_t smem_e[];
+    int32_t* J = (int32_t*)smem_e;
+    uint32_t* sp = smem_e + d.L;
+    const int x = blockIdx.x;
+    for (int r = threadIdx.x; r < d.L; r += blockDim.x) J[r] = d.Jq[r];
+    for (int w = threadIdx.x; w < d.W; w += blockDim.x) sp[w] = d.spins[(size_t)x * d.W + w];
+    __syncthreads();
+    int32_t* hx = d.h + (size_t)x * d.q * d.L;
+    for (int i = threadIdx.x; i < d.L; i += blockDim.x) {
+        for (int k = 0; k < d.q; ++k) {
+            int32_t acc = 0;
+            for (int w = 0; w < d.W; ++w) {
+                uint32_t m = match_nibbles(sp[w], (uint32_t)k);
+                while (m) {
+                    const int bit = __ffs(m) - 1;
+                    m &= m - 1;
+                    const int j = 8 * w + (bit >> 2);
+                    const int dist = j > i ? j - i : i - j;
+                    acc += J[dist];
+                }
+            }
+            hx[(size_t)k * d.L + i] = acc;
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------
+// a7. Swap event (Eq. 9; 126: pairs (t,t+1), t even, then t
+// odd).  Run by ONE CTA per ensemble after every replica of the ensemble has
+// published its energy.  Configurations stay where they are stored; the
+// slot -> storage permutation is exchanged (A12).  Accept iff
+//   d = (beta_t - beta_{t+1}) (E_t - E_{t+1}) 2^-24 >= 0  or  u < exp(d),
+// u from Philox(t, sweep, 0, e<<4|SWAP).  fp64 throughout, one rounding in d.
+// ---------------------------------------------------------------------------
+__device__ inline void swap_event(const Dev& d, int e, uint32_t sweep) {
+    int* perm = d.perm + (size_t)e * d.n_rep;
+    const long long* E = d.E + (size_t)e * d.n_rep;
+    pt_obs* obs = d.obs + (size_t)e * d.n_rep;
+    const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_SWAP;
+    for (int stage = 0; stage < 2; ++stage) {
+        for (int t = stage + 2 * (int)threadIdx.x; t + 1 < d.n_rep; t += 2 * (int)blockDim.x) {
+            const int sa = perm[t], sb = perm[t + 1];
+            const long long Ea = __ldcg(E + sa), Eb = __ldcg(E + sb);
+            const double dd = __dmul_rn(d.beta[t] - d.beta[t + 1], ldexp((double)(Ea - Eb), -24));
+            const Philox4 p = philox4x32_10((uint32_t)t, sweep, 0u, c3, d.key0, d.key1);
+            const double u = uniform53(p.w1, p.w2);
+            obs[t].swap_attempts += 1;
+            if (dd >= 0.0 || u < exp(dd)) {
+                perm[t] = sb;
+                perm[t + 1] = sa;
+                obs[t].swap_accepts += 1;
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// Called by every CTA of a sweep kernel at the end of a launch that ends with a
+// swap event: the CTA that arrives last at the ensemble's counter runs the
+// event (no CTA ever waits for another one).  All threads of the CTA must call.
+__device__ inline void arrive_and_swap(const Dev& d, int e, uint32_t sweep) {
+    __shared__ int s_last;
+    __threadfence();  // this thread's global writes (E, spins, fields, obs) before the arrival
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const unsigned prev = atomicAdd(d.done + e, 1u);
+        s_last = (prev == (unsigned)d.n_rep - 1u);
+        __threadfence();
+    }
+    __syncthreads();
+    if (s_last) {
+        swap_event(d, e, sweep);
+        if (threadIdx.x == 0) d.done[e] = 0u;
+    }
+}
+
+// Stand-alone swap kernel (one CTA per ensemble), used when a swap event has
+// to follow sweeps that were launched without one.
+__global__ void swap_kernel(Dev d, uint32_t sweep) { swap_event(d, blockIdx.x, sweep); }
+
+// ---------------------------------------------------------------------------
+// a8 helper.  N_max = max_k N_k of the configuration in packed words sp[W]
+// (Eq. 10).  All threads call; result valid in thread 0.
+// s_cnt: 16 ints of shared memory.
+// ---------------------------------------------------------------------------
+__device__ inline int count_nmax(const uint32_t* sp, int W, int q, int* s_cnt) {
+    if (threadIdx.x < 16) s_cnt[threadIdx.x] = 0;
+    __syncthreads();
+    for (int w = threadIdx.x; w < W; w += blockDim.x) {
+        const uint32_t word = sp[w];
+        for (int k = 0; k < q; ++k) {
+            const int c = __popc(match_nibbles(word, (uint32_t)k));
+            if (c) atomicAdd(&s_cnt[k], c);
+        }
+    }
+    __syncthreads();
+    int nmax = 0;
+    if (threadIdx.x == 0)
+        for (int k = 0; k < q; ++k) nmax = max(nmax, s_cnt[k]);
+    return nmax;
+}
+
+// Per-launch accumulators kept by thread 0 of a sweep CTA.
+struct ObsAcc {
+    long long n = 0, sE = 0, sN = 0, sN2 = 0, acc = 0, att = 0;
+    unsigned long long e2lo = 0;
+    long long e2hi = 0;
+    __device__ void sample(long long E, int nmax) {
+        n += 1; sE += E; sN += nmax; sN2 += (long long)nmax * nmax;
+        add_square_128(e2lo, e2hi, E);
+    }
+    __device__ void flush(pt_obs* o) const {
+        o->n_samples += n; o->sum_E += sE; o->sum_Nmax += sN; o->sum_Nmax2 += sN2;
+        o->flip_attempts += att; o->flip_accepts += acc;
+        const unsigned long long nlo = o->sum_E2_lo + e2lo;
+        o->sum_E2_hi = (long long)((unsigned long long)o->sum_E2_hi + (unsigned long long)e2hi +
+                                   (nlo < e2lo ? 1ull : 0ull));
+        o->sum_E2_lo = nlo;
+    }
+};
+
+// ---------------------------------------------------------------------------
+// I/O kernels (slot order outside, storage order inside).
+// ---------------------------------------------------------------------------
+__global__ void unpack_spins_kernel(Dev d, uint8_t* __restrict__ out) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)d.n_ens * d.n_rep * d.W;
+    if (gid >= total) return;
+    const int w = (int)(gid % d.W);
+    const int x = (int)(gid / d.W);  // e*n_rep + slot
+    const int e = x / d.n_rep;
+    const int st = d.perm[x];
+    const uint32_t word = d.spins[((size_t)e * d.n_rep + st) * d.W + w];
+    uint8_t* o = out + (size_t)x * d.L + 8 * w;
+#pragma unroll
+    for (int n = 0; n < 8; ++n) o[n] = (uint8_t)(((word >> (4 * n)) & 15u) + 1u);  // A4: API colours 1..q
+}
+
+__global__ void check_spins_kernel(Dev d, const uint8_t* __restrict__ in, int* __restrict__ bad) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)d.n_ens * d.n_rep * d.L;
+    if (gid >= total) return;
+    const int v = in[gid];
+    if (v < 1 || v > d.q) atomicOr(bad, 1);
+}
+
+__global__ void pack_spins_kernel(Dev d, const uint8_t* __restrict__ in) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = (long long)d.n_ens * d.n_rep * d.W;
+    if (gid >= total) return;
+    const int w = (int)(gid % d.W);
+    const int x = (int)(gid / d.W);
+    const int e = x / d.n_rep;
+    const int st = d.perm[x];
+    const uint8_t* s = in + (size_t)x * d.L + 8 * w;
+    uint32_t word = 0;
+#pragma unroll
+    for (int n = 0; n < 8; ++n) word |= (uint32_t)(s[n] - 1) << (4 * n);
+    d.spins[((size_t)e * d.n_rep + st) * d.W + w] = word;
+}
+
+// out[e][slot] = in[e][perm[e][slot]]
+__global__ void gather_slots_kernel(Dev d, const long long* __restrict__ in, long long* __restrict__ out) {
+    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= d.n_ens * d.n_rep) return;
+    const int e = gid / d.n_rep;
+    out[gid] = in[(size_t)e * d.n_rep + d.perm[gid]];
+}
+
+}  // namespace ptk

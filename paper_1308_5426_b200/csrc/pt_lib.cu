@@ -1,0 +1,402 @@
+// pt_lib.cu -- host side of libpt (C ABI in include/pt.h) for sm_100a.
+// Validates arguments, owns the device state of a context and enqueues the
+// kernels of pt_kernels.cuh / pt_sweep_*.cuh.  There is no CPU fallback: every
+// step of the path (J* table, hot start, energies, sweeps, swaps, observables)
+// runs in the kernels; without a CUDA device every call fails with PT_ECUDA.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "pt.h"
+#include "pt_kernels.cuh"
+#include "pt_sweep_direct.cuh"
+#include "pt_sweep_field.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string& msg) {
+    g_err = msg;
+    return code;
+}
+
+#define PT_CUDA(call)                                                                      \
+    do {                                                                                   \
+        cudaError_t err__ = (call);                                                        \
+        if (err__ != cudaSuccess)                                                          \
+            return fail(err__ == cudaErrorMemoryAllocation ? PT_ENOMEM : PT_ECUDA,         \
+                        std::string(#call) + ": " + cudaGetErrorString(err__));            \
+    } while (0)
+
+constexpr size_t kSmemLimit = 227 * 1024;  // per CTA on sm_100
+
+}  // namespace
+
+struct pt_ctx {
+    int L = 0, q = 0, n_ens = 0, n_rep = 0, ens_base = 0;
+    double sigma = 0;
+    uint64_t seed = 0;
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int variant = PT_VARIANT_FIELD;
+    bool fields_valid = false;
+    int64_t sweep = 0;
+    int32_t* d_Jq = nullptr;
+    uint32_t* d_Jpair = nullptr;
+    double* d_beta = nullptr;
+    double* d_scale = nullptr;
+    uint32_t* d_spins = nullptr;
+    long long* d_E = nullptr;
+    long long* d_Etmp = nullptr;
+    long long* d_Eout = nullptr;
+    int* d_perm = nullptr;
+    pt_obs* d_obs = nullptr;
+    int32_t* d_h = nullptr;
+    unsigned* d_done = nullptr;
+    int* d_flag = nullptr;
+
+    int R() const { return n_ens * n_rep; }
+    ptk::Dev dev() const {
+        ptk::Dev d;
+        d.L = L; d.W = L / 8; d.q = q; d.n_ens = n_ens; d.n_rep = n_rep; d.ens_base = ens_base;
+        d.key0 = (uint32_t)seed; d.key1 = (uint32_t)(seed >> 32);
+        d.Jq = d_Jq; d.Jpair = d_Jpair; d.beta = d_beta; d.thr_scale = d_scale;
+        d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done;
+        return d;
+    }
+};
+
+namespace {
+
+bool field_fits(int L, int q) { return ptk::field_smem_bytes(L, q) + 256 <= kSmemLimit; }
+bool direct_applies(int L, int q) { return ptk::direct_applies(L, q); }
+
+void free_ctx(pt_ctx* c) {
+    if (!c) return;
+    cudaFree(c->d_Jq); cudaFree(c->d_Jpair); cudaFree(c->d_beta); cudaFree(c->d_scale);
+    cudaFree(c->d_spins); cudaFree(c->d_E); cudaFree(c->d_Etmp); cudaFree(c->d_Eout);
+    cudaFree(c->d_perm); cudaFree(c->d_obs); cudaFree(c->d_h); cudaFree(c->d_done); cudaFree(c->d_flag);
+    delete c;
+}
+
+int recompute_energy(pt_ctx* c, long long* d_out) {
+    const size_t smem = (size_t)(c->L + c->L / 8) * 4;
+    if (smem > 48 * 1024)
+        PT_CUDA(cudaFuncSetAttribute(ptk::energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ptk::energy_kernel<<<c->R(), 256, smem, c->stream>>>(c->dev(), d_out);
+    PT_CUDA(cudaGetLastError());
+    return PT_OK;
+}
+
+int ensure_fields(pt_ctx* c) {
+    if (c->fields_valid) return PT_OK;
+    if (!c->d_h) PT_CUDA(cudaMalloc(&c->d_h, (size_t)c->R() * c->q * c->L * sizeof(int32_t)));
+    const size_t smem = (size_t)(c->L + c->L / 8) * 4;
+    if (smem > 48 * 1024)
+        PT_CUDA(cudaFuncSetAttribute(ptk::build_fields_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    ptk::build_fields_kernel<<<c->R(), 256, smem, c->stream>>>(c->dev());
+    PT_CUDA(cudaGetLastError());
+    c->fields_valid = true;
+    return PT_OK;
+}
+
+int resolve_variant(int L, int q, int variant, int* out) {
+    if (variant == PT_VARIANT_AUTO) variant = direct_applies(L, q) ? PT_VARIANT_DIRECT : PT_VARIANT_FIELD;
+    if (variant == PT_VARIANT_DIRECT) {
+        if (!direct_applies(L, q)) return fail(PT_EINVAL, "direct variant needs L % 32 == 0, L >= 64 and q <= 8");
+        if (ptk::direct_smem_bytes(L) + 256 > kSmemLimit)
+            return fail(PT_ECAPACITY, "direct variant does not fit in shared memory for this L");
+    } else if (variant == PT_VARIANT_FIELD) {
+        if (!field_fits(L, q)) return fail(PT_ECAPACITY, "local-field table (L*q*4 bytes) does not fit in shared memory");
+    } else {
+        return fail(PT_EINVAL, "unknown variant");
+    }
+    *out = variant;
+    return PT_OK;
+}
+
+// Enqueue one launch covering n_sweeps sweeps, optionally closed by a swap event.
+int launch_sweeps(pt_ctx* c, int n_sweeps, bool do_swap) {
+    const ptk::Dev d = c->dev();
+    if (c->variant == PT_VARIANT_FIELD) {
+        int rc = ensure_fields(c);
+        if (rc) return rc;
+        const size_t smem = ptk::field_smem_bytes(c->L, c->q);
+        PT_CUDA(cudaFuncSetAttribute(ptk::sweep_field_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        ptk::sweep_field_kernel<<<c->R(), ptk::FIELD_THREADS, smem, c->stream>>>(d, (long long)c->sweep, n_sweeps,
+                                                                                 do_swap ? 1 : 0);
+    } else {
+        c->fields_valid = false;
+        int rc = ptk::launch_sweep_direct(d, (long long)c->sweep, n_sweeps, do_swap ? 1 : 0, c->stream);
+        if (rc) return fail(PT_ECUDA, std::string("sweep_direct launch: ") + cudaGetErrorString((cudaError_t)rc));
+    }
+    PT_CUDA(cudaGetLastError());
+    c->sweep += n_sweeps;
+    return PT_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* pt_last_error(void) { return g_err.c_str(); }
+
+int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep, const double* betas,
+                 uint64_t seed, int ens_base) {
+    if (!out) return fail(PT_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (L < 8 || (L % 8) != 0) return fail(PT_EINVAL, "L must be >= 8 and a multiple of 8");
+    if (L > (1 << 20)) return fail(PT_EINVAL, "L too large");
+    if (q < 2 || q > 16) return fail(PT_EINVAL, "q must be in 2..16");
+    if (!(sigma > 0.0) || !std::isfinite(sigma)) return fail(PT_EINVAL, "sigma must be finite and > 0");
+    if (n_ens < 1 || n_rep < 1) return fail(PT_EINVAL, "n_ens and n_rep must be >= 1");
+    if ((long long)n_ens * n_rep > (1 << 24)) return fail(PT_EINVAL, "too many replicas");
+    if (ens_base < 0 || (long long)ens_base + n_ens > (1ll << 28)) return fail(PT_EINVAL, "ens_base out of range");
+    if (!betas) return fail(PT_EINVAL, "betas is NULL");
+    for (int t = 0; t < n_rep; ++t)
+        if (!(betas[t] >= 0.0) || !std::isfinite(betas[t])) return fail(PT_EINVAL, "betas must be finite and >= 0");
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(PT_ECUDA, "no CUDA device: libpt has no CPU path");
+    }
+    int dev = 0;
+    PT_CUDA(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    PT_CUDA(cudaGetDeviceProperties(&prop, dev));
+    if (prop.major != 10) return fail(PT_ECUDA, "libpt is built for sm_100a (B200) only");
+
+    int variant = 0;
+    {
+        int rc = resolve_variant(L, q, PT_VARIANT_AUTO, &variant);
+        if (rc) return rc;
+    }
+
+    pt_ctx* c = new (std::nothrow) pt_ctx;
+    if (!c) return fail(PT_ENOMEM, "host allocation failed");
+    c->L = L; c->q = q; c->sigma = sigma; c->n_ens = n_ens; c->n_rep = n_rep; c->seed = seed;
+    c->ens_base = ens_base; c->device = dev; c->variant = variant;
+    const int R = c->R();
+    const int W = L / 8;
+
+#define PT_CUDA_C(call)                                                                                   \
+    do {                                                                                                  \
+        cudaError_t err__ = (call);                                                                       \
+        if (err__ != cudaSuccess) {                                                                       \
+            free_ctx(c);                                                                                  \
+            return fail(err__ == cudaErrorMemoryAllocation ? PT_ENOMEM : PT_ECUDA,                        \
+                        std::string(#call) + ": " + cudaGetErrorString(err__));                           \
+        }                                                                                                 \
+    } while (0)
+
+    PT_CUDA_C(cudaMalloc(&c->d_Jq, (size_t)L * sizeof(int32_t)));
+    PT_CUDA_C(cudaMalloc(&c->d_Jpair, (size_t)2 * L * sizeof(uint32_t)));
+    PT_CUDA_C(cudaMalloc(&c->d_beta, (size_t)n_rep * sizeof(double)));
+    PT_CUDA_C(cudaMalloc(&c->d_scale, (size_t)n_rep * sizeof(double)));
+    PT_CUDA_C(cudaMalloc(&c->d_spins, (size_t)R * W * sizeof(uint32_t)));
+    PT_CUDA_C(cudaMalloc(&c->d_E, (size_t)R * sizeof(long long)));
+    PT_CUDA_C(cudaMalloc(&c->d_Etmp, (size_t)R * sizeof(long long)));
+    PT_CUDA_C(cudaMalloc(&c->d_Eout, (size_t)R * sizeof(long long)));
+    PT_CUDA_C(cudaMalloc(&c->d_perm, (size_t)R * sizeof(int)));
+    PT_CUDA_C(cudaMalloc(&c->d_obs, (size_t)R * sizeof(pt_obs)));
+    PT_CUDA_C(cudaMalloc(&c->d_done, (size_t)n_ens * sizeof(unsigned)));
+    PT_CUDA_C(cudaMalloc(&c->d_flag, sizeof(int)));
+    PT_CUDA_C(cudaMemset(c->d_obs, 0, (size_t)R * sizeof(pt_obs)));
+    PT_CUDA_C(cudaMemset(c->d_done, 0, (size_t)n_ens * sizeof(unsigned)));
+
+    std::vector<double> scale(n_rep);
+    for (int t = 0; t < n_rep; ++t) scale[t] = betas[t] > 0.0 ? 16777216.0 / betas[t] : INFINITY;
+    PT_CUDA_C(cudaMemcpy(c->d_beta, betas, (size_t)n_rep * sizeof(double), cudaMemcpyHostToDevice));
+    PT_CUDA_C(cudaMemcpy(c->d_scale, scale.data(), (size_t)n_rep * sizeof(double), cudaMemcpyHostToDevice));
+
+    // a1: couplings
+    ptk::jstar_kernel<<<(L / 2 + 128) / 128, 128>>>(L, sigma, c->d_Jq, nullptr);
+    PT_CUDA_C(cudaGetLastError());
+    std::vector<int32_t> Jq(L);
+    PT_CUDA_C(cudaMemcpy(Jq.data(), c->d_Jq, (size_t)L * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    long long rowsum = 0;
+    bool bad = false;
+    for (int r = 0; r < L; ++r) { rowsum += Jq[r]; bad |= Jq[r] < 0; }
+    if (bad || rowsum >= (1ll << 31)) {
+        free_ctx(c);
+        return fail(PT_EOVERFLOW, "sum_r Jq[r] >= 2^31: sigma too small for int32 energy differences");
+    }
+    ptk::pack_pairs_kernel<<<(L / 2 + 127) / 128, 128>>>(L, c->d_Jq, c->d_Jpair);
+    PT_CUDA_C(cudaGetLastError());
+
+    // a2: hot start, permutation, energies
+    const ptk::Dev d = c->dev();
+    const long long nwords = (long long)R * W;
+    ptk::init_spins_kernel<<<(unsigned)((nwords + 255) / 256), 256>>>(d);
+    PT_CUDA_C(cudaGetLastError());
+    ptk::init_perm_kernel<<<(R + 255) / 256, 256>>>(d);
+    PT_CUDA_C(cudaGetLastError());
+    {
+        int rc = recompute_energy(c, c->d_E);
+        if (rc) { free_ctx(c); return rc; }
+    }
+    PT_CUDA_C(cudaDeviceSynchronize());
+#undef PT_CUDA_C
+    *out = c;
+    return PT_OK;
+}
+
+int pt_create(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep, const double* betas,
+              uint64_t seed) {
+    return pt_create_ex(out, L, q, sigma, n_ens, n_rep, betas, seed, 0);
+}
+
+void pt_destroy(pt_ctx* ctx) {
+    if (!ctx) return;
+    cudaStreamSynchronize(ctx->stream);
+    free_ctx(ctx);
+}
+
+int pt_sweeps_async(pt_ctx* c, int64_t n, int swap_every, int64_t* n_launches) {
+    if (!c) return fail(PT_EINVAL, "ctx is NULL");
+    if (n < 0 || swap_every < 0) return fail(PT_EINVAL, "n and swap_every must be >= 0");
+    int64_t launches = 0;
+    constexpr int64_t kMaxChunk = 1 << 16;  // sweeps per launch when no swap event intervenes
+    while (n > 0) {
+        int64_t chunk = n < kMaxChunk ? n : kMaxChunk;
+        bool do_swap = false;
+        if (swap_every > 0) {
+            const int64_t to_event = swap_every - (c->sweep % swap_every);
+            if (to_event <= chunk) { chunk = to_event; do_swap = true; }
+        }
+        int rc = launch_sweeps(c, (int)chunk, do_swap);
+        if (rc) return rc;
+        launches += 1;
+        n -= chunk;
+    }
+    if (n_launches) *n_launches = launches;
+    return PT_OK;
+}
+
+int pt_sync(pt_ctx* c) {
+    if (!c) return fail(PT_EINVAL, "ctx is NULL");
+    PT_CUDA(cudaStreamSynchronize(c->stream));
+    PT_CUDA(cudaGetLastError());
+    return PT_OK;
+}
+
+int pt_sweeps(pt_ctx* c, int64_t n, int swap_every) {
+    int rc = pt_sweeps_async(c, n, swap_every, nullptr);
+    if (rc) return rc;
+    return pt_sync(c);
+}
+
+int pt_energy_dev(pt_ctx* c, int64_t* E_out_dev, int recompute) {
+    if (!c || !E_out_dev) return fail(PT_EINVAL, "NULL argument");
+    const long long* src = c->d_E;
+    if (recompute) {
+        int rc = recompute_energy(c, c->d_Etmp);
+        if (rc) return rc;
+        src = c->d_Etmp;
+    }
+    ptk::gather_slots_kernel<<<(c->R() + 255) / 256, 256, 0, c->stream>>>(c->dev(), src, (long long*)E_out_dev);
+    PT_CUDA(cudaGetLastError());
+    return pt_sync(c);
+}
+
+int pt_energy(pt_ctx* c, int64_t* E_out, int recompute) {
+    if (!c || !E_out) return fail(PT_EINVAL, "NULL argument");
+    int rc = pt_energy_dev(c, (int64_t*)c->d_Eout, recompute);
+    if (rc) return rc;
+    PT_CUDA(cudaMemcpy(E_out, c->d_Eout, (size_t)c->R() * sizeof(int64_t), cudaMemcpyDeviceToHost));
+    return PT_OK;
+}
+
+int pt_observables(pt_ctx* c, pt_obs* out) {
+    if (!c || !out) return fail(PT_EINVAL, "NULL argument");
+    int rc = pt_sync(c);
+    if (rc) return rc;
+    PT_CUDA(cudaMemcpy(out, c->d_obs, (size_t)c->R() * sizeof(pt_obs), cudaMemcpyDeviceToHost));
+    for (int x = 0; x < c->R(); ++x) out[x].near_ties = -1;
+    return PT_OK;
+}
+
+int pt_get_spins_dev(pt_ctx* c, uint8_t* out_dev) {
+    if (!c || !out_dev) return fail(PT_EINVAL, "NULL argument");
+    const long long nwords = (long long)c->R() * (c->L / 8);
+    ptk::unpack_spins_kernel<<<(unsigned)((nwords + 255) / 256), 256, 0, c->stream>>>(c->dev(), out_dev);
+    PT_CUDA(cudaGetLastError());
+    return pt_sync(c);
+}
+
+int pt_get_spins(pt_ctx* c, uint8_t* out) {
+    if (!c || !out) return fail(PT_EINVAL, "NULL argument");
+    const size_t n = (size_t)c->R() * c->L;
+    uint8_t* tmp = nullptr;
+    PT_CUDA(cudaMalloc(&tmp, n));
+    int rc = pt_get_spins_dev(c, tmp);
+    if (rc == PT_OK) {
+        cudaError_t err = cudaMemcpy(out, tmp, n, cudaMemcpyDeviceToHost);
+        if (err != cudaSuccess) rc = fail(PT_ECUDA, cudaGetErrorString(err));
+    }
+    cudaFree(tmp);
+    return rc;
+}
+
+int pt_set_spins(pt_ctx* c, const uint8_t* in) {
+    if (!c || !in) return fail(PT_EINVAL, "NULL argument");
+    const size_t n = (size_t)c->R() * c->L;
+    uint8_t* tmp = nullptr;
+    PT_CUDA(cudaMalloc(&tmp, n));
+    int rc = PT_OK;
+    do {
+        cudaError_t err = cudaMemcpyAsync(tmp, in, n, cudaMemcpyHostToDevice, c->stream);
+        if (err == cudaSuccess) err = cudaMemsetAsync(c->d_flag, 0, sizeof(int), c->stream);
+        if (err != cudaSuccess) { rc = fail(PT_ECUDA, cudaGetErrorString(err)); break; }
+        ptk::check_spins_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->dev(), tmp, c->d_flag);
+        int flag = 0;
+        err = cudaMemcpyAsync(&flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+        if (err == cudaSuccess) err = cudaStreamSynchronize(c->stream);
+        if (err != cudaSuccess) { rc = fail(PT_ECUDA, cudaGetErrorString(err)); break; }
+        if (flag) { rc = fail(PT_EINVAL, "colour outside 1..q"); break; }
+        const long long nwords = (long long)c->R() * (c->L / 8);
+        ptk::pack_spins_kernel<<<(unsigned)((nwords + 255) / 256), 256, 0, c->stream>>>(c->dev(), tmp);
+        c->fields_valid = false;
+        rc = recompute_energy(c, c->d_E);
+        if (rc) break;
+        rc = pt_sync(c);
+    } while (0);
+    cudaFree(tmp);
+    return rc;
+}
+
+int pt_get_couplings(pt_ctx* c, int32_t* Jq) {
+    if (!c || !Jq) return fail(PT_EINVAL, "NULL argument");
+    PT_CUDA(cudaMemcpy(Jq, c->d_Jq, (size_t)c->L * sizeof(int32_t), cudaMemcpyDeviceToHost));
+    return PT_OK;
+}
+
+int64_t pt_sweep_counter(pt_ctx* c) { return c ? c->sweep : -1; }
+
+int pt_set_variant(pt_ctx* c, int variant) {
+    if (!c) return fail(PT_EINVAL, "ctx is NULL");
+    int v = 0;
+    int rc = resolve_variant(c->L, c->q, variant, &v);
+    if (rc) return rc;
+    c->variant = v;
+    return PT_OK;
+}
+
+int pt_get_variant(pt_ctx* c) { return c ? c->variant : PT_EINVAL; }
+
+int pt_set_stream(pt_ctx* c, void* cuda_stream) {
+    if (!c) return fail(PT_EINVAL, "ctx is NULL");
+    PT_CUDA(cudaStreamSynchronize(c->stream));
+    c->stream = (cudaStream_t)cuda_stream;
+    return PT_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,138 @@
+// pt_sweep_field.cuh -- Metropolis sweep, local-field variant (north_star (3)).
+//
+// One CTA per replica.  Shared memory holds the couplings Jq[L], the packed
+// spins, the per-colour local fields h[k][i] = sum_{j!=i} Jq[|i-j|][c_j==k]
+// (colour-major, so that consecutive threads update consecutive banks), and
+// for the running sweep the proposed colours and integer acceptance
+// thresholds of all sites.  Because the generator is counter based and every
+// site is visited once per sweep, proposal b_i and threshold theta_i of every
+// site are known at the start of the sweep and are drawn by all threads in
+// parallel; the sequential part of Eq. 8 is then
+//   dE_i = h[a_i][i] - h[b_i][i]  (energy of the changed spin
+//   before and after),   accept iff dE_i <= theta_i,
+// which warp 0 evaluates for 32 consecutive sites at once against the current
+// fields: the first accepting lane is THE next accepted step of the sequential
+// sweep (all sites before it reject against exactly these fields).  The whole
+// CTA then applies it: h[a][j] -= Jq[|j-f|], h[b][j] += Jq[|j-f|] for all j,
+// and the scan resumes behind it.  Results are identical to the site-by-site
+// order because all arithmetic is integer.
+#pragma once
+#include "pt_kernels.cuh"
+
+namespace ptk {
+
+constexpr int FIELD_THREADS = 512;
+
+// dynamic smem layout (32-bit words): J[L] | theta[L] | sp[W] | bq[W] | h[q*L]
+__host__ __device__ inline size_t field_smem_bytes(int L, int q) {
+    return (size_t)(2 * L + 2 * (L / 8) + q * L) * 4;
+}
+
+__global__ void __launch_bounds__(FIELD_THREADS, 1)
+sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
+    extern __shared__ uint32_t smem_f[];
+    const int L = d.L, W = d.W, q = d.q;
+    int32_t* J = (int32_t*)smem_f;
+    int32_t* theta = J + L;
+    uint32_t* sp = (uint32_t*)(theta + L);
+    uint32_t* bq = sp + W;
+    int32_t* h = (int32_t*)(bq + W);
+    __shared__ int s_flip[4];
+    __shared__ int s_cnt[16];
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int e = blockIdx.x / d.n_rep, t = blockIdx.x % d.n_rep;
+    const int st = d.perm[blockIdx.x];
+    const size_t x = (size_t)e * d.n_rep + st;
+    uint32_t* g_sp = d.spins + x * W;
+    int32_t* g_h = d.h + x * (size_t)q * L;
+
+    for (int r = tid; r < L; r += FIELD_THREADS) J[r] = d.Jq[r];
+    for (int w = tid; w < W; w += FIELD_THREADS) sp[w] = g_sp[w];
+    for (int k = tid; k < q * L; k += FIELD_THREADS) h[k] = g_h[k];
+    long long E = d.E[x];
+    const double scale = d.thr_scale[t];
+    const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_SWEEP;
+    ObsAcc oa;
+    __syncthreads();
+
+    for (int s = 0; s < n_sweeps; ++s) {
+        const uint32_t sweep = (uint32_t)(sweep0 + s + 1);
+        // proposals and thresholds of all sites (A6, A7, A9), one word of 8 sites per thread
+        for (int w = tid; w < W; w += FIELD_THREADS) {
+            const uint32_t word = sp[w];
+            uint32_t bword = 0;
+#pragma unroll
+            for (int n = 0; n < 8; ++n) {
+                const int i = 8 * w + n;
+                const Philox4 p = philox4x32_10((uint32_t)i, sweep, (uint32_t)t, c3, d.key0, d.key1);
+                const uint32_t a = (word >> (4 * n)) & 15u;
+                const uint32_t k = __umulhi(p.w0, (uint32_t)(q - 1));
+                const uint32_t b = k + (k >= a ? 1u : 0u);
+                bword |= b << (4 * n);
+                theta[i] = accept_threshold(uniform53(p.w1, p.w2), scale);
+            }
+            bq[w] = bword;
+        }
+        __syncthreads();
+
+        int pos = 0;
+        while (true) {
+            if (warp == 0) {
+                int f = L, fa = 0, fb = 0, fdE = 0;
+                for (int base = pos; base < L; base += 32) {
+                    const int i = base + lane;
+                    int a = 0, b = 0, dE = 0;
+                    bool acc = false;
+                    if (i < L) {
+                        a = get_nibble(sp, i);
+                        b = get_nibble(bq, i);
+                        dE = h[a * L + i] - h[b * L + i];
+                        acc = dE <= theta[i];
+                    }
+                    const unsigned m = __ballot_sync(0xffffffffu, acc);
+                    if (m) {
+                        const int src = __ffs(m) - 1;
+                        f = base + src;
+                        fa = __shfl_sync(0xffffffffu, a, src);
+                        fb = __shfl_sync(0xffffffffu, b, src);
+                        fdE = __shfl_sync(0xffffffffu, dE, src);
+                        break;
+                    }
+                }
+                if (lane == 0) { s_flip[0] = f; s_flip[1] = fa; s_flip[2] = fb; s_flip[3] = fdE; }
+            }
+            __syncthreads();
+            const int f = s_flip[0];
+            if (f >= L) break;
+            const int a = s_flip[1], b = s_flip[2];
+            int32_t* ha = h + a * L;
+            int32_t* hb = h + b * L;
+            for (int j = tid; j < L; j += FIELD_THREADS) {
+                const int dist = j > f ? j - f : f - j;
+                const int32_t Jv = J[dist];  // J[0] = 0: the site's own field is unchanged
+                ha[j] -= Jv;
+                hb[j] += Jv;
+            }
+            if (tid == 0) {
+                const int sh = (f & 7) << 2;
+                sp[f >> 3] = (sp[f >> 3] & ~(15u << sh)) | ((uint32_t)b << sh);
+                E += s_flip[3];
+                oa.acc += 1;
+            }
+            pos = f + 1;
+            __syncthreads();
+        }
+        // a8: sample after the sweep, before the swap event (A15)
+        const int nmax = count_nmax(sp, W, q, s_cnt);
+        if (tid == 0) { oa.att += L; oa.sample(E, nmax); }
+        __syncthreads();
+    }
+
+    for (int w = tid; w < W; w += FIELD_THREADS) g_sp[w] = sp[w];
+    for (int k = tid; k < q * L; k += FIELD_THREADS) g_h[k] = h[k];
+    if (tid == 0) { d.E[x] = E; oa.flush(d.obs + blockIdx.x); }
+    if (do_swap) arrive_and_swap(d, e, (uint32_t)(sweep0 + n_sweeps));
+}
+
+}  // namespace ptk

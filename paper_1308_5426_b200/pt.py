@@ -1,0 +1,195 @@
+"""Thin ctypes binding of libpt.so (include/pt.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI.  There is no
+CPU fallback: a missing libpt.so raises at import, a missing GPU raises PTError
+(PT_ECUDA) from pt_create.  PyTorch, when importable, supplies the CUDA stream
+(`PT.use_torch_stream`) and device buffers for the *_dev calls.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpt.so")
+
+VARIANT_AUTO, VARIANT_FIELD, VARIANT_DIRECT = 0, 1, 2
+_VARIANTS = {"auto": VARIANT_AUTO, "field": VARIANT_FIELD, "direct": VARIANT_DIRECT}
+STATUS = {0: "PT_OK", -1: "PT_EINVAL", -2: "PT_EOVERFLOW", -3: "PT_ENOMEM", -4: "PT_ECUDA", -5: "PT_ECAPACITY"}
+
+# every symbol include/pt.h declares
+SYMBOLS = ["pt_create", "pt_create_ex", "pt_destroy", "pt_sweeps", "pt_energy", "pt_energy_dev",
+           "pt_observables", "pt_get_spins", "pt_get_spins_dev", "pt_set_spins", "pt_get_couplings",
+           "pt_sweep_counter", "pt_set_variant", "pt_get_variant", "pt_set_stream", "pt_sweeps_async",
+           "pt_sync", "pt_last_error"]
+
+
+class PTError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("%s (%d): %s" % (STATUS.get(code, "?"), code, msg))
+        self.code = code
+
+
+class Obs(ctypes.Structure):  # pt_obs
+    _fields_ = [("n_samples", ctypes.c_int64), ("sum_E", ctypes.c_int64),
+                ("sum_E2_lo", ctypes.c_uint64), ("sum_E2_hi", ctypes.c_int64),
+                ("sum_Nmax", ctypes.c_int64), ("sum_Nmax2", ctypes.c_int64),
+                ("flip_attempts", ctypes.c_int64), ("flip_accepts", ctypes.c_int64),
+                ("swap_attempts", ctypes.c_int64), ("swap_accepts", ctypes.c_int64),
+                ("near_ties", ctypes.c_int64)]
+
+
+OBS_FIELDS = [f[0] for f in Obs._fields_]
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError("libpt.so is not built (run `python -m paper_1308_5426_b200.build`); "
+                      "there is no CPU fallback")
+
+_lib = ctypes.CDLL(LIB_PATH)
+_vp, _i32, _i64, _u64, _dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_uint64, ctypes.c_double
+_lib.pt_create.argtypes = [ctypes.POINTER(_vp), _i32, _i32, _dbl, _i32, _i32, _vp, _u64]
+_lib.pt_create_ex.argtypes = [ctypes.POINTER(_vp), _i32, _i32, _dbl, _i32, _i32, _vp, _u64, _i32]
+_lib.pt_destroy.argtypes = [_vp]
+_lib.pt_destroy.restype = None
+_lib.pt_sweeps.argtypes = [_vp, _i64, _i32]
+_lib.pt_sweeps_async.argtypes = [_vp, _i64, _i32, ctypes.POINTER(_i64)]
+_lib.pt_sync.argtypes = [_vp]
+_lib.pt_energy.argtypes = [_vp, _vp, _i32]
+_lib.pt_energy_dev.argtypes = [_vp, _vp, _i32]
+_lib.pt_observables.argtypes = [_vp, _vp]
+_lib.pt_get_spins.argtypes = [_vp, _vp]
+_lib.pt_get_spins_dev.argtypes = [_vp, _vp]
+_lib.pt_set_spins.argtypes = [_vp, _vp]
+_lib.pt_get_couplings.argtypes = [_vp, _vp]
+_lib.pt_sweep_counter.argtypes = [_vp]
+_lib.pt_sweep_counter.restype = _i64
+_lib.pt_set_variant.argtypes = [_vp, _i32]
+_lib.pt_get_variant.argtypes = [_vp]
+_lib.pt_set_stream.argtypes = [_vp, _vp]
+_lib.pt_last_error.restype = ctypes.c_char_p
+
+
+def _check(rc):
+    if rc != 0:
+        raise PTError(rc, (_lib.pt_last_error() or b"").decode())
+
+
+def _p(a):
+    return a.ctypes.data_as(_vp)
+
+
+class PT:
+    """One libpt context: n_ens ensembles x n_rep replicas of the (L, q, sigma) model."""
+
+    def __init__(self, L, q, sigma, n_ens, n_rep, betas, seed, ens_base=0, variant="auto"):
+        b = np.ascontiguousarray(betas, dtype=np.float64)
+        if b.ndim != 1 or b.shape[0] != n_rep:
+            raise ValueError("betas must have n_rep entries")
+        self.L, self.q, self.n_ens, self.n_rep = int(L), int(q), int(n_ens), int(n_rep)
+        self.betas = b
+        self._h = _vp()
+        _check(_lib.pt_create_ex(ctypes.byref(self._h), int(L), int(q), float(sigma), int(n_ens), int(n_rep),
+                                 _p(b), int(seed) & 0xFFFFFFFFFFFFFFFF, int(ens_base)))
+        if variant != "auto":
+            self.set_variant(variant)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.pt_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    # -- the calls of include/pt.h ------------------------------------------------
+    def sweeps(self, n, swap_every=1):
+        _check(_lib.pt_sweeps(self._h, int(n), int(swap_every)))
+
+    def sweeps_async(self, n, swap_every=1):
+        k = _i64(0)
+        _check(_lib.pt_sweeps_async(self._h, int(n), int(swap_every), ctypes.byref(k)))
+        return k.value
+
+    def sync(self):
+        _check(_lib.pt_sync(self._h))
+
+    def energy(self, recompute=False):
+        E = np.zeros((self.n_ens, self.n_rep), dtype=np.int64)
+        _check(_lib.pt_energy(self._h, _p(E), int(bool(recompute))))
+        return E
+
+    def energy_dev(self, out, recompute=False):
+        """out: torch int64 CUDA tensor with n_ens*n_rep elements (device pointer passed through)."""
+        assert out.is_cuda and out.numel() == self.n_ens * self.n_rep and out.element_size() == 8
+        _check(_lib.pt_energy_dev(self._h, ctypes.c_void_p(out.data_ptr()), int(bool(recompute))))
+        return out
+
+    def observables(self):
+        arr = (Obs * (self.n_ens * self.n_rep))()
+        _check(_lib.pt_observables(self._h, ctypes.byref(arr)))
+        out = {}
+        for name in OBS_FIELDS:
+            dt = np.uint64 if name == "sum_E2_lo" else np.int64
+            out[name] = np.array([getattr(o, name) for o in arr], dtype=dt).reshape(self.n_ens, self.n_rep)
+        return out
+
+    def get_spins(self):
+        s = np.zeros((self.n_ens, self.n_rep, self.L), dtype=np.uint8)
+        _check(_lib.pt_get_spins(self._h, _p(s)))
+        return s
+
+    def get_spins_dev(self, out):
+        assert out.is_cuda and out.numel() == self.n_ens * self.n_rep * self.L and out.element_size() == 1
+        _check(_lib.pt_get_spins_dev(self._h, ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    def set_spins(self, spins):
+        s = np.ascontiguousarray(spins, dtype=np.uint8)
+        if s.size != self.n_ens * self.n_rep * self.L:
+            raise ValueError("spins must have n_ens*n_rep*L entries")
+        _check(_lib.pt_set_spins(self._h, _p(s)))
+
+    def get_couplings(self):
+        J = np.zeros(self.L, dtype=np.int32)
+        _check(_lib.pt_get_couplings(self._h, _p(J)))
+        return J
+
+    def sweep_counter(self):
+        return int(_lib.pt_sweep_counter(self._h))
+
+    def set_variant(self, variant):
+        _check(_lib.pt_set_variant(self._h, _VARIANTS[variant] if isinstance(variant, str) else int(variant)))
+
+    def get_variant(self):
+        v = _lib.pt_get_variant(self._h)
+        return {VARIANT_FIELD: "field", VARIANT_DIRECT: "direct"}.get(v, str(v))
+
+    def set_stream(self, cuda_stream_ptr):
+        _check(_lib.pt_set_stream(self._h, ctypes.c_void_p(int(cuda_stream_ptr) if cuda_stream_ptr else None)))
+
+    def use_torch_stream(self, stream=None):
+        """Run this context's kernels on a torch.cuda stream (default: the current one)."""
+        import torch
+        s = stream if stream is not None else torch.cuda.current_stream()
+        self.set_stream(s.cuda_stream)
+        return s
+
+
+def derived(obs, L, q):
+    """<E>/L, <M>, <M^2> from the integer accumulators (one fixed fp64 formula; Eq. 10)."""
+    n = obs["n_samples"].astype(np.float64)
+    e = obs["sum_E"].astype(np.float64) / (n * L * 16777216.0)
+    m1 = obs["sum_Nmax"].astype(np.float64) / (n * L)
+    m2 = obs["sum_Nmax2"].astype(np.float64) / (n * float(L) * float(L))
+    M = (q * m1 - 1.0) / (q - 1.0)
+    M2 = (q * q * m2 - 2.0 * q * m1 + 1.0) / ((q - 1.0) ** 2)
+    return {"E_per_spin": e, "M": M, "M2": M2}

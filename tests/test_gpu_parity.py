@@ -1,0 +1,215 @@
+"""GPU parity: libpt (through the C ABI binding) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): spins and integer energies bit-identical, all integer
+accumulators identical, oracle near-tie count 0 (so the integer-threshold form of Eq. 8,
+reading A9, provably takes the same decisions).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1308_5426_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+THREADS = max(1, min(32, os.cpu_count() or 1))
+FULL = os.environ.get("PT_FULL", "0") == "1"
+CMP_FIELDS = ["n_samples", "sum_E", "sum_E2_lo", "sum_E2_hi", "sum_Nmax", "sum_Nmax2",
+              "flip_attempts", "flip_accepts", "swap_attempts", "swap_accepts"]
+
+
+@pytest.fixture(scope="module")
+def pt():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test on a box without CUDA")
+    from paper_1308_5426_b200 import pt as ptmod
+    return ptmod
+
+
+def assert_same_state(g, o, what):
+    np.testing.assert_array_equal(g.get_spins(), o.get_spins(), err_msg=what + ": spins")
+    np.testing.assert_array_equal(g.energy(), o.energy(), err_msg=what + ": running E")
+    np.testing.assert_array_equal(g.energy(recompute=True), o.energy(recompute=True), err_msg=what + ": recounted E")
+    go, oo = g.observables(), o.observables()
+    for f in CMP_FIELDS:
+        np.testing.assert_array_equal(go[f], oo[f], err_msg=what + ": " + f)
+    assert int(oo["near_ties"].sum()) == 0, what + ": oracle saw near-ties, threshold form not guaranteed"
+    assert (go["near_ties"] == -1).all()
+
+
+def make_pair(pt, oracle, w, variant, n_ens=None):
+    b = inputs.betas(w)
+    ne = n_ens or w.n_ens
+    g = pt.PT(w.L, w.q, w.sigma, ne, w.n_rep, b, w.seed, variant=variant)
+    o = oracle.Oracle(w.L, w.q, w.sigma, ne, w.n_rep, b, w.seed)
+    return g, o
+
+
+@pytest.mark.parametrize("L,sigma", [(8, 0.5), (64, 0.5), (256, 0.4), (1024, 0.8), (4096, 0.3), (2048, 0.1),
+                                     (2048, 1.0), (200, 0.37)])
+def test_couplings_equal_oracle(pt, oracle, L, sigma):
+    g = pt.PT(L, 3, sigma, 1, 1, [1.0], 1, variant="field" if L * 3 * 4 < 200000 else "auto")
+    np.testing.assert_array_equal(g.get_couplings(), oracle.couplings(L, sigma))
+    g.close()
+
+
+@pytest.mark.parametrize("variant", ["field", "direct"])
+def test_cfg0_full(pt, oracle, variant):
+    w = inputs.config(0)
+    g, o = make_pair(pt, oracle, w, variant)
+    assert g.get_variant() == variant
+    assert_same_state(g, o, "cfg0 start")
+    done = 0
+    for n in (1, 2, 7, 90, 900):  # call splitting must not matter (A10)
+        g.sweeps(n, w.swap_every)
+        o.sweeps(n, w.swap_every)
+        done += n
+        assert g.sweep_counter() == done
+        assert_same_state(g, o, "cfg0 %s after %d sweeps" % (variant, done))
+    assert int(o.observables()["swap_accepts"].sum()) > 0 and int(o.observables()["flip_accepts"].sum()) > 0
+
+
+@pytest.mark.parametrize("variant", ["field", "direct"])
+def test_cfg1_full_with_burn_in(pt, oracle, variant):
+    w = inputs.config(1)
+    g, o = make_pair(pt, oracle, w, variant)
+    g.sweeps(w.burn_in, w.swap_every)
+    o.sweeps(w.burn_in, w.swap_every, field=True, threads=THREADS)
+    assert_same_state(g, o, "cfg1 after burn-in")
+    g0, o0 = g.observables(), o.observables()
+    n = w.sweeps - w.burn_in
+    g.sweeps(n, w.swap_every)
+    o.sweeps(n, w.swap_every, field=True, threads=THREADS)
+    assert_same_state(g, o, "cfg1 end")
+    g1, o1 = g.observables(), o.observables()
+    dg = pt.derived({k: g1[k] - g0[k] for k in g1}, w.L, w.q)
+    do = pt.derived({k: o1[k] - o0[k] for k in o1}, w.L, w.q)
+    for k in dg:
+        np.testing.assert_allclose(dg[k], do[k], rtol=1e-12, atol=0)
+    # physics sanity (Table 1: T_c(q=3, sigma=0.4) = 2.085): ordered at T=1, disordered at T=3
+    assert dg["M"][0, 0] > 0.9 and dg["M"][0, -1] < 0.3
+
+
+@pytest.mark.parametrize("variant", ["field", "direct"])
+def test_cfg2_cold_half(pt, oracle, variant):
+    w = inputs.config(2)
+    g, o = make_pair(pt, oracle, w, variant)
+    start = inputs.cold_half_spins(w, o.get_spins())
+    g.set_spins(start)
+    o.set_spins(start)
+    assert_same_state(g, o, "cfg2 start")
+    n = w.sweeps if FULL else 1500
+    g.sweeps(n, w.swap_every)
+    o.sweeps(n, w.swap_every, field=True, threads=THREADS)
+    assert_same_state(g, o, "cfg2 after %d sweeps" % n)
+
+
+@pytest.mark.parametrize("variant", ["field", "direct"])
+def test_cfg3_first_sweeps(pt, oracle, variant):
+    """Headline configuration in the launch configuration bench.py times (one CTA per replica, swap every sweep)."""
+    w = inputs.config(3)
+    g, o = make_pair(pt, oracle, w, variant)
+    n = 12
+    g.sweeps(n, w.swap_every)
+    o.sweeps(n, w.swap_every, field=True, threads=THREADS)
+    assert_same_state(g, o, "cfg3 after %d sweeps" % n)
+
+
+@pytest.mark.parametrize("idx", [0, 9, 14, 25, 39])
+def test_cfg4_members_first_sweeps(pt, oracle, idx):
+    w = inputs.config4()[idx]
+    g, o = make_pair(pt, oracle, w, "auto")
+    g.sweeps(10, 1)
+    o.sweeps(10, 1, field=True, threads=THREADS)
+    assert_same_state(g, o, w.name)
+
+
+@pytest.mark.parametrize("variant", ["field", "direct"])
+@pytest.mark.parametrize("swap_every", [0, 1, 3])
+def test_ensembles_and_swap_period(pt, oracle, variant, swap_every):
+    L, q, sigma, n_ens, n_rep = 128, 4, 0.6, 3, 5   # odd replica count: last slot idles in stage 0 (A11)
+    b = inputs.geometric_betas(0.7, 2.2, n_rep)
+    g = pt.PT(L, q, sigma, n_ens, n_rep, b, 77, variant=variant)
+    o = oracle.Oracle(L, q, sigma, n_ens, n_rep, b, 77)
+    for n in (4, 5, 30):
+        g.sweeps(n, swap_every)
+        o.sweeps(n, swap_every)
+        assert_same_state(g, o, "ens/swap_every=%d" % swap_every)
+    s = g.get_spins()
+    assert not np.array_equal(s[0], s[1])  # different ensembles draw different streams
+
+
+def test_variants_can_be_switched_mid_run(pt, oracle):
+    w = inputs.config(0)
+    g, o = make_pair(pt, oracle, w, "field")
+    for k, v in enumerate(["direct", "field", "direct", "field"]):
+        g.set_variant(v)
+        g.sweeps(25 + k, 1)
+        o.sweeps(25 + k, 1)
+        assert_same_state(g, o, "switch to " + v)
+
+
+def test_ragged_and_edge_shapes(pt, oracle):
+    # L not a multiple of 32 or 64 (field variant only), q = 2 and q = 16, beta = 0, single replica
+    for (L, q, n_rep, betas) in [(8, 2, 1, [0.5]), (40, 16, 3, [0.0, 0.4, 1.5]), (200, 9, 4, [1.2, 0.9, 0.9, 0.1]),
+                                 (64, 8, 2, [2.0, 0.0])]:
+        g = pt.PT(L, q, 0.45, 2, n_rep, betas, 5)
+        o = oracle.Oracle(L, q, 0.45, 2, n_rep, betas, 5)
+        g.sweeps(40, 1)
+        o.sweeps(40, 1)
+        assert_same_state(g, o, "shape L=%d q=%d" % (L, q))
+
+
+def test_ens_base_shards_ensembles(pt, oracle):
+    """Two contexts with ens_base 0 and 2 reproduce ensembles 0-1 and 2-3 of one 4-ensemble context."""
+    L, q, n_rep = 64, 3, 4
+    b = inputs.geometric_betas(0.8, 2.0, n_rep)
+    whole = pt.PT(L, q, 0.5, 4, n_rep, b, 9)
+    lo = pt.PT(L, q, 0.5, 2, n_rep, b, 9, ens_base=0)
+    hi = pt.PT(L, q, 0.5, 2, n_rep, b, 9, ens_base=2)
+    for c in (whole, lo, hi):
+        c.sweeps(50, 1)
+    np.testing.assert_array_equal(whole.get_spins(), np.concatenate([lo.get_spins(), hi.get_spins()]))
+    np.testing.assert_array_equal(whole.energy(), np.concatenate([lo.energy(), hi.energy()]))
+
+
+def test_errors(pt):
+    with pytest.raises(pt.PTError) as ei:
+        pt.PT(12, 3, 0.5, 1, 1, [1.0], 1)
+    assert ei.value.code == -1
+    for bad in [dict(q=1), dict(q=17), dict(sigma=0.0), dict(sigma=float("nan")), dict(betas=[-1.0])]:
+        kw = dict(L=64, q=3, sigma=0.5, n_ens=1, n_rep=1, betas=[1.0], seed=1)
+        kw.update(bad)
+        with pytest.raises(pt.PTError):
+            pt.PT(**kw)
+    with pytest.raises(pt.PTError) as ei:
+        pt.PT(4096, 3, 0.001, 1, 1, [1.0], 1)   # couplings overflow int32 row sums
+    assert ei.value.code == -2
+    g = pt.PT(64, 3, 0.5, 1, 2, [1.0, 0.5], 1)
+    with pytest.raises(pt.PTError):
+        g.sweeps(-1, 1)
+    bad = np.full((1, 2, 64), 4, dtype=np.uint8)
+    before = g.get_spins()
+    with pytest.raises(pt.PTError):
+        g.set_spins(bad)
+    np.testing.assert_array_equal(g.get_spins(), before)
+    g2 = pt.PT(72, 3, 0.5, 1, 1, [1.0], 1)
+    with pytest.raises(pt.PTError):
+        g2.set_variant("direct")
+
+
+def test_dev_pointer_calls_and_torch_stream(pt):
+    import torch
+    w = inputs.config(0)
+    g = pt.PT(w.L, w.q, w.sigma, 1, w.n_rep, inputs.betas(w), w.seed)
+    s = torch.cuda.Stream()
+    g.use_torch_stream(s)
+    g.sweeps(20, 1)
+    E = torch.empty(w.n_rep, dtype=torch.int64, device="cuda")
+    sp = torch.empty(w.n_rep * w.L, dtype=torch.uint8, device="cuda")
+    g.energy_dev(E, recompute=True)
+    g.get_spins_dev(sp)
+    np.testing.assert_array_equal(E.cpu().numpy().reshape(1, -1), g.energy())
+    np.testing.assert_array_equal(sp.cpu().numpy().reshape(1, w.n_rep, w.L), g.get_spins())
