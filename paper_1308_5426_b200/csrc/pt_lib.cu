@@ -124,10 +124,12 @@ int resolve_variant(int L, int q, int variant, int* out) {
 
 // Enqueue one launch covering n_sweeps sweeps, optionally closed by a swap event.
 int launch_sweeps(pt_ctx* c, int n_sweeps, bool do_swap) {
-    const ptk::Dev d = c->dev();
     if (c->variant == PT_VARIANT_FIELD) {
         int rc = ensure_fields(c);
         if (rc) return rc;
+    }
+    const ptk::Dev d = c->dev();  // after ensure_fields: it may allocate d_h
+    if (c->variant == PT_VARIANT_FIELD) {
         const size_t smem = ptk::field_smem_bytes(c->L, c->q);
         PT_CUDA(cudaFuncSetAttribute(ptk::sweep_field_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ptk::sweep_field_kernel<<<c->R(), ptk::FIELD_THREADS, smem, c->stream>>>(d, (long long)c->sweep, n_sweeps,
