@@ -48,6 +48,7 @@ struct pt_ctx {
     int variant = PT_VARIANT_FIELD;
     bool fields_valid = false;
     int64_t sweep = 0;
+    int r_hi = 0;  // largest r <= L/2 with Jq[r] >= 2^16 (direct variant: reach of the high halves)
     int32_t* d_Jq = nullptr;
     uint32_t* d_Jpair = nullptr;
     double* d_beta = nullptr;
@@ -136,7 +137,7 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, bool do_swap) {
                                                                                  do_swap ? 1 : 0);
     } else {
         c->fields_valid = false;
-        int rc = ptk::launch_sweep_direct(d, (long long)c->sweep, n_sweeps, do_swap ? 1 : 0, c->stream);
+        int rc = ptk::launch_sweep_direct(d, (long long)c->sweep, n_sweeps, do_swap ? 1 : 0, c->r_hi, c->stream);
         if (rc) return fail(PT_ECUDA, std::string("sweep_direct launch: ") + cudaGetErrorString((cudaError_t)rc));
     }
     PT_CUDA(cudaGetLastError());
@@ -227,6 +228,8 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
     long long rowsum = 0;
     bool bad = false;
     for (int r = 0; r < L; ++r) { rowsum += Jq[r]; bad |= Jq[r] < 0; }
+    for (int r = 1; r <= L / 2; ++r)
+        if (Jq[r] >= 65536) c->r_hi = r;
     if (bad || rowsum >= (1ll << 31)) {
         free_ctx(c);
         return fail(PT_EOVERFLOW, "sum_r Jq[r] >= 2^31: sigma too small for int32 energy differences");
