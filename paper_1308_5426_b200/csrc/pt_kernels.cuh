@@ -24,6 +24,7 @@ struct Dev {
     pt_obs* obs;              // [n_ens][n_rep]     slot order
     int32_t* h;               // [n_ens*n_rep][q][L] storage order (field variant)
     unsigned* done;           // [n_ens] arrival counters of the swap event
+    long long* dbg;           // PT_TIMING builds: [n_ens*n_rep][32 warps][8] clock sums (else unused)
 };
 
 // ---------------------------------------------------------------------------

@@ -62,6 +62,7 @@ struct pt_ctx {
     int32_t* d_h = nullptr;
     unsigned* d_done = nullptr;
     int* d_flag = nullptr;
+    long long* d_dbg = nullptr;
 
     int R() const { return n_ens * n_rep; }
     ptk::Dev dev() const {
@@ -69,7 +70,7 @@ struct pt_ctx {
         d.L = L; d.W = L / 8; d.q = q; d.n_ens = n_ens; d.n_rep = n_rep; d.ens_base = ens_base;
         d.key0 = (uint32_t)seed; d.key1 = (uint32_t)(seed >> 32);
         d.Jq = d_Jq; d.Jpair = d_Jpair; d.beta = d_beta; d.thr_scale = d_scale;
-        d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done;
+        d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done; d.dbg = d_dbg;
         return d;
     }
 };
@@ -83,7 +84,7 @@ void free_ctx(pt_ctx* c) {
     if (!c) return;
     cudaFree(c->d_Jq); cudaFree(c->d_Jpair); cudaFree(c->d_beta); cudaFree(c->d_scale);
     cudaFree(c->d_spins); cudaFree(c->d_E); cudaFree(c->d_Etmp); cudaFree(c->d_Eout);
-    cudaFree(c->d_perm); cudaFree(c->d_obs); cudaFree(c->d_h); cudaFree(c->d_done); cudaFree(c->d_flag);
+    cudaFree(c->d_perm); cudaFree(c->d_obs); cudaFree(c->d_h); cudaFree(c->d_done); cudaFree(c->d_flag); cudaFree(c->d_dbg);
     delete c;
 }
 
@@ -214,6 +215,10 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
     PT_CUDA_C(cudaMalloc(&c->d_flag, sizeof(int)));
     PT_CUDA_C(cudaMemset(c->d_obs, 0, (size_t)R * sizeof(pt_obs)));
     PT_CUDA_C(cudaMemset(c->d_done, 0, (size_t)n_ens * sizeof(unsigned)));
+#ifdef PT_TIMING
+    PT_CUDA_C(cudaMalloc(&c->d_dbg, (size_t)R * 32 * 8 * sizeof(long long)));
+    PT_CUDA_C(cudaMemset(c->d_dbg, 0, (size_t)R * 32 * 8 * sizeof(long long)));
+#endif
 
     std::vector<double> scale(n_rep);
     for (int t = 0; t < n_rep; ++t) scale[t] = betas[t] > 0.0 ? 16777216.0 / betas[t] : INFINITY;
@@ -385,6 +390,16 @@ int pt_get_couplings(pt_ctx* c, int32_t* Jq) {
 }
 
 int64_t pt_sweep_counter(pt_ctx* c) { return c ? c->sweep : -1; }
+
+#ifdef PT_TIMING
+// Development builds only (-DPT_TIMING): per-warp clock sums of the sweep kernel, [R][32][8].
+int pt_debug_timing(pt_ctx* c, long long* out) {
+    if (!c || !out || !c->d_dbg) return fail(PT_EINVAL, "no timing buffer");
+    PT_CUDA(cudaMemcpy(out, c->d_dbg, (size_t)c->R() * 32 * 8 * sizeof(long long), cudaMemcpyDeviceToHost));
+    PT_CUDA(cudaMemset(c->d_dbg, 0, (size_t)c->R() * 32 * 8 * sizeof(long long)));
+    return PT_OK;
+}
+#endif
 
 int pt_set_variant(pt_ctx* c, int variant) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");

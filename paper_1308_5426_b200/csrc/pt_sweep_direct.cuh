@@ -50,9 +50,10 @@
 namespace ptk {
 
 constexpr int DIRECT_MAX_BULK = 512;
-constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 64;  // + two chain warps
+constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 32;  // + the chain warp
 constexpr int DIRECT_NPAIR = 35;   // packed coupling pairs per thread and half
-constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: 224 sites around a block
+constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: the 224 sites (56 quads) around a block
+constexpr int DIRECT_NEAR_QUADS = 56;
 
 __host__ __device__ inline bool direct_applies(int L, int q) {
     return (L % 64) == 0 && L >= 64 && L <= 64 * (DIRECT_MAX_BULK / 8) && q <= 8;
@@ -61,15 +62,29 @@ __host__ __device__ inline int direct_bulk_threads(int L) {
     const int t = 8 * (L / 64);
     return t < 32 ? 32 : (t + 31) / 32 * 32;
 }
-__host__ __device__ inline int direct_threads(int L) { return direct_bulk_threads(L) + 64; }
-// dynamic smem (32-bit words): theta[L] | lut[2L] | sp[W] | sp0[W] | bq[W] | part[64] | Jz[96] | PPhi[256]
+__host__ __device__ inline int direct_threads(int L) { return direct_bulk_threads(L) + 32; }
+// Near quads per bulk thread (template parameter NEARQ): 0 = the bulk warps sum both halves everywhere.
+__host__ __device__ inline int direct_nearq(int L, int r_hi) {
+    const int njr = L / 64;
+    const int nq = (DIRECT_NEAR_QUADS + njr - 1) / njr;
+    if (r_hi > DIRECT_NEAR_R || L < 256 || nq > 4) return 0;
+    return nq == 3 ? 4 : nq;
+}
+// dynamic smem (32-bit words): theta[L] | lut[2L] | sp[W] | sp0[W] | bq[W] | selb[L/4] | cm[2][64][32] | part[64] | Jz[96]
 __host__ __device__ inline size_t direct_smem_bytes(int L) {
-    return (size_t)(3 * L + 3 * (L / 8) + 64 + 96 + 256) * 4;
+    return (size_t)(3 * L + 3 * (L / 8) + L / 4 + 4096 + 64 + 96) * 4;
 }
 
 __device__ __forceinline__ int dp4a_s32_u32(int a, uint32_t b, int c) {
     int d;
     asm("dp4a.s32.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+// PRMT without the selector masking of __byte_perm (colours are < 8, so bit 3 of every selector nibble is 0;
+// selector bits above 15 are ignored by the instruction)
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
     return d;
 }
 
@@ -91,9 +106,10 @@ struct DirectSmem {
     uint32_t* sp;     // [W]  live packed spins
     uint32_t* sp0;    // [W]  spins at the start of the running sweep
     uint32_t* bq;     // [W]  proposed colours
+    uint8_t* selb;    // [L]  a0 | b << 4: colour at the start of the sweep and proposed colour
+    int32_t* cm;      // [2][64][32] correction terms of a block, double buffered (see CORR below)
     uint32_t* part;   // [2][32] block sums S_i, double buffered
     int32_t* Jz;      // [96] Jz[n] = 0 for n < 32, Jq[n - 32] above
-    uint32_t* PPhi;   // [256] index r + 128 -> hi(|r|) | hi(|r-1|) << 16, hi(d) = Jq[d] >> 16 for 1 <= d <= r_hi
 };
 
 // Start of a sweep, all threads: proposals, thresholds and colour tables of all sites (A6, A7, A9) and the
@@ -103,7 +119,7 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
     const int W = d.W, q = d.q;
     for (int w = threadIdx.x; w < W; w += blockDim.x) {
         const uint32_t word = m.sp[w];
-        uint32_t bword = 0;
+        uint32_t bword = 0, s0 = 0, s1 = 0;
 #pragma unroll
         for (int n = 0; n < 8; ++n) {
             const int i = 8 * w + n;
@@ -112,6 +128,7 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
             const uint32_t k = __umulhi(p.w0, (uint32_t)(q - 1));
             const uint32_t b = k + (k >= a ? 1u : 0u);
             bword |= b << (4 * n);
+            if (n < 4) s0 |= (a | (b << 4)) << (8 * n); else s1 |= (a | (b << 4)) << (8 * (n - 4));
             m.theta[i] = accept_threshold(uniform53(p.w1, p.w2), scale);
             const unsigned long long tab =
                 0x0101010101010101ull + (1ull << (8 * a)) - (1ull << (8 * b));  // byte k = s'(k)
@@ -119,6 +136,7 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
         }
         m.bq[w] = bword;
         m.sp0[w] = word;
+        reinterpret_cast<uint2*>(m.selb)[w] = make_uint2(s0, s1);
     }
 }
 
@@ -140,12 +158,28 @@ __device__ __forceinline__ int direct_nmax(const uint32_t* sp, int W, int q, int
     return nmax;
 }
 
-template <bool FULL_HI>
+// Column of site l in row f of the correction matrix (rotated so that the bulk threads' stores, 8 site groups x 4
+// rows per warp, hit 32 different banks; a row read by the chain warp is a permutation of the banks anyway).
+__device__ __forceinline__ int cm_index(int f, int l) { return (f << 5) | ((l + 2 * (f & 3)) & 31); }
+
+#ifdef PT_TIMING
+#define PT_T0(v) const long long v = clock64()
+#define PT_ACC(slot, v) tacc[slot] += clock64() - (v)
+#else
+#define PT_T0(v)
+#define PT_ACC(slot, v)
+#endif
+
+// NEARQ = 0: the bulk warps sum both 16-bit halves of every coupling.  NEARQ = 1, 2, 4: they sum the low halves
+// only, plus the high halves of NEARQ of the 56 quads of sites within distance 95 of the block (requires
+// r_hi <= 95 and NEARQ * L/64 >= 56).
+template <int NEARQ>
 __global__ void __launch_bounds__(DIRECT_MAX_THREADS, 1)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi) {
+    constexpr bool FULL_HI = NEARQ == 0;
     extern __shared__ uint32_t smem_d[];
     const int L = d.L, W = d.W, q = d.q;
-    const int NT = blockDim.x, NTB = NT - 64;
+    const int NT = blockDim.x, NTB = NT - 32;
     const int NB = L >> 5;
     DirectSmem m;
     m.theta = (int32_t*)smem_d;
@@ -153,29 +187,27 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
     m.sp = (uint32_t*)(m.lut + L);
     m.sp0 = m.sp + W;
     m.bq = m.sp0 + W;
-    m.part = m.bq + W;
+    m.selb = (uint8_t*)(m.bq + W);
+    m.cm = (int32_t*)(m.selb + L);
+    m.part = (uint32_t*)(m.cm + 4096);
     m.Jz = (int32_t*)(m.part + 64);
-    m.PPhi = (uint32_t*)(m.Jz + 96);
     __shared__ int s_cnt[16];
     __shared__ uint32_t s_mask[2];
-    __shared__ long long s_dE[2];
-    __shared__ int s_nacc[2];
+    __shared__ long long s_dE;
+    __shared__ int s_nacc;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int e = blockIdx.x / d.n_rep, t = blockIdx.x % d.n_rep;
     const int st = d.perm[blockIdx.x];
     const size_t x = (size_t)e * d.n_rep + st;
     uint32_t* g_sp = d.spins + x * W;
+#ifdef PT_TIMING
+    long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    PT_T0(t_kernel);
+#endif
 
     for (int w = tid; w < W; w += NT) m.sp[w] = g_sp[w];
-    if (tid < 96) m.Jz[tid] = tid < 32 ? 0 : d.Jq[tid - 32];
-    for (int n = tid; n < 256; n += NT) {
-        const int r = n - 128;
-        const int r0 = r < 0 ? -r : r, r1 = r - 1 < 0 ? 1 - r : r - 1;
-        const uint32_t h0 = (r0 >= 1 && r0 <= r_hi) ? ((uint32_t)d.Jq[r0] >> 16) : 0u;
-        const uint32_t h1 = (r1 >= 1 && r1 <= r_hi) ? ((uint32_t)d.Jq[r1] >> 16) : 0u;
-        m.PPhi[n] = h0 | (h1 << 16);
-    }
+    for (int n = tid; n < 96; n += NT) m.Jz[n] = n < 32 ? 0 : d.Jq[n - 32];
     if (tid < 64) m.part[tid] = 0u;
     const double scale = d.thr_scale[t];
     const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_SWEEP;
@@ -204,20 +236,49 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
             }
             if (!FULL_HI) PH[0] = 0u;
         }
+        // NEAR: high halves of quad n = jr + NJR*iq (sites i0 - 96 + 4n + {0..3}) for this thread's 4 sites:
+        // NP[iq][mm][0] = hi(|r|) | hi(|r-1|) << 16, [1] = hi(|r-2|) | hi(|r-3|) << 16, r = gbase + 2mm + 96 - 4n,
+        // hi(x) = Jq[x] >> 16 for 1 <= x <= r_hi, else 0.
+        uint32_t NP[NEARQ ? NEARQ : 1][4][2];
+        if (NEARQ) {
+#pragma unroll
+            for (int iq = 0; iq < (NEARQ ? NEARQ : 1); ++iq) {
+                const int n = jr + NJR * iq;
+#pragma unroll
+                for (int mm = 0; mm < 4; ++mm) {
+                    uint32_t hv[4];
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        int r = gbase + 2 * mm + 96 - 4 * n - c;
+                        r = r < 0 ? -r : r;
+                        hv[c] = (active && n < DIRECT_NEAR_QUADS && r >= 1 && r <= r_hi) ? ((uint32_t)__ldg(d.Jq + r) >> 16)
+                                                                                        : 0u;
+                    }
+                    NP[iq][mm][0] = hv[0] | (hv[1] << 16);
+                    NP[iq][mm][1] = hv[2] | (hv[3] << 16);
+                }
+            }
+        }
         long long E = d.E[x];
         ObsAcc oa;
         cta_sync();
 
         for (int s = 0; s < n_sweeps; ++s) {
+            PT_T0(t_draw);
             direct_draw(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
             cta_sync();
+            PT_ACC(0, t_draw);
+            PT_T0(t_loop);
             for (int kb = 0; kb <= NB; ++kb) {   // interval kb-1: sum block kb
+                PT_T0(t_b);
                 if (kb < NB) {
                     const int i0 = kb << 5;
                     uint32_t val[4] = {0u, 0u, 0u, 0u};
                     if (active) {
-                        const int wj = ((i0 >> 3) + 8 * jr) % W;
-                        const int wj2 = (wj + 4) % W;
+                        int wj = (i0 >> 3) + 8 * jr;
+                        wj -= wj >= W ? W : 0;
+                        int wj2 = wj + 4;
+                        wj2 -= wj2 >= W ? W : 0;
                         const uint4 wa = *reinterpret_cast<const uint4*>(m.sp + wj);
                         // the second half of the last range is block kb-1, which is being decided: sweep-start copy
                         const uint4 wb = *reinterpret_cast<const uint4*>((jr == NJR - 1 ? m.sp0 : m.sp) + wj2);
@@ -231,7 +292,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                             const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
 #pragma unroll
                             for (int mm = 0; mm < 4; ++mm) {
-                                const uint32_t S = __byte_perm(lt[mm].x, lt[mm].y, sel);
+                                const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
                                 const int tt = 3 - mm + 2 * u;
                                 alo[mm] = __dp2a_lo(PL[tt], S, alo[mm]);
                                 alo[mm] = __dp2a_hi(PL[tt + 1], S, alo[mm]);
@@ -241,8 +302,40 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                                 }
                             }
                         }
+                        if (NEARQ) {
+#pragma unroll
+                            for (int iq = 0; iq < (NEARQ ? NEARQ : 1); ++iq) {
+                                const int n = jr + NJR * iq;   // quads 16..23 are block kb-1: sweep-start copy
+                                int w = (i0 >> 3) - 12 + (n >> 1);
+                                w += w < 0 ? W : 0;
+                                w -= w >= W ? W : 0;
+                                const uint32_t word = ((n >= 16 && n < 24) ? m.sp0 : m.sp)[w];
+                                const uint32_t sel = (n & 1) ? (word >> 16) : word;
+#pragma unroll
+                                for (int mm = 0; mm < 4; ++mm) {
+                                    const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
+                                    ahi[mm] = __dp2a_lo(NP[iq][mm][0], S, ahi[mm]);
+                                    ahi[mm] = __dp2a_hi(NP[iq][mm][1], S, ahi[mm]);
+                                }
+                            }
+                        }
 #pragma unroll
                         for (int mm = 0; mm < 4; ++mm) val[mm] = alo[mm] + (ahi[mm] << 16);
+                        // CORR: correction terms of block kb for a change a_f -> b_f accepted at site
+                        // i0 - 32 + f, f = 0..63 (previous block, then own block):
+                        //   cm[f][l] = Jq[l + 32 - f] (s'_l(b_f) - s'_l(a_f))    (0 for l + 32 <= f)
+                        int32_t* cmb = m.cm + (kb & 1) * 2048;
+                        for (int f = jr; f < 64; f += NJR) {
+                            int jf = i0 - 32 + f;
+                            jf += jf < 0 ? L : 0;
+                            const uint32_t sf = m.selb[jf];
+#pragma unroll
+                            for (int mm = 0; mm < 4; ++mm) {
+                                const int l = gbase + 2 * mm;
+                                const uint32_t sv = prmt(lt[mm].x, lt[mm].y, sf);  // byte 0 = s'_l(a_f), byte 1 = s'_l(b_f)
+                                cmb[cm_index(f, l)] = m.Jz[64 + l - f] * dp4a_s32_u32(0x000001ff, sv, 0);
+                            }
+                        }
                     }
 #pragma unroll
                     for (int mm = 0; mm < 4; ++mm) {
@@ -254,23 +347,32 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                         for (int mm = 0; mm < 4; ++mm) atomicAdd(&m.part[(kb & 1) * 32 + gbase + 2 * mm], val[mm]);
                     }
                 }
+                PT_ACC(1, t_b);
                 cta_sync();
             }
-            cta_sync();  // chain warps have published their sums
+            PT_ACC(2, t_loop);
+            PT_T0(t_end);
+            cta_sync();  // the chain warp has published its sums
             // a8: sample after the sweep, before the swap event (A15)
             const int nmax = direct_nmax(m.sp, W, q, s_cnt);
             if (tid == 0) {
-                E += s_dE[0] + s_dE[1];
-                oa.acc += s_nacc[0] + s_nacc[1];
+                E += s_dE;
+                oa.acc += s_nacc;
                 oa.att += L;
                 oa.sample(E, nmax);
             }
             cta_sync();
+            PT_ACC(3, t_end);
         }
         if (tid == 0) { d.E[x] = E; oa.flush(d.obs + blockIdx.x); }
+#ifdef PT_TIMING
+        if (lane == 0 && d.dbg) {
+            tacc[4] = clock64() - t_kernel;
+            for (int n = 0; n < 8; ++n) d.dbg[((size_t)blockIdx.x * 32 + warp) * 8 + n] += tacc[n];
+        }
+#endif
     } else {
-        // =========================== CHAIN warps ===========================
-        const int cw = warp - (NTB >> 5);  // chain warp 0 decides the even blocks, 1 the odd blocks
+        // =========================== CHAIN warp ===========================
         // sum_r Jq[r]
         uint32_t rowsum;
         {
@@ -278,98 +380,80 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
             for (int r = lane; r < L; r += 32) acc += (uint32_t)d.Jq[r];
             rowsum = __reduce_add_sync(0xffffffffu, acc);
         }
+        // A zero the compiler cannot see through: keeps the adds of the sequential part three-input IADD3s on the
+        // ALU pipe (a two-input add may be issued as IMAD.IADD on the FMA pipe, which the bulk warps saturate).
         cta_sync();
+        const int zero = m.Jz[lane];
 
         for (int s = 0; s < n_sweeps; ++s) {
             direct_draw(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
             cta_sync();
-            // state carried from PREP (interval k-1) to CHAIN (interval k)
-            int cin[32], cpv[32];
-            int th = 0;
             long long dE_acc = 0;
             int n_acc = 0;
+            cta_sync();  // interval -1: block 0 is being summed
+            for (int k = 0; k < NB; ++k) {
+                PT_T0(t_c);
+                const int i0 = k << 5;
+                const int32_t* cmb = m.cm + (k & 1) * 2048;
+                const uint32_t S = m.part[(k & 1) * 32 + lane];
+                const int th = m.theta[i0 + lane];
+                const uint32_t mp = k > 0 ? s_mask[(k - 1) & 1] : 0u;
+                int cin[32];
 #pragma unroll
-            for (int f = 0; f < 32; ++f) { cin[f] = 0; cpv[f] = 0; }
-
-            for (int k = -1; k < NB; ++k) {
-                if (k >= 0 && (k & 1) == cw) {
-                    // ---- CHAIN of block k ----
-                    const int i0 = k << 5;
-                    const uint32_t S = m.part[(k & 1) * 32 + lane];
-                    m.part[(k & 1) * 32 + lane] = 0u;
-                    int dE = (int)(S - rowsum);
-                    const uint32_t mp = k > 0 ? s_mask[(k - 1) & 1] : 0u;
-                    {
-                        int c0 = 0, c1 = 0, c2 = 0, c3s = 0;
+                for (int f = 0; f < 32; ++f) cin[f] = cmb[cm_index(32 + f, lane)];
+                m.part[(k & 1) * 32 + lane] = 0u;
+                int dE = (int)(S - rowsum);
+                if (mp) {   // changes accepted in block k-1, which the bulk sum saw as it was before
+                    int c0 = 0, c1 = 0, c2 = 0, c3s = 0;
 #pragma unroll
-                        for (int f = 0; f < 32; f += 4) {
-                            c0 += ((mp >> f) & 1u) ? cpv[f] : 0;
-                            c1 += ((mp >> (f + 1)) & 1u) ? cpv[f + 1] : 0;
-                            c2 += ((mp >> (f + 2)) & 1u) ? cpv[f + 2] : 0;
-                            c3s += ((mp >> (f + 3)) & 1u) ? cpv[f + 3] : 0;
-                        }
-                        dE += (c0 + c1) + (c2 + c3s);
+                    for (int f = 0; f < 32; f += 4) {
+                        c0 += ((mp >> f) & 1u) ? cmb[cm_index(f, lane)] : 0;
+                        c1 += ((mp >> (f + 1)) & 1u) ? cmb[cm_index(f + 1, lane)] : 0;
+                        c2 += ((mp >> (f + 2)) & 1u) ? cmb[cm_index(f + 2, lane)] : 0;
+                        c3s += ((mp >> (f + 3)) & 1u) ? cmb[cm_index(f + 3, lane)] : 0;
                     }
-                    unsigned mask = __ballot_sync(0xffffffffu, dE <= th);
-#pragma unroll
-                    for (int f = 0; f < 31; ++f) {
-                        dE += ((mask >> f) & 1u) ? cin[f] : 0;  // cin[f] = 0 for lanes <= f: their decision is final
-                        mask = __ballot_sync(0xffffffffu, dE <= th);
-                    }
-                    if ((mask >> lane) & 1u) dE_acc += dE;
-                    if (lane == 0) { n_acc += __popc(mask); s_mask[k & 1] = mask; }
-                    if (lane < 4) {
-                        const int w = (i0 >> 3) + lane;
-                        const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
-                        m.sp[w] = (m.sp[w] & ~nm) | (m.bq[w] & nm);
-                    }
-                } else if (k + 1 < NB && ((k + 1) & 1) == cw) {
-                    // ---- PREP of block k+1: threshold and correction terms; NEAR: high halves around the block ----
-                    const int i0 = (k + 1) << 5;
-                    const int il = i0 + lane;
-                    const int ip = (il - 32 + L) % L;
-                    th = m.theta[il];
-                    const uint2 tab = m.lut[il];
-                    const uint32_t sel = (uint32_t)get_nibble(m.sp, il) | ((uint32_t)get_nibble(m.bq, il) << 4);
-                    const uint32_t selp = (uint32_t)get_nibble(m.sp0, ip) | ((uint32_t)get_nibble(m.bq, ip) << 4);
-                    const int32_t* Jl = m.Jz + 32 + lane;
-#pragma unroll
-                    for (int f = 0; f < 32; ++f) {
-                        const uint32_t sf = __shfl_sync(0xffffffffu, sel, f);
-                        const uint32_t sv = __byte_perm(tab.x, tab.y, sf);  // byte 0 = s'_l(a_f), byte 1 = s'_l(b_f)
-                        cin[f] = Jl[-f] * dp4a_s32_u32(0x000001ff, sv, 0);
-                        const uint32_t pf = __shfl_sync(0xffffffffu, selp, f);
-                        const uint32_t pv = __byte_perm(tab.x, tab.y, pf);
-                        cpv[f] = Jl[32 - f] * dp4a_s32_u32(0x000001ff, pv, 0);
-                    }
-                    if (!FULL_HI) {
-                        uint32_t acc = 0;
-                        const int w0 = (i0 >> 3) - 12 + W;   // window: sites i0-96 .. i0+127 = 28 words
-                        const uint32_t* pp = m.PPhi + 128 + lane + 96;
-#pragma unroll 4
-                        for (int n = 0; n < 28; ++n) {
-                            const int w = (w0 + n) % W;
-                            // words 8..11 of the window are block k (being decided): sweep-start copy
-                            const uint32_t word = (n >= 8 && n < 12) ? m.sp0[w] : m.sp[w];
-                            const uint32_t S0 = __byte_perm(tab.x, tab.y, word);
-                            const uint32_t S1 = __byte_perm(tab.x, tab.y, word >> 16);
-                            // site j = i0 - 96 + 8n + {0..7}; r = il - j = lane + 96 - 8n - {0..7}
-                            acc = __dp2a_lo(pp[-8 * n], S0, acc);
-                            acc = __dp2a_hi(pp[-8 * n - 2], S0, acc);
-                            acc = __dp2a_lo(pp[-8 * n - 4], S1, acc);
-                            acc = __dp2a_hi(pp[-8 * n - 6], S1, acc);
-                        }
-                        atomicAdd(&m.part[((k + 1) & 1) * 32 + lane], acc << 16);
-                    }
+                    dE += (c0 + c1) + (c2 + c3s);
                 }
+                PT_ACC(1, t_c);
+                PT_T0(t_s);
+                // the sequential part: lane f's decision is final once steps 0..f-1 are done (cin[f] = 0 for
+                // lanes <= f); if it accepts, every later lane takes the correction
+#pragma unroll
+                for (int f = 0; f < 31; ++f) {
+                    const int X = dE + cin[f] + zero;
+                    asm volatile(
+                        "{\n\t.reg .pred pf, pq, pa;\n\t"
+                        "setp.eq.s32 pf, %1, %2;\n\t"
+                        "setp.le.and.s32 pq, %0, %3, pf;\n\t"
+                        "vote.sync.any.pred pa, pq, 0xffffffff;\n\t"
+                        "selp.s32 %0, %4, %0, pa;\n\t}"
+                        : "+r"(dE)
+                        : "r"(lane), "r"(f), "r"(th), "r"(X));
+                }
+                const unsigned mask = __ballot_sync(0xffffffffu, dE <= th);
+                PT_ACC(2, t_s);
+                if ((mask >> lane) & 1u) dE_acc += dE;
+                if (lane == 0) { n_acc += __popc(mask); s_mask[k & 1] = mask; }
+                if (lane < 4) {
+                    const int w = (i0 >> 3) + lane;
+                    const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
+                    m.sp[w] = (m.sp[w] & ~nm) | (m.bq[w] & nm);
+                }
+                PT_ACC(0, t_c);
                 cta_sync();
             }
             for (int o = 16; o > 0; o >>= 1) dE_acc += __shfl_xor_sync(0xffffffffu, dE_acc, o);
-            if (lane == 0) { s_dE[cw] = dE_acc; s_nacc[cw] = n_acc; }
+            if (lane == 0) { s_dE = dE_acc; s_nacc = n_acc; }
             cta_sync();
             direct_nmax(m.sp, W, q, s_cnt);
             cta_sync();
         }
+#ifdef PT_TIMING
+        if (lane == 0 && d.dbg) {
+            tacc[4] = clock64() - t_kernel;
+            for (int n = 0; n < 8; ++n) d.dbg[((size_t)blockIdx.x * 32 + warp) * 8 + n] += tacc[n];
+        }
+#endif
     }
 
     cta_sync();
@@ -381,8 +465,13 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
 inline int launch_sweep_direct(const Dev& d, long long sweep0, int n_sweeps, int do_swap, int r_hi,
                                cudaStream_t stream) {
     const size_t smem = direct_smem_bytes(d.L);
-    const bool full_hi = r_hi > DIRECT_NEAR_R || d.L < 256;  // NEAR's 224-site window must not wrap onto itself
-    auto kern = full_hi ? sweep_direct_kernel<true> : sweep_direct_kernel<false>;
+    void (*kern)(Dev, long long, int, int, int) = nullptr;
+    switch (direct_nearq(d.L, r_hi)) {
+        case 1: kern = sweep_direct_kernel<1>; break;
+        case 2: kern = sweep_direct_kernel<2>; break;
+        case 4: kern = sweep_direct_kernel<4>; break;
+        default: kern = sweep_direct_kernel<0>; break;
+    }
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return (int)err;
     kern<<<d.n_ens * d.n_rep, direct_threads(d.L), smem, stream>>>(d, sweep0, n_sweeps, do_swap, r_hi);
