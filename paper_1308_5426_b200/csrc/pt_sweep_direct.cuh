@@ -269,24 +269,37 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
             cta_sync();
             PT_ACC(0, t_draw);
             PT_T0(t_loop);
+            // per-thread cursors, advanced by one block (32 sites = 4 words) per interval
+            const uint2* lutp = m.lut + gbase;
+            int wj = 8 * jr;                                    // first word of this thread's j-range
+            // the second half of the last range is block kb-1, which is being decided: sweep-start copy
+            const uint32_t* sp2 = (jr == NJR - 1) ? m.sp0 : m.sp;
+            int wn[NEARQ ? NEARQ : 1];                          // NEAR: word of quad n = jr + NJR*iq
+#pragma unroll
+            for (int iq = 0; iq < (NEARQ ? NEARQ : 1); ++iq) {
+                wn[iq] = ((jr + NJR * iq) >> 1) - 12;
+                wn[iq] += wn[iq] < 0 ? W : 0;
+            }
+            int jf = L - 32 + jr;                               // CORR fast path (NJR == 64): site of row f = jr
+            jf -= jf >= L ? L : 0;
+            int Jc[4];
+#pragma unroll
+            for (int mm = 0; mm < 4; ++mm) Jc[mm] = (NJR == 64) ? m.Jz[64 + gbase + 2 * mm - jr] : 0;
             for (int kb = 0; kb <= NB; ++kb) {   // interval kb-1: sum block kb
                 PT_T0(t_b);
                 if (kb < NB) {
-                    const int i0 = kb << 5;
                     uint32_t val[4] = {0u, 0u, 0u, 0u};
                     if (active) {
-                        int wj = (i0 >> 3) + 8 * jr;
-                        wj -= wj >= W ? W : 0;
                         int wj2 = wj + 4;
                         wj2 -= wj2 >= W ? W : 0;
                         const uint4 wa = *reinterpret_cast<const uint4*>(m.sp + wj);
-                        // the second half of the last range is block kb-1, which is being decided: sweep-start copy
-                        const uint4 wb = *reinterpret_cast<const uint4*>((jr == NJR - 1 ? m.sp0 : m.sp) + wj2);
+                        const uint4 wb = *reinterpret_cast<const uint4*>(sp2 + wj2);
                         const uint32_t words[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
                         uint2 lt[4];
-                        uint32_t alo[4] = {0u, 0u, 0u, 0u}, ahi[4] = {0u, 0u, 0u, 0u};
+                        // two accumulators per site (even / odd pair of j) keep the IDP.2A chains short
+                        uint32_t alo[4] = {0u, 0u, 0u, 0u}, alo2[4] = {0u, 0u, 0u, 0u}, ahi[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
-                        for (int mm = 0; mm < 4; ++mm) lt[mm] = m.lut[i0 + gbase + 2 * mm];
+                        for (int mm = 0; mm < 4; ++mm) lt[mm] = lutp[2 * mm];
 #pragma unroll
                         for (int u = 0; u < 16; ++u) {
                             const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
@@ -295,21 +308,19 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                                 const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
                                 const int tt = 3 - mm + 2 * u;
                                 alo[mm] = __dp2a_lo(PL[tt], S, alo[mm]);
-                                alo[mm] = __dp2a_hi(PL[tt + 1], S, alo[mm]);
+                                alo2[mm] = __dp2a_hi(PL[tt + 1], S, alo2[mm]);
                                 if (FULL_HI) {
                                     ahi[mm] = __dp2a_lo(PH[FULL_HI ? tt : 0], S, ahi[mm]);
                                     ahi[mm] = __dp2a_hi(PH[FULL_HI ? tt + 1 : 0], S, ahi[mm]);
                                 }
                             }
                         }
+#ifndef PT_EXP_NOEXTRA
                         if (NEARQ) {
 #pragma unroll
                             for (int iq = 0; iq < (NEARQ ? NEARQ : 1); ++iq) {
                                 const int n = jr + NJR * iq;   // quads 16..23 are block kb-1: sweep-start copy
-                                int w = (i0 >> 3) - 12 + (n >> 1);
-                                w += w < 0 ? W : 0;
-                                w -= w >= W ? W : 0;
-                                const uint32_t word = ((n >= 16 && n < 24) ? m.sp0 : m.sp)[w];
+                                const uint32_t word = ((n >= 16 && n < 24) ? m.sp0 : m.sp)[wn[iq]];
                                 const uint32_t sel = (n & 1) ? (word >> 16) : word;
 #pragma unroll
                                 for (int mm = 0; mm < 4; ++mm) {
@@ -319,23 +330,46 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                                 }
                             }
                         }
+#endif
 #pragma unroll
-                        for (int mm = 0; mm < 4; ++mm) val[mm] = alo[mm] + (ahi[mm] << 16);
+                        for (int mm = 0; mm < 4; ++mm) val[mm] = alo[mm] + alo2[mm] + (ahi[mm] << 16);
                         // CORR: correction terms of block kb for a change a_f -> b_f accepted at site
                         // i0 - 32 + f, f = 0..63 (previous block, then own block):
                         //   cm[f][l] = Jq[l + 32 - f] (s'_l(b_f) - s'_l(a_f))    (0 for l + 32 <= f)
+#ifndef PT_EXP_NOEXTRA
                         int32_t* cmb = m.cm + (kb & 1) * 2048;
-                        for (int f = jr; f < 64; f += NJR) {
-                            int jf = i0 - 32 + f;
-                            jf += jf < 0 ? L : 0;
+                        if (NJR == 64) {
                             const uint32_t sf = m.selb[jf];
 #pragma unroll
                             for (int mm = 0; mm < 4; ++mm) {
-                                const int l = gbase + 2 * mm;
                                 const uint32_t sv = prmt(lt[mm].x, lt[mm].y, sf);  // byte 0 = s'_l(a_f), byte 1 = s'_l(b_f)
-                                cmb[cm_index(f, l)] = m.Jz[64 + l - f] * dp4a_s32_u32(0x000001ff, sv, 0);
+                                cmb[cm_index(jr, gbase + 2 * mm)] = Jc[mm] * dp4a_s32_u32(0x000001ff, sv, 0);
+                            }
+                        } else {
+                            for (int f = jr; f < 64; f += NJR) {
+                                int j2 = jf - jr + f;
+                                j2 -= j2 >= L ? L : 0;
+                                const uint32_t sf = m.selb[j2];
+#pragma unroll
+                                for (int mm = 0; mm < 4; ++mm) {
+                                    const int l = gbase + 2 * mm;
+                                    const uint32_t sv = prmt(lt[mm].x, lt[mm].y, sf);
+                                    cmb[cm_index(f, l)] = m.Jz[64 + l - f] * dp4a_s32_u32(0x000001ff, sv, 0);
+                                }
                             }
                         }
+#endif
+                        // advance the cursors
+                        lutp += 32;
+                        wj += 4;
+                        wj -= wj >= W ? W : 0;
+#pragma unroll
+                        for (int iq = 0; iq < (NEARQ ? NEARQ : 1); ++iq) {
+                            wn[iq] += 4;
+                            wn[iq] -= wn[iq] >= W ? W : 0;
+                        }
+                        jf += 32;
+                        jf -= jf >= L ? L : 0;
                     }
 #pragma unroll
                     for (int mm = 0; mm < 4; ++mm) {
@@ -418,6 +452,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                 PT_T0(t_s);
                 // the sequential part: lane f's decision is final once steps 0..f-1 are done (cin[f] = 0 for
                 // lanes <= f); if it accepts, every later lane takes the correction
+#ifndef PT_EXP_NOCHAIN
 #pragma unroll
                 for (int f = 0; f < 31; ++f) {
                     const int X = dE + cin[f] + zero;
@@ -430,6 +465,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                         : "+r"(dE)
                         : "r"(lane), "r"(f), "r"(th), "r"(X));
                 }
+#endif
                 const unsigned mask = __ballot_sync(0xffffffffu, dE <= th);
                 PT_ACC(2, t_s);
                 if ((mask >> lane) & 1u) dE_acc += dE;
