@@ -48,6 +48,7 @@ struct pt_ctx {
     int variant = PT_VARIANT_FIELD;
     bool fields_valid = false;
     int64_t sweep = 0;
+    long long rowsum = 0;  // sum_r Jq[r]
     int r_hi = 0;  // largest r <= L/2 with Jq[r] >= 2^16 (direct variant: reach of the high halves)
     int32_t* d_Jq = nullptr;
     uint32_t* d_Jpair = nullptr;
@@ -109,10 +110,13 @@ int ensure_fields(pt_ctx* c) {
     return PT_OK;
 }
 
-int resolve_variant(int L, int q, int variant, int* out) {
-    if (variant == PT_VARIANT_AUTO) variant = direct_applies(L, q) ? PT_VARIANT_DIRECT : PT_VARIANT_FIELD;
+// rowsum = sum_r Jq[r]: the direct variant keeps theta - dE in int32 and needs |dE| <= rowsum < 2^30 - 1.
+int resolve_variant(int L, int q, long long rowsum, int variant, int* out) {
+    const bool direct_ok = direct_applies(L, q) && rowsum < (1ll << 30) - 1;
+    if (variant == PT_VARIANT_AUTO) variant = direct_ok ? PT_VARIANT_DIRECT : PT_VARIANT_FIELD;
     if (variant == PT_VARIANT_DIRECT) {
-        if (!direct_applies(L, q)) return fail(PT_EINVAL, "direct variant needs L % 32 == 0, L >= 64 and q <= 8");
+        if (!direct_ok)
+            return fail(PT_EINVAL, "direct variant needs L % 64 == 0, 64 <= L <= 4096, q <= 8 and sum_r Jq[r] < 2^30 - 1");
         if (ptk::direct_smem_bytes(L) + 256 > kSmemLimit)
             return fail(PT_ECAPACITY, "direct variant does not fit in shared memory for this L");
     } else if (variant == PT_VARIANT_FIELD) {
@@ -180,7 +184,7 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
 
     int variant = 0;
     {
-        int rc = resolve_variant(L, q, PT_VARIANT_AUTO, &variant);
+        int rc = resolve_variant(L, q, 0, PT_VARIANT_AUTO, &variant);
         if (rc) return rc;
     }
 
@@ -235,6 +239,11 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
     for (int r = 0; r < L; ++r) { rowsum += Jq[r]; bad |= Jq[r] < 0; }
     for (int r = 1; r <= L / 2; ++r)
         if (Jq[r] >= 65536) c->r_hi = r;
+    c->rowsum = rowsum;
+    {
+        int rc = resolve_variant(L, q, rowsum, PT_VARIANT_AUTO, &c->variant);
+        if (rc) { free_ctx(c); return rc; }
+    }
     if (bad || rowsum >= (1ll << 31)) {
         free_ctx(c);
         return fail(PT_EOVERFLOW, "sum_r Jq[r] >= 2^31: sigma too small for int32 energy differences");
@@ -404,7 +413,7 @@ int pt_debug_timing(pt_ctx* c, long long* out) {
 int pt_set_variant(pt_ctx* c, int variant) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");
     int v = 0;
-    int rc = resolve_variant(c->L, c->q, variant, &v);
+    int rc = resolve_variant(c->L, c->q, c->rowsum, variant, &v);
     if (rc) return rc;
     c->variant = v;
     return PT_OK;

@@ -129,7 +129,7 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
             const uint32_t b = k + (k >= a ? 1u : 0u);
             bword |= b << (4 * n);
             if (n < 4) s0 |= (a | (b << 4)) << (8 * n); else s1 |= (a | (b << 4)) << (8 * (n - 4));
-            m.theta[i] = accept_threshold(uniform53(p.w1, p.w2), scale);
+            m.theta[i] = min(accept_threshold(uniform53(p.w1, p.w2), scale), 1 << 30);  // |dE| < 2^30: same decisions
             const unsigned long long tab =
                 0x0101010101010101ull + (1ull << (8 * a)) - (1ull << (8 * b));  // byte k = s'(k)
             m.lut[i] = make_uint2((uint32_t)tab, (uint32_t)(tab >> 32));
@@ -158,9 +158,12 @@ __device__ __forceinline__ int direct_nmax(const uint32_t* sp, int W, int q, int
     return nmax;
 }
 
-// Column of site l in row f of the correction matrix (rotated so that the bulk threads' stores, 8 site groups x 4
-// rows per warp, hit 32 different banks; a row read by the chain warp is a permutation of the banks anyway).
-__device__ __forceinline__ int cm_index(int f, int l) { return (f << 5) | ((l + 2 * (f & 3)) & 31); }
+// Correction matrix of a block: entry (row f = 0..63, site l = 0..31) at word l*64 + ((f + 4l + 8(l>>3)) & 63).
+// Site-major, so that the chain lane l fetches its 64 entries as 16 LDS.128; the rotation makes both those loads
+// (8 consecutive lanes hit 8 different 16-byte columns) and the bulk threads' stores (8 site groups x 4 consecutive
+// rows per warp hit 32 different banks) conflict-free.
+__device__ __forceinline__ int cm_rot(int l) { return 4 * l + 8 * (l >> 3); }
+__device__ __forceinline__ int cm_index(int f, int l) { return (l << 6) | ((f + cm_rot(l)) & 63); }
 
 #ifdef PT_TIMING
 #define PT_T0(v) const long long v = clock64()
@@ -170,13 +173,50 @@ __device__ __forceinline__ int cm_index(int f, int l) { return (f << 5) | ((l + 
 #define PT_ACC(slot, v)
 #endif
 
+// sum over the 4 bits b..b+3 of m of (bit ? c : 0), added to acc: 4 LOP3 (bit test -> predicate), 4 SEL, 2 IADD3,
+// all on the ALU pipe (the compiler's own choice for this pattern is shift pairs on the FMA or uniform pipes)
+__device__ __forceinline__ int masked_add4(int acc, unsigned m, int b, int4 c) {
+    asm("{\n\t.reg .pred p0, p1, p2, p3;\n\t.reg .b32 t0, t1, t2, t3;\n\t"
+        "and.b32 t0, %5, %6;\n\tsetp.ne.u32 p0, t0, 0;\n\t"
+        "and.b32 t1, %5, %7;\n\tsetp.ne.u32 p1, t1, 0;\n\t"
+        "and.b32 t2, %5, %8;\n\tsetp.ne.u32 p2, t2, 0;\n\t"
+        "and.b32 t3, %5, %9;\n\tsetp.ne.u32 p3, t3, 0;\n\t"
+        "selp.b32 t0, %1, 0, p0;\n\tselp.b32 t1, %2, 0, p1;\n\tselp.b32 t2, %3, 0, p2;\n\tselp.b32 t3, %4, 0, p3;\n\t"
+        "add.s32 t0, t0, t1;\n\tadd.s32 t2, t2, t3;\n\tadd.s32 t0, t0, t2;\n\tadd.s32 %0, %0, t0;\n\t}"
+        : "+r"(acc)
+        : "r"(c.x), "r"(c.y), "r"(c.z), "r"(c.w), "r"(m), "r"(1u << b), "r"(2u << b), "r"(4u << b), "r"(8u << b));
+    return acc;
+}
+
+// ---- mbarrier (shared-memory transaction barrier) helpers: producer/consumer hand-off between the warps ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+// release: the arriving thread's earlier shared-memory writes are visible to whoever sees the phase complete
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
+}
+// blocks until the phase with the given parity has completed (acquire)
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "MBAR_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra MBAR_DONE;\n\t"
+        "bra MBAR_WAIT;\n\t"
+        "MBAR_DONE:\n\t}" ::"r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+}
+
 // NEARQ = 0: the bulk warps sum both 16-bit halves of every coupling.  NEARQ = 1, 2, 4: they sum the low halves
 // only, plus the high halves of NEARQ of the 56 quads of sites within distance 95 of the block (requires
-// r_hi <= 95 and NEARQ * L/64 >= 56).
-template <int NEARQ>
+// r_hi <= 95 and NEARQ * L/64 >= 56).  NJR64: L == 4096 (64 j-ranges), one CORR row per thread, straight-line code.
+template <int NEARQ, bool NJR64>
 __global__ void __launch_bounds__(DIRECT_MAX_THREADS, 1)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi) {
     constexpr bool FULL_HI = NEARQ == 0;
+    constexpr int NQ = NEARQ ? NEARQ : 1;
     extern __shared__ uint32_t smem_d[];
     const int L = d.L, W = d.W, q = d.q;
     const int NT = blockDim.x, NTB = NT - 32;
@@ -192,9 +232,11 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
     m.part = (uint32_t*)(m.cm + 4096);
     m.Jz = (int32_t*)(m.part + 64);
     __shared__ int s_cnt[16];
-    __shared__ uint32_t s_mask[2];
     __shared__ long long s_dE;
     __shared__ int s_nacc;
+    // full[s]: the block sums and correction rows of buffer s are complete (one arrival per bulk warp);
+    // done[s]: the chain warp has decided the block of buffer s and written its spins (one arrival).
+    __shared__ __align__(8) uint64_t s_full[2], s_done[2];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int e = blockIdx.x / d.n_rep, t = blockIdx.x % d.n_rep;
@@ -217,7 +259,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
         // thread -> (site group g, j-range jr); group g = sites 8(g>>1) + (g&1) + {0,2,4,6}
         const int g = tid & 7, jr = tid >> 3;
         const int par = g & 1, gbase = 8 * (g >> 1) + par;
-        const int NJR = L / 64;
+        const int NJR = NJR64 ? 64 : L / 64;
         const bool active = jr < NJR;
         // couplings of this thread: pair tt holds Jq[r], Jq[r-1] with r = R0 - 2 tt  (mod L)
         uint32_t PL[DIRECT_NPAIR];
@@ -239,10 +281,10 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
         // NEAR: high halves of quad n = jr + NJR*iq (sites i0 - 96 + 4n + {0..3}) for this thread's 4 sites:
         // NP[iq][mm][0] = hi(|r|) | hi(|r-1|) << 16, [1] = hi(|r-2|) | hi(|r-3|) << 16, r = gbase + 2mm + 96 - 4n,
         // hi(x) = Jq[x] >> 16 for 1 <= x <= r_hi, else 0.
-        uint32_t NP[NEARQ ? NEARQ : 1][4][2];
+        uint32_t NP[NQ][4][2];
         if (NEARQ) {
 #pragma unroll
-            for (int iq = 0; iq < (NEARQ ? NEARQ : 1); ++iq) {
+            for (int iq = 0; iq < NQ; ++iq) {
                 const int n = jr + NJR * iq;
 #pragma unroll
                 for (int mm = 0; mm < 4; ++mm) {
@@ -259,6 +301,13 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                 }
             }
         }
+        // CORR with one row per thread (NJR64): couplings Jq[l + 32 - f] of row f = jr for this thread's 4 sites
+        int Jc[4];
+#pragma unroll
+        for (int mm = 0; mm < 4; ++mm) {
+            const int dist = gbase + 2 * mm + 32 - jr;
+            Jc[mm] = (NJR64 && dist > 0) ? __ldg(d.Jq + dist) : 0;
+        }
         long long E = d.E[x];
         ObsAcc oa;
         cta_sync();
@@ -266,127 +315,133 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
         for (int s = 0; s < n_sweeps; ++s) {
             PT_T0(t_draw);
             direct_draw(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
+            if (tid == 0) {
+                mbar_init(&s_full[0], NTB >> 5); mbar_init(&s_full[1], NTB >> 5);
+                mbar_init(&s_done[0], 1); mbar_init(&s_done[1], 1);
+            }
             cta_sync();
             PT_ACC(0, t_draw);
             PT_T0(t_loop);
-            // per-thread cursors, advanced by one block (32 sites = 4 words) per interval
+            // per-thread cursors, advanced by one block (32 sites = 4 words) per block
             const uint2* lutp = m.lut + gbase;
             int wj = 8 * jr;                                    // first word of this thread's j-range
             // the second half of the last range is block kb-1, which is being decided: sweep-start copy
             const uint32_t* sp2 = (jr == NJR - 1) ? m.sp0 : m.sp;
-            int wn[NEARQ ? NEARQ : 1];                          // NEAR: word of quad n = jr + NJR*iq
+            int wn[NQ];                                         // NEAR: word of quad n = jr + NJR*iq
 #pragma unroll
-            for (int iq = 0; iq < (NEARQ ? NEARQ : 1); ++iq) {
+            for (int iq = 0; iq < NQ; ++iq) {
                 wn[iq] = ((jr + NJR * iq) >> 1) - 12;
                 wn[iq] += wn[iq] < 0 ? W : 0;
             }
-            int jf = L - 32 + jr;                               // CORR fast path (NJR == 64): site of row f = jr
+            int jf = L - 32 + jr;                               // CORR: site of row f = jr
             jf -= jf >= L ? L : 0;
-            int Jc[4];
-#pragma unroll
-            for (int mm = 0; mm < 4; ++mm) Jc[mm] = (NJR == 64) ? m.Jz[64 + gbase + 2 * mm - jr] : 0;
-            for (int kb = 0; kb <= NB; ++kb) {   // interval kb-1: sum block kb
+            for (int kb = 0; kb < NB; ++kb) {
+                // block kb is summed against: blocks < kb-1 final (the chain warp is done with block kb-2, which
+                // also frees buffer kb&1), block kb-1 as at the start of the sweep, blocks >= kb untouched
+                if (kb >= 2) mbar_wait(&s_done[kb & 1], ((kb >> 1) - 1) & 1);
                 PT_T0(t_b);
-                if (kb < NB) {
-                    uint32_t val[4] = {0u, 0u, 0u, 0u};
-                    if (active) {
-                        int wj2 = wj + 4;
-                        wj2 -= wj2 >= W ? W : 0;
-                        const uint4 wa = *reinterpret_cast<const uint4*>(m.sp + wj);
-                        const uint4 wb = *reinterpret_cast<const uint4*>(sp2 + wj2);
-                        const uint32_t words[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
-                        uint2 lt[4];
-                        // two accumulators per site (even / odd pair of j) keep the IDP.2A chains short
-                        uint32_t alo[4] = {0u, 0u, 0u, 0u}, alo2[4] = {0u, 0u, 0u, 0u}, ahi[4] = {0u, 0u, 0u, 0u};
+                uint32_t val[4] = {0u, 0u, 0u, 0u};
+                if (active) {
+                    int wj2 = wj + 4;
+                    wj2 -= wj2 >= W ? W : 0;
+                    const uint4 wa = *reinterpret_cast<const uint4*>(m.sp + wj);
+                    const uint4 wb = *reinterpret_cast<const uint4*>(sp2 + wj2);
+                    const uint32_t words[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
+                    uint2 lt[4];
 #pragma unroll
-                        for (int mm = 0; mm < 4; ++mm) lt[mm] = lutp[2 * mm];
+                    for (int mm = 0; mm < 4; ++mm) lt[mm] = lutp[2 * mm];
+                    uint32_t nword[NQ];
 #pragma unroll
-                        for (int u = 0; u < 16; ++u) {
-                            const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
+                    for (int iq = 0; iq < NQ; ++iq) {   // quads 16..23 are block kb-1: sweep-start copy
+                        const int n = jr + NJR * iq;
+                        nword[iq] = NEARQ ? ((n >= 16 && n < 24) ? m.sp0 : m.sp)[wn[iq]] : 0u;
+                    }
+                    const uint32_t sf64 = NJR64 ? m.selb[jf] : 0u;
+                    // two accumulators per site (even / odd pair of j) keep the IDP.2A chains short
+                    uint32_t alo[4] = {0u, 0u, 0u, 0u}, alo2[4] = {0u, 0u, 0u, 0u}, ahi[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+                    for (int u = 0; u < 16; ++u) {
+                        const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
+#pragma unroll
+                        for (int mm = 0; mm < 4; ++mm) {
+                            const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
+                            const int tt = 3 - mm + 2 * u;
+                            alo[mm] = __dp2a_lo(PL[tt], S, alo[mm]);
+                            alo2[mm] = __dp2a_hi(PL[tt + 1], S, alo2[mm]);
+                            if (FULL_HI) {
+                                ahi[mm] = __dp2a_lo(PH[FULL_HI ? tt : 0], S, ahi[mm]);
+                                ahi[mm] = __dp2a_hi(PH[FULL_HI ? tt + 1 : 0], S, ahi[mm]);
+                            }
+                        }
+                    }
+#ifndef PT_EXP_NOEXTRA
+                    if (NEARQ) {
+#pragma unroll
+                        for (int iq = 0; iq < NQ; ++iq) {
+                            const int n = jr + NJR * iq;
+                            const uint32_t sel = (n & 1) ? (nword[iq] >> 16) : nword[iq];
 #pragma unroll
                             for (int mm = 0; mm < 4; ++mm) {
                                 const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
-                                const int tt = 3 - mm + 2 * u;
-                                alo[mm] = __dp2a_lo(PL[tt], S, alo[mm]);
-                                alo2[mm] = __dp2a_hi(PL[tt + 1], S, alo2[mm]);
-                                if (FULL_HI) {
-                                    ahi[mm] = __dp2a_lo(PH[FULL_HI ? tt : 0], S, ahi[mm]);
-                                    ahi[mm] = __dp2a_hi(PH[FULL_HI ? tt + 1 : 0], S, ahi[mm]);
-                                }
+                                ahi[mm] = __dp2a_lo(NP[iq][mm][0], S, ahi[mm]);
+                                ahi[mm] = __dp2a_hi(NP[iq][mm][1], S, ahi[mm]);
                             }
                         }
-#ifndef PT_EXP_NOEXTRA
-                        if (NEARQ) {
+                    }
+                    // CORR: correction terms of block kb for a change a_f -> b_f accepted at site
+                    // i0 - 32 + f, f = 0..63 (previous block, then own block):
+                    //   cm[f][l] = Jq[l + 32 - f] (s'_l(b_f) - s'_l(a_f))    (0 for l + 32 <= f)
+                    int32_t* cmb = m.cm + (kb & 1) * 2048;
+                    if (NJR64) {
 #pragma unroll
-                            for (int iq = 0; iq < (NEARQ ? NEARQ : 1); ++iq) {
-                                const int n = jr + NJR * iq;   // quads 16..23 are block kb-1: sweep-start copy
-                                const uint32_t word = ((n >= 16 && n < 24) ? m.sp0 : m.sp)[wn[iq]];
-                                const uint32_t sel = (n & 1) ? (word >> 16) : word;
-#pragma unroll
-                                for (int mm = 0; mm < 4; ++mm) {
-                                    const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
-                                    ahi[mm] = __dp2a_lo(NP[iq][mm][0], S, ahi[mm]);
-                                    ahi[mm] = __dp2a_hi(NP[iq][mm][1], S, ahi[mm]);
-                                }
-                            }
+                        for (int mm = 0; mm < 4; ++mm) {
+                            const uint32_t sv = prmt(lt[mm].x, lt[mm].y, sf64);  // byte 0 = s'_l(a_f), byte 1 = s'_l(b_f)
+                            cmb[cm_index(jr, gbase + 2 * mm)] = Jc[mm] * dp4a_s32_u32(0x000001ff, sv, 0);
                         }
-#endif
-#pragma unroll
-                        for (int mm = 0; mm < 4; ++mm) val[mm] = alo[mm] + alo2[mm] + (ahi[mm] << 16);
-                        // CORR: correction terms of block kb for a change a_f -> b_f accepted at site
-                        // i0 - 32 + f, f = 0..63 (previous block, then own block):
-                        //   cm[f][l] = Jq[l + 32 - f] (s'_l(b_f) - s'_l(a_f))    (0 for l + 32 <= f)
-#ifndef PT_EXP_NOEXTRA
-                        int32_t* cmb = m.cm + (kb & 1) * 2048;
-                        if (NJR == 64) {
-                            const uint32_t sf = m.selb[jf];
+                    } else {
+                        for (int f = jr; f < 64; f += NJR) {
+                            int j2 = jf - jr + f;
+                            j2 -= j2 >= L ? L : 0;
+                            const uint32_t sf = m.selb[j2];
 #pragma unroll
                             for (int mm = 0; mm < 4; ++mm) {
-                                const uint32_t sv = prmt(lt[mm].x, lt[mm].y, sf);  // byte 0 = s'_l(a_f), byte 1 = s'_l(b_f)
-                                cmb[cm_index(jr, gbase + 2 * mm)] = Jc[mm] * dp4a_s32_u32(0x000001ff, sv, 0);
-                            }
-                        } else {
-                            for (int f = jr; f < 64; f += NJR) {
-                                int j2 = jf - jr + f;
-                                j2 -= j2 >= L ? L : 0;
-                                const uint32_t sf = m.selb[j2];
-#pragma unroll
-                                for (int mm = 0; mm < 4; ++mm) {
-                                    const int l = gbase + 2 * mm;
-                                    const uint32_t sv = prmt(lt[mm].x, lt[mm].y, sf);
-                                    cmb[cm_index(f, l)] = m.Jz[64 + l - f] * dp4a_s32_u32(0x000001ff, sv, 0);
-                                }
+                                const int l = gbase + 2 * mm;
+                                const uint32_t sv = prmt(lt[mm].x, lt[mm].y, sf);
+                                cmb[cm_index(f, l)] = m.Jz[64 + l - f] * dp4a_s32_u32(0x000001ff, sv, 0);
                             }
                         }
+                    }
 #endif
-                        // advance the cursors
-                        lutp += 32;
-                        wj += 4;
-                        wj -= wj >= W ? W : 0;
 #pragma unroll
-                        for (int iq = 0; iq < (NEARQ ? NEARQ : 1); ++iq) {
-                            wn[iq] += 4;
-                            wn[iq] -= wn[iq] >= W ? W : 0;
-                        }
-                        jf += 32;
-                        jf -= jf >= L ? L : 0;
-                    }
+                    for (int mm = 0; mm < 4; ++mm) val[mm] = alo[mm] + alo2[mm] + (ahi[mm] << 16);
+                    // advance the cursors
+                    lutp += 32;
+                    wj += 4;
+                    wj -= wj >= W ? W : 0;
 #pragma unroll
-                    for (int mm = 0; mm < 4; ++mm) {
-                        val[mm] += __shfl_xor_sync(0xffffffffu, val[mm], 8);
-                        val[mm] += __shfl_xor_sync(0xffffffffu, val[mm], 16);
+                    for (int iq = 0; iq < NQ; ++iq) {
+                        wn[iq] += 4;
+                        wn[iq] -= wn[iq] >= W ? W : 0;
                     }
-                    if (lane < 8) {
-#pragma unroll
-                        for (int mm = 0; mm < 4; ++mm) atomicAdd(&m.part[(kb & 1) * 32 + gbase + 2 * mm], val[mm]);
-                    }
+                    jf += 32;
+                    jf -= jf >= L ? L : 0;
                 }
+#pragma unroll
+                for (int mm = 0; mm < 4; ++mm) {
+                    val[mm] += __shfl_xor_sync(0xffffffffu, val[mm], 8);
+                    val[mm] += __shfl_xor_sync(0xffffffffu, val[mm], 16);
+                }
+                if (lane < 8) {
+#pragma unroll
+                    for (int mm = 0; mm < 4; ++mm) atomicAdd(&m.part[(kb & 1) * 32 + gbase + 2 * mm], val[mm]);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&s_full[kb & 1]);
                 PT_ACC(1, t_b);
-                cta_sync();
             }
             PT_ACC(2, t_loop);
             PT_T0(t_end);
-            cta_sync();  // the chain warp has published its sums
+            cta_sync();  // the chain warp has decided the last block and published its sums
             // a8: sample after the sweep, before the swap event (A15)
             const int nmax = direct_nmax(m.sp, W, q, s_cnt);
             if (tid == 0) {
@@ -414,69 +469,107 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
             for (int r = lane; r < L; r += 32) acc += (uint32_t)d.Jq[r];
             rowsum = __reduce_add_sync(0xffffffffu, acc);
         }
+        cta_sync();
         // A zero the compiler cannot see through: keeps the adds of the sequential part three-input IADD3s on the
         // ALU pipe (a two-input add may be issued as IMAD.IADD on the FMA pipe, which the bulk warps saturate).
-        cta_sync();
         const int zero = m.Jz[lane];
+        // lane-select constants of the sequential part: step f compares the slack against 0 in lane f only
+        int K[32];
+#pragma unroll
+        for (int f = 0; f < 32; ++f) K[f] = (lane == f) ? zero : 0x7fffffff;
+        const int rot = cm_rot(lane);
 
         for (int s = 0; s < n_sweeps; ++s) {
             direct_draw(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
             cta_sync();
             long long dE_acc = 0;
             int n_acc = 0;
-            cta_sync();  // interval -1: block 0 is being summed
+            uint32_t mp = 0u;   // accept mask of the previous block
             for (int k = 0; k < NB; ++k) {
-                PT_T0(t_c);
                 const int i0 = k << 5;
-                const int32_t* cmb = m.cm + (k & 1) * 2048;
-                const uint32_t S = m.part[(k & 1) * 32 + lane];
+                const int32_t* cml = m.cm + (k & 1) * 2048 + (lane << 6);
+                // independent of the bulk: threshold, and the words of the block for the final update
                 const int th = m.theta[i0 + lane];
-                const uint32_t mp = k > 0 ? s_mask[(k - 1) & 1] : 0u;
-                int cin[32];
+                const int wsp = (i0 >> 3) + (lane & 3);
+                const uint32_t w_old = m.sp[wsp], w_new = m.bq[wsp];
+                mbar_wait(&s_full[k & 1], (k >> 1) & 1);
+                PT_T0(t_c);
+                const uint32_t S = m.part[(k & 1) * 32 + lane];
+                int4 cv[16];   // cv[0..7]: rows of the previous block, cv[8..15]: rows of the own block
 #pragma unroll
-                for (int f = 0; f < 32; ++f) cin[f] = cmb[cm_index(32 + f, lane)];
+                for (int i = 0; i < 16; ++i) cv[i] = *reinterpret_cast<const int4*>(cml + ((4 * i + rot) & 63));
                 m.part[(k & 1) * 32 + lane] = 0u;
-                int dE = (int)(S - rowsum);
+                // slack y = theta - dE: the site accepts iff y >= 0 (theta <= 2^30 and |dE| < 2^30: no overflow)
+                int y = th - (int)(S - rowsum);
+                const unsigned lz = (unsigned)zero;   // per-lane opaque 0: keeps the masks in vector registers
                 if (mp) {   // changes accepted in block k-1, which the bulk sum saw as it was before
-                    int c0 = 0, c1 = 0, c2 = 0, c3s = 0;
+                    const unsigned mv = mp ^ lz;
+                    int c0 = 0, c1 = 0;
 #pragma unroll
-                    for (int f = 0; f < 32; f += 4) {
-                        c0 += ((mp >> f) & 1u) ? cmb[cm_index(f, lane)] : 0;
-                        c1 += ((mp >> (f + 1)) & 1u) ? cmb[cm_index(f + 1, lane)] : 0;
-                        c2 += ((mp >> (f + 2)) & 1u) ? cmb[cm_index(f + 2, lane)] : 0;
-                        c3s += ((mp >> (f + 3)) & 1u) ? cmb[cm_index(f + 3, lane)] : 0;
+                    for (int i = 0; i < 8; i += 2) {
+                        c0 = masked_add4(c0, mv, 4 * i, cv[i]);
+                        c1 = masked_add4(c1, mv, 4 * i + 4, cv[i + 1]);
                     }
-                    dE += (c0 + c1) + (c2 + c3s);
+                    y -= c0 + c1;
                 }
                 PT_ACC(1, t_c);
                 PT_T0(t_s);
-                // the sequential part: lane f's decision is final once steps 0..f-1 are done (cin[f] = 0 for
-                // lanes <= f); if it accepts, every later lane takes the correction
-#ifndef PT_EXP_NOCHAIN
+#ifdef PT_CHAIN_SEQ
+                // the sequential part: lane f's decision is final once steps 0..f-1 are done (its own later
+                // corrections are 0); if it accepts, every later lane takes the correction
 #pragma unroll
                 for (int f = 0; f < 31; ++f) {
-                    const int X = dE + cin[f] + zero;
+                    const int cf = (f & 3) == 0 ? cv[8 + (f >> 2)].x : (f & 3) == 1 ? cv[8 + (f >> 2)].y
+                                 : (f & 3) == 2 ? cv[8 + (f >> 2)].z : cv[8 + (f >> 2)].w;
                     asm volatile(
-                        "{\n\t.reg .pred pf, pq, pa;\n\t"
-                        "setp.eq.s32 pf, %1, %2;\n\t"
-                        "setp.le.and.s32 pq, %0, %3, pf;\n\t"
+                        "{\n\t.reg .pred pq, pa;\n\t.reg .s32 t;\n\t"
+                        "setp.ge.s32 pq, %0, %1;\n\t"
                         "vote.sync.any.pred pa, pq, 0xffffffff;\n\t"
-                        "selp.s32 %0, %4, %0, pa;\n\t}"
-                        : "+r"(dE)
-                        : "r"(lane), "r"(f), "r"(th), "r"(X));
+                        "sub.s32 t, %3, %2;\n\t"
+                        "@pa add.s32 %0, %0, t;\n\t}"
+                        : "+r"(y)
+                        : "r"(K[f]), "r"(cf), "r"(zero));
                 }
+                const unsigned mask = __ballot_sync(0xffffffffu, y >= 0);
+#else
+                // The accept mask a of the block is the unique solution of the triangular system
+                //   a_l = [ y_l - sum_{f<l} a_f cm[32+f][l] >= 0 ]      (cm[32+f][l] = 0 for f >= l),
+                // which the site-by-site order solves by forward substitution.  Here: fixed-point iteration
+                // a <- F(a) from the guess "no correction"; after t rounds the first t bits are exact, so it ends
+                // after at most 32 rounds with exactly the sequential result, and in practice after a few.
+                unsigned mask = __ballot_sync(0xffffffffu, y >= 0);
+                int yy = y;
+                if (mask) {   // nothing accepted at first sight: nothing to correct, the guess is the solution
+                    for (int it = 0; it < 32; ++it) {
+                        const unsigned mv = mask ^ lz;
+                        int c0 = 0, c1 = 0;
+#pragma unroll
+                        for (int i = 0; i < 8; i += 2) {
+                            c0 = masked_add4(c0, mv, 4 * i, cv[8 + i]);
+                            c1 = masked_add4(c1, mv, 4 * i + 4, cv[8 + i + 1]);
+                        }
+                        yy = y - (c0 + c1);
+                        const unsigned m2 = __ballot_sync(0xffffffffu, yy >= 0);
+#ifdef PT_TIMING
+                        tacc[5] += 1;
 #endif
-                const unsigned mask = __ballot_sync(0xffffffffu, dE <= th);
-                PT_ACC(2, t_s);
-                if ((mask >> lane) & 1u) dE_acc += dE;
-                if (lane == 0) { n_acc += __popc(mask); s_mask[k & 1] = mask; }
-                if (lane < 4) {
-                    const int w = (i0 >> 3) + lane;
-                    const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
-                    m.sp[w] = (m.sp[w] & ~nm) | (m.bq[w] & nm);
+                        if (m2 == mask) break;
+                        mask = m2;
+                    }
                 }
+                y = yy;   // slack of every site at its own turn (corrections of later sites are 0)
+#endif
+                PT_ACC(2, t_s);
+                if (lane < 4) {
+                    const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
+                    m.sp[wsp] = (w_old & ~nm) | (w_new & nm);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&s_done[k & 1]);   // block k is final, buffer k&1 is free
+                if ((mask >> lane) & 1u) dE_acc += th - y;
+                n_acc += __popc(mask);
+                mp = mask;
                 PT_ACC(0, t_c);
-                cta_sync();
             }
             for (int o = 16; o > 0; o >>= 1) dE_acc += __shfl_xor_sync(0xffffffffu, dE_acc, o);
             if (lane == 0) { s_dE = dE_acc; s_nacc = n_acc; }
@@ -502,11 +595,12 @@ inline int launch_sweep_direct(const Dev& d, long long sweep0, int n_sweeps, int
                                cudaStream_t stream) {
     const size_t smem = direct_smem_bytes(d.L);
     void (*kern)(Dev, long long, int, int, int) = nullptr;
+    const bool l4096 = d.L == 4096;
     switch (direct_nearq(d.L, r_hi)) {
-        case 1: kern = sweep_direct_kernel<1>; break;
-        case 2: kern = sweep_direct_kernel<2>; break;
-        case 4: kern = sweep_direct_kernel<4>; break;
-        default: kern = sweep_direct_kernel<0>; break;
+        case 1: kern = l4096 ? sweep_direct_kernel<1, true> : sweep_direct_kernel<1, false>; break;
+        case 2: kern = sweep_direct_kernel<2, false>; break;
+        case 4: kern = sweep_direct_kernel<4, false>; break;
+        default: kern = l4096 ? sweep_direct_kernel<0, true> : sweep_direct_kernel<0, false>; break;
     }
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return (int)err;
