@@ -50,7 +50,8 @@
 namespace ptk {
 
 constexpr int DIRECT_MAX_BULK = 512;
-constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 32;  // + the chain warp
+constexpr int DIRECT_CHAIN_WARPS = 4;                       // one per SM sub-partition
+constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 32 * DIRECT_CHAIN_WARPS;
 constexpr int DIRECT_NPAIR = 35;   // packed coupling pairs per thread and half
 constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: the 224 sites (56 quads) around a block
 constexpr int DIRECT_NEAR_QUADS = 56;
@@ -62,7 +63,7 @@ __host__ __device__ inline int direct_bulk_threads(int L) {
     const int t = 8 * (L / 64);
     return t < 32 ? 32 : (t + 31) / 32 * 32;
 }
-__host__ __device__ inline int direct_threads(int L) { return direct_bulk_threads(L) + 32; }
+__host__ __device__ inline int direct_threads(int L) { return direct_bulk_threads(L) + 32 * DIRECT_CHAIN_WARPS; }
 // Near quads per bulk thread (template parameter NEARQ): 0 = the bulk warps sum both halves everywhere.
 __host__ __device__ inline int direct_nearq(int L, int r_hi) {
     const int njr = L / 64;
@@ -219,7 +220,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
     constexpr int NQ = NEARQ ? NEARQ : 1;
     extern __shared__ uint32_t smem_d[];
     const int L = d.L, W = d.W, q = d.q;
-    const int NT = blockDim.x, NTB = NT - 32;
+    const int NT = blockDim.x, NTB = NT - 32 * DIRECT_CHAIN_WARPS;
     const int NB = L >> 5;
     DirectSmem m;
     m.theta = (int32_t*)smem_d;
@@ -237,6 +238,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
     // full[s]: the block sums and correction rows of buffer s are complete (one arrival per bulk warp);
     // done[s]: the chain warp has decided the block of buffer s and written its spins (one arrival).
     __shared__ __align__(8) uint64_t s_full[2], s_done[2];
+    __shared__ __align__(16) int s_xch[2][32][4];   // partial sums exchanged between the chain warps
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int e = blockIdx.x / d.n_rep, t = blockIdx.x % d.n_rep;
@@ -461,7 +463,12 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
         }
 #endif
     } else {
-        // =========================== CHAIN warp ===========================
+        // =========================== CHAIN warps ===========================
+        // Four warps, one per SM sub-partition (a warp gets about a fifth of its scheduler's issue slots next to
+        // four bulk warps, so the work of a block is spread over all four schedulers).  Every warp keeps the
+        // slack y_l of all 32 sites (lane = site); warp cw owns the correction rows f = 8cw..8cw+7 and adds
+        // their part of every masked sum; the parts are exchanged through shared memory (named barrier 1).
+        const int cw = warp - (NTB >> 5);
         // sum_r Jq[r]
         uint32_t rowsum;
         {
@@ -470,14 +477,11 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
             rowsum = __reduce_add_sync(0xffffffffu, acc);
         }
         cta_sync();
-        // A zero the compiler cannot see through: keeps the adds of the sequential part three-input IADD3s on the
-        // ALU pipe (a two-input add may be issued as IMAD.IADD on the FMA pipe, which the bulk warps saturate).
-        const int zero = m.Jz[lane];
-        // lane-select constants of the sequential part: step f compares the slack against 0 in lane f only
-        int K[32];
-#pragma unroll
-        for (int f = 0; f < 32; ++f) K[f] = (lane == f) ? zero : 0x7fffffff;
+        // A per-lane zero the compiler cannot see through: xor-ed into the accept masks it keeps the bit tests
+        // on the ALU pipe (LOP3 -> predicate, SEL) instead of shift pairs on the FMA or uniform pipes.
+        const unsigned lz = (unsigned)m.Jz[lane];
         const int rot = cm_rot(lane);
+        int xb = 0;   // exchange buffer in use
 
         for (int s = 0; s < n_sweeps; ++s) {
             direct_draw(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
@@ -495,60 +499,40 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                 mbar_wait(&s_full[k & 1], (k >> 1) & 1);
                 PT_T0(t_c);
                 const uint32_t S = m.part[(k & 1) * 32 + lane];
-                int4 cv[16];   // cv[0..7]: rows of the previous block, cv[8..15]: rows of the own block
-#pragma unroll
-                for (int i = 0; i < 16; ++i) cv[i] = *reinterpret_cast<const int4*>(cml + ((4 * i + rot) & 63));
-                m.part[(k & 1) * 32 + lane] = 0u;
+                // this warp's 8 rows of the previous block (f = 8cw..) and of the own block (f = 32 + 8cw..)
+                const int4 cp0 = *reinterpret_cast<const int4*>(cml + ((8 * cw + rot) & 63));
+                const int4 cp1 = *reinterpret_cast<const int4*>(cml + ((8 * cw + 4 + rot) & 63));
+                const int4 co0 = *reinterpret_cast<const int4*>(cml + ((32 + 8 * cw + rot) & 63));
+                const int4 co1 = *reinterpret_cast<const int4*>(cml + ((36 + 8 * cw + rot) & 63));
                 // slack y = theta - dE: the site accepts iff y >= 0 (theta <= 2^30 and |dE| < 2^30: no overflow)
                 int y = th - (int)(S - rowsum);
-                const unsigned lz = (unsigned)zero;   // per-lane opaque 0: keeps the masks in vector registers
                 if (mp) {   // changes accepted in block k-1, which the bulk sum saw as it was before
-                    const unsigned mv = mp ^ lz;
-                    int c0 = 0, c1 = 0;
-#pragma unroll
-                    for (int i = 0; i < 8; i += 2) {
-                        c0 = masked_add4(c0, mv, 4 * i, cv[i]);
-                        c1 = masked_add4(c1, mv, 4 * i + 4, cv[i + 1]);
-                    }
-                    y -= c0 + c1;
+                    const unsigned mv = (mp >> (8 * cw)) ^ lz;
+                    const int part = masked_add4(masked_add4(0, mv, 0, cp0), mv, 4, cp1);
+                    s_xch[xb][lane][cw] = part;
+                    asm volatile("bar.sync 1, 128;" ::: "memory");
+                    const int4 pv = *reinterpret_cast<const int4*>(&s_xch[xb][lane][0]);
+                    xb ^= 1;
+                    y -= (pv.x + pv.y) + (pv.z + pv.w);
                 }
                 PT_ACC(1, t_c);
                 PT_T0(t_s);
-#ifdef PT_CHAIN_SEQ
-                // the sequential part: lane f's decision is final once steps 0..f-1 are done (its own later
-                // corrections are 0); if it accepts, every later lane takes the correction
-#pragma unroll
-                for (int f = 0; f < 31; ++f) {
-                    const int cf = (f & 3) == 0 ? cv[8 + (f >> 2)].x : (f & 3) == 1 ? cv[8 + (f >> 2)].y
-                                 : (f & 3) == 2 ? cv[8 + (f >> 2)].z : cv[8 + (f >> 2)].w;
-                    asm volatile(
-                        "{\n\t.reg .pred pq, pa;\n\t.reg .s32 t;\n\t"
-                        "setp.ge.s32 pq, %0, %1;\n\t"
-                        "vote.sync.any.pred pa, pq, 0xffffffff;\n\t"
-                        "sub.s32 t, %3, %2;\n\t"
-                        "@pa add.s32 %0, %0, t;\n\t}"
-                        : "+r"(y)
-                        : "r"(K[f]), "r"(cf), "r"(zero));
-                }
-                const unsigned mask = __ballot_sync(0xffffffffu, y >= 0);
-#else
                 // The accept mask a of the block is the unique solution of the triangular system
                 //   a_l = [ y_l - sum_{f<l} a_f cm[32+f][l] >= 0 ]      (cm[32+f][l] = 0 for f >= l),
                 // which the site-by-site order solves by forward substitution.  Here: fixed-point iteration
                 // a <- F(a) from the guess "no correction"; after t rounds the first t bits are exact, so it ends
-                // after at most 32 rounds with exactly the sequential result, and in practice after a few.
+                // after at most 32 rounds with exactly the sequential result, and in practice after two or three.
                 unsigned mask = __ballot_sync(0xffffffffu, y >= 0);
                 int yy = y;
                 if (mask) {   // nothing accepted at first sight: nothing to correct, the guess is the solution
                     for (int it = 0; it < 32; ++it) {
-                        const unsigned mv = mask ^ lz;
-                        int c0 = 0, c1 = 0;
-#pragma unroll
-                        for (int i = 0; i < 8; i += 2) {
-                            c0 = masked_add4(c0, mv, 4 * i, cv[8 + i]);
-                            c1 = masked_add4(c1, mv, 4 * i + 4, cv[8 + i + 1]);
-                        }
-                        yy = y - (c0 + c1);
+                        const unsigned mv = (mask >> (8 * cw)) ^ lz;
+                        const int part = masked_add4(masked_add4(0, mv, 0, co0), mv, 4, co1);
+                        s_xch[xb][lane][cw] = part;
+                        asm volatile("bar.sync 1, 128;" ::: "memory");
+                        const int4 pv = *reinterpret_cast<const int4*>(&s_xch[xb][lane][0]);
+                        xb ^= 1;
+                        yy = y - ((pv.x + pv.y) + (pv.z + pv.w));
                         const unsigned m2 = __ballot_sync(0xffffffffu, yy >= 0);
 #ifdef PT_TIMING
                         tacc[5] += 1;
@@ -557,28 +541,32 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                         mask = m2;
                     }
                 }
-                y = yy;   // slack of every site at its own turn (corrections of later sites are 0)
-#endif
                 PT_ACC(2, t_s);
-                if (lane < 4) {
-                    const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
-                    m.sp[wsp] = (w_old & ~nm) | (w_new & nm);
+                if (cw == 0) {
+                    if (lane < 4) {
+                        const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
+                        m.sp[wsp] = (w_old & ~nm) | (w_new & nm);
+                    }
+                    m.part[(k & 1) * 32 + lane] = 0u;
                 }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&s_done[k & 1]);   // block k is final, buffer k&1 is free
-                if ((mask >> lane) & 1u) dE_acc += th - y;
-                n_acc += __popc(mask);
+                // every chain warp has read the buffers of block k before buffer k&1 is handed back
+                asm volatile("bar.sync 1, 128;" ::: "memory");
+                if (cw == 0) {
+                    if (lane == 0) mbar_arrive(&s_done[k & 1]);   // block k is final, buffer k&1 is free
+                    if ((mask >> lane) & 1u) dE_acc += th - yy;   // yy: slack of every site at its own turn
+                    n_acc += __popc(mask);
+                }
                 mp = mask;
                 PT_ACC(0, t_c);
             }
             for (int o = 16; o > 0; o >>= 1) dE_acc += __shfl_xor_sync(0xffffffffu, dE_acc, o);
-            if (lane == 0) { s_dE = dE_acc; s_nacc = n_acc; }
+            if (cw == 0 && lane == 0) { s_dE = dE_acc; s_nacc = n_acc; }
             cta_sync();
             direct_nmax(m.sp, W, q, s_cnt);
             cta_sync();
         }
 #ifdef PT_TIMING
-        if (lane == 0 && d.dbg) {
+        if (lane == 0 && d.dbg && warp < 32) {
             tacc[4] = clock64() - t_kernel;
             for (int n = 0; n < 8; ++n) d.dbg[((size_t)blockIdx.x * 32 + warp) * 8 + n] += tacc[n];
         }
