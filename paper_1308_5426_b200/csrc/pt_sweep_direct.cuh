@@ -71,9 +71,9 @@ __host__ __device__ inline int direct_nearq(int L, int r_hi) {
     if (r_hi > DIRECT_NEAR_R || L < 256 || nq > 4) return 0;
     return nq == 3 ? 4 : nq;
 }
-// dynamic smem (32-bit words): theta[L] | lut[2L] | sp[W] | sp0[W] | bq[W] | selb[L/4] | cm[2][64][32] | part[64] | Jz[96]
+// dynamic smem (32-bit words): theta[L] | lut[2L] | sp[W] | sp0[W] | bq[W] | selb[L/4] | part[64] | Jz[96]
 __host__ __device__ inline size_t direct_smem_bytes(int L) {
-    return (size_t)(3 * L + 3 * (L / 8) + L / 4 + 4096 + 64 + 96) * 4;
+    return (size_t)(3 * L + 3 * (L / 8) + L / 4 + 64 + 96) * 4;
 }
 
 __device__ __forceinline__ int dp4a_s32_u32(int a, uint32_t b, int c) {
@@ -108,7 +108,6 @@ struct DirectSmem {
     uint32_t* sp0;    // [W]  spins at the start of the running sweep
     uint32_t* bq;     // [W]  proposed colours
     uint8_t* selb;    // [L]  a0 | b << 4: colour at the start of the sweep and proposed colour
-    int32_t* cm;      // [2][64][32] correction terms of a block, double buffered (see CORR below)
     uint32_t* part;   // [2][32] block sums S_i, double buffered
     int32_t* Jz;      // [96] Jz[n] = 0 for n < 32, Jq[n - 32] above
 };
@@ -158,13 +157,6 @@ __device__ __forceinline__ int direct_nmax(const uint32_t* sp, int W, int q, int
         for (int k = 0; k < q; ++k) nmax = max(nmax, s_cnt[k]);
     return nmax;
 }
-
-// Correction matrix of a block: entry (row f = 0..63, site l = 0..31) at word l*64 + ((f + 4l + 8(l>>3)) & 63).
-// Site-major, so that the chain lane l fetches its 64 entries as 16 LDS.128; the rotation makes both those loads
-// (8 consecutive lanes hit 8 different 16-byte columns) and the bulk threads' stores (8 site groups x 4 consecutive
-// rows per warp hit 32 different banks) conflict-free.
-__device__ __forceinline__ int cm_rot(int l) { return 4 * l + 8 * (l >> 3); }
-__device__ __forceinline__ int cm_index(int f, int l) { return (l << 6) | ((f + cm_rot(l)) & 63); }
 
 #ifdef PT_TIMING
 #define PT_T0(v) const long long v = clock64()
@@ -229,8 +221,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
     m.sp0 = m.sp + W;
     m.bq = m.sp0 + W;
     m.selb = (uint8_t*)(m.bq + W);
-    m.cm = (int32_t*)(m.selb + L);
-    m.part = (uint32_t*)(m.cm + 4096);
+    m.part = (uint32_t*)(m.selb + L);
     m.Jz = (int32_t*)(m.part + 64);
     __shared__ int s_cnt[16];
     __shared__ long long s_dE;
@@ -303,13 +294,6 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                 }
             }
         }
-        // CORR with one row per thread (NJR64): couplings Jq[l + 32 - f] of row f = jr for this thread's 4 sites
-        int Jc[4];
-#pragma unroll
-        for (int mm = 0; mm < 4; ++mm) {
-            const int dist = gbase + 2 * mm + 32 - jr;
-            Jc[mm] = (NJR64 && dist > 0) ? __ldg(d.Jq + dist) : 0;
-        }
         long long E = d.E[x];
         ObsAcc oa;
         cta_sync();
@@ -335,8 +319,6 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                 wn[iq] = ((jr + NJR * iq) >> 1) - 12;
                 wn[iq] += wn[iq] < 0 ? W : 0;
             }
-            int jf = L - 32 + jr;                               // CORR: site of row f = jr
-            jf -= jf >= L ? L : 0;
             for (int kb = 0; kb < NB; ++kb) {
                 // block kb is summed against: blocks < kb-1 final (the chain warp is done with block kb-2, which
                 // also frees buffer kb&1), block kb-1 as at the start of the sweep, blocks >= kb untouched
@@ -358,7 +340,6 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                         const int n = jr + NJR * iq;
                         nword[iq] = NEARQ ? ((n >= 16 && n < 24) ? m.sp0 : m.sp)[wn[iq]] : 0u;
                     }
-                    const uint32_t sf64 = NJR64 ? m.selb[jf] : 0u;
                     // two accumulators per site (even / odd pair of j) keep the IDP.2A chains short
                     uint32_t alo[4] = {0u, 0u, 0u, 0u}, alo2[4] = {0u, 0u, 0u, 0u}, ahi[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
@@ -390,29 +371,6 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                             }
                         }
                     }
-                    // CORR: correction terms of block kb for a change a_f -> b_f accepted at site
-                    // i0 - 32 + f, f = 0..63 (previous block, then own block):
-                    //   cm[f][l] = Jq[l + 32 - f] (s'_l(b_f) - s'_l(a_f))    (0 for l + 32 <= f)
-                    int32_t* cmb = m.cm + (kb & 1) * 2048;
-                    if (NJR64) {
-#pragma unroll
-                        for (int mm = 0; mm < 4; ++mm) {
-                            const uint32_t sv = prmt(lt[mm].x, lt[mm].y, sf64);  // byte 0 = s'_l(a_f), byte 1 = s'_l(b_f)
-                            cmb[cm_index(jr, gbase + 2 * mm)] = Jc[mm] * dp4a_s32_u32(0x000001ff, sv, 0);
-                        }
-                    } else {
-                        for (int f = jr; f < 64; f += NJR) {
-                            int j2 = jf - jr + f;
-                            j2 -= j2 >= L ? L : 0;
-                            const uint32_t sf = m.selb[j2];
-#pragma unroll
-                            for (int mm = 0; mm < 4; ++mm) {
-                                const int l = gbase + 2 * mm;
-                                const uint32_t sv = prmt(lt[mm].x, lt[mm].y, sf);
-                                cmb[cm_index(f, l)] = m.Jz[64 + l - f] * dp4a_s32_u32(0x000001ff, sv, 0);
-                            }
-                        }
-                    }
 #endif
 #pragma unroll
                     for (int mm = 0; mm < 4; ++mm) val[mm] = alo[mm] + alo2[mm] + (ahi[mm] << 16);
@@ -425,8 +383,6 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                         wn[iq] += 4;
                         wn[iq] -= wn[iq] >= W ? W : 0;
                     }
-                    jf += 32;
-                    jf -= jf >= L ? L : 0;
                 }
 #pragma unroll
                 for (int mm = 0; mm < 4; ++mm) {
@@ -480,7 +436,16 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
         // A per-lane zero the compiler cannot see through: xor-ed into the accept masks it keeps the bit tests
         // on the ALU pipe (LOP3 -> predicate, SEL) instead of shift pairs on the FMA or uniform pipes.
         const unsigned lz = (unsigned)m.Jz[lane];
-        const int rot = cm_rot(lane);
+        // CORR: this warp's correction rows for lane = site l.  If site f of the previous block (rows f = 8cw+j)
+        // or of the own block (rows 32 + 8cw + j) accepts a_f -> b_f, dE_l changes by
+        //   Jq[dist] (s'_l(b_f) - s'_l(a_f)),   dist = l + 32 - f  resp.  l - f  (nothing for dist <= 0).
+        int Jp[8], Jo[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int dp = lane + 32 - (8 * cw + j), dn = lane - (8 * cw + j);
+            Jp[j] = __ldg(d.Jq + dp);               // 1 <= dp <= 63 < L
+            Jo[j] = dn > 0 ? __ldg(d.Jq + dn) : 0;
+        }
         int xb = 0;   // exchange buffer in use
 
         for (int s = 0; s < n_sweeps; ++s) {
@@ -491,19 +456,30 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
             uint32_t mp = 0u;   // accept mask of the previous block
             for (int k = 0; k < NB; ++k) {
                 const int i0 = k << 5;
-                const int32_t* cml = m.cm + (k & 1) * 2048 + (lane << 6);
-                // independent of the bulk: threshold, and the words of the block for the final update
+                // independent of the bulk: threshold, the words of the block for the final update, and the
+                // correction rows (from the colours at the start of the sweep and the proposals: selb)
                 const int th = m.theta[i0 + lane];
                 const int wsp = (i0 >> 3) + (lane & 3);
                 const uint32_t w_old = m.sp[wsp], w_new = m.bq[wsp];
+                const uint2 tab = m.lut[i0 + lane];
+                int ipv = i0 - 32 + 8 * cw;
+                ipv += ipv < 0 ? L : 0;
+                const uint2 sfp = *reinterpret_cast<const uint2*>(m.selb + ipv);            // a | b << 4 of 8 sites
+                const uint2 sfo = *reinterpret_cast<const uint2*>(m.selb + i0 + 8 * cw);
+                int cp[8], co[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const uint32_t wp = j < 4 ? sfp.x : sfp.y, wo = j < 4 ? sfo.x : sfo.y;
+                    // selector byte j: nibble 0 = a_f, nibble 1 = b_f (the two higher nibbles pick bytes that the
+                    // dot product weights with 0); byte 0 of the result = s'_l(a_f), byte 1 = s'_l(b_f)
+                    cp[j] = Jp[j] * dp4a_s32_u32(0x000001ff, prmt(tab.x, tab.y, wp >> (8 * (j & 3))), 0);
+                    co[j] = Jo[j] * dp4a_s32_u32(0x000001ff, prmt(tab.x, tab.y, wo >> (8 * (j & 3))), 0);
+                }
+                const int4 cp0 = make_int4(cp[0], cp[1], cp[2], cp[3]), cp1 = make_int4(cp[4], cp[5], cp[6], cp[7]);
+                const int4 co0 = make_int4(co[0], co[1], co[2], co[3]), co1 = make_int4(co[4], co[5], co[6], co[7]);
                 mbar_wait(&s_full[k & 1], (k >> 1) & 1);
                 PT_T0(t_c);
                 const uint32_t S = m.part[(k & 1) * 32 + lane];
-                // this warp's 8 rows of the previous block (f = 8cw..) and of the own block (f = 32 + 8cw..)
-                const int4 cp0 = *reinterpret_cast<const int4*>(cml + ((8 * cw + rot) & 63));
-                const int4 cp1 = *reinterpret_cast<const int4*>(cml + ((8 * cw + 4 + rot) & 63));
-                const int4 co0 = *reinterpret_cast<const int4*>(cml + ((32 + 8 * cw + rot) & 63));
-                const int4 co1 = *reinterpret_cast<const int4*>(cml + ((36 + 8 * cw + rot) & 63));
                 // slack y = theta - dE: the site accepts iff y >= 0 (theta <= 2^30 and |dE| < 2^30: no overflow)
                 int y = th - (int)(S - rowsum);
                 if (mp) {   // changes accepted in block k-1, which the bulk sum saw as it was before
