@@ -233,15 +233,24 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int e = blockIdx.x / d.n_rep, t = blockIdx.x % d.n_rep;
-    const int st = d.perm[blockIdx.x];
-    const size_t x = (size_t)e * d.n_rep + st;
-    uint32_t* g_sp = d.spins + x * W;
+    // Programmatic dependent launch: this grid may start while the previous sweep launch is still draining, and
+    // everything up to PT_AFTER_PREVIOUS_GRID (coupling registers, tables) overlaps with it; what the previous
+    // launch writes (perm, spins, E, obs) is only read behind griddepcontrol.wait.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    size_t x = 0;
+    uint32_t* g_sp = nullptr;
+#define PT_AFTER_PREVIOUS_GRID()                                             \
+    do {                                                                     \
+        asm volatile("griddepcontrol.wait;" ::: "memory");                   \
+        x = (size_t)e * d.n_rep + d.perm[blockIdx.x];                        \
+        g_sp = d.spins + x * W;                                              \
+        for (int w = tid; w < W; w += NT) m.sp[w] = g_sp[w];                 \
+    } while (0)
 #ifdef PT_TIMING
     long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     PT_T0(t_kernel);
 #endif
 
-    for (int w = tid; w < W; w += NT) m.sp[w] = g_sp[w];
     for (int n = tid; n < 96; n += NT) m.Jz[n] = n < 32 ? 0 : d.Jq[n - 32];
     if (tid < 64) m.part[tid] = 0u;
     const double scale = d.thr_scale[t];
@@ -294,6 +303,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                 }
             }
         }
+        PT_AFTER_PREVIOUS_GRID();
         long long E = d.E[x];
         ObsAcc oa;
         cta_sync();
@@ -432,10 +442,6 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
             for (int r = lane; r < L; r += 32) acc += (uint32_t)d.Jq[r];
             rowsum = __reduce_add_sync(0xffffffffu, acc);
         }
-        cta_sync();
-        // A per-lane zero the compiler cannot see through: xor-ed into the accept masks it keeps the bit tests
-        // on the ALU pipe (LOP3 -> predicate, SEL) instead of shift pairs on the FMA or uniform pipes.
-        const unsigned lz = (unsigned)m.Jz[lane];
         // CORR: this warp's correction rows for lane = site l.  If site f of the previous block (rows f = 8cw+j)
         // or of the own block (rows 32 + 8cw + j) accepts a_f -> b_f, dE_l changes by
         //   Jq[dist] (s'_l(b_f) - s'_l(a_f)),   dist = l + 32 - f  resp.  l - f  (nothing for dist <= 0).
@@ -446,6 +452,11 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
             Jp[j] = __ldg(d.Jq + dp);               // 1 <= dp <= 63 < L
             Jo[j] = dn > 0 ? __ldg(d.Jq + dn) : 0;
         }
+        PT_AFTER_PREVIOUS_GRID();
+        cta_sync();
+        // A per-lane zero the compiler cannot see through: xor-ed into the accept masks it keeps the bit tests
+        // on the ALU pipe (LOP3 -> predicate, SEL) instead of shift pairs on the FMA or uniform pipes.
+        const unsigned lz = (unsigned)m.Jz[lane];
         int xb = 0;   // exchange buffer in use
 
         for (int s = 0; s < n_sweeps; ++s) {
@@ -568,7 +579,19 @@ inline int launch_sweep_direct(const Dev& d, long long sweep0, int n_sweeps, int
     }
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return (int)err;
-    kern<<<d.n_ens * d.n_rep, direct_threads(d.L), smem, stream>>>(d, sweep0, n_sweeps, do_swap, r_hi);
+    // programmatic dependent launch: successive sweep launches of a stream overlap their prologue/epilogue
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)(d.n_ens * d.n_rep));
+    cfg.blockDim = dim3((unsigned)direct_threads(d.L));
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    err = cudaLaunchKernelEx(&cfg, kern, d, sweep0, n_sweeps, do_swap, r_hi);
+    if (err != cudaSuccess) return (int)err;
     return (int)cudaGetLastError();
 }
 
