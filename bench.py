@@ -27,9 +27,13 @@ from paper_1308_5426_b200 import inputs  # noqa: E402
 
 METRIC = "Metropolis spin-flip attempts/s at L=4096 q=8 128 replicas"
 UNIT = "attempts/s"
-# IDP.2A issue rate assumed for the ALU roofline (lanes per clock per SM on the FMA-heavy pipe:
-# B300_MICROARCH.md "Pipe rates": rt_SMSP = 2 -> 16 lanes/clk/SMSP x 4 SMSPs); DESIGN.md section 6.
+# ALU roofline: the algorithmic work of one attempt is L pair terms, each ONE integer
+# multiply-accumulate (16-bit coupling half x 8-bit weight); IDP.2A does two of them per lane and issues at a measured
+# 64 lanes/clk/SM on the FMA-heavy pipe (profiles/r1_a_direct_v1a.md), so peak = 148 SMs x 64 x 2 MAC x f_SM.
 IDP_LANES_PER_CLK_PER_SM = 64
+MACS_PER_IDP_LANE = 2
+# dram__bytes_read.sum + dram__bytes_write.sum of one sweep_direct_kernel launch (ncu --set full, profiles/r1_c_direct_v5.md)
+DRAM_BYTES_PER_LAUNCH = 417.0e3
 N_SM = 148
 
 
@@ -72,6 +76,14 @@ class ClockSampler(threading.Thread):
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "error": self.err}
         return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.max_mhz, "samples": len(self.sm),
                 "reasons": [n for b, n in self.REASONS.items() if self.mask & b]}
+
+
+def measured_hbm_gbs():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"])
+    except Exception:
+        return 6650.0   # fallback stated in the profiling guide
 
 
 def oracle_threads():
@@ -219,16 +231,20 @@ def run_ours(args):
 
     if rank == 0:
         f_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
-        pair_terms_per_launch = w.n_rep * w.L * w.L          # one IDP.2A lane-op pair per (i,j) term and 16-bit half
-        launch_s = ms * 1e-3 / max(1, launches)
-        achieved = pair_terms_per_launch / launch_s / 1e12
-        peak = N_SM * IDP_LANES_PER_CLK_PER_SM * 2 / 2 * f_hz / 1e12   # 2 MACs per lane-op, 2 MACs per pair term
-        roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tpair-terms/s", "frac": achieved / peak,
-                    "traffic": None, "kernel": "sweep_%s_kernel" % variant,
-                    "note": "peak = 148 SMs x 64 IDP.2A lanes/clk/SM x sampled SM clock (%.0f MHz), one lane-op per "
-                            "pair term per 16-bit half (DESIGN.md section 6); of derived ALU peak, not of "
-                            "MEASURED_PEAKS.json (HBM/tensor peaks do not bound this path); DRAM traffic per launch is "
-                            "~%d KB of packed spins" % (f_hz / 1e6, 2 * w.n_rep * w.L // 2 // 1024)}
+        macs_per_launch = w.n_rep * w.L * w.L                # one multiply-accumulate per pair term (i, j)
+        launch_s = ms * 1e-3 / max(1, launches)              # CUDA events on the launching stream, K launches
+        achieved = macs_per_launch / launch_s / 1e12
+        peak = N_SM * IDP_LANES_PER_CLK_PER_SM * MACS_PER_IDP_LANE * f_hz / 1e12
+        roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tmac/s", "frac": achieved / peak,
+                    "traffic": DRAM_BYTES_PER_LAUNCH if variant == "direct" else None,
+                    "kernel": "sweep_%s_kernel" % variant,
+                    "note": "algorithmic work = n_rep*L^2 = %.3e integer multiply-accumulates per launch (one per "
+                            "pair term); peak = 148 SMs x 64 IDP.2A lanes/clk/SM (measured issue rate) x 2 MAC x "
+                            "sampled SM clock %.0f MHz -- a derived ALU peak, not MEASURED_PEAKS.json (its HBM and "
+                            "tensor figures do not bound this path: %.0f KB of DRAM traffic per launch = %.2f GB/s "
+                            "of the measured %.0f GB/s); 128 of 148 SMs carry a replica"
+                            % (macs_per_launch, f_hz / 1e6, DRAM_BYTES_PER_LAUNCH / 1e3,
+                               DRAM_BYTES_PER_LAUNCH / launch_s / 1e9, measured_hbm_gbs())}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "int32", "data": "synthetic", "config": workload_config(w, variant, world),

@@ -3,47 +3,55 @@
 // after", an O(L) sum per step, O(L^2) per sweep), organised for sm_100a.
 //
 // One CTA per replica, sites in blocks of 32 (site order 0..L-1, A5).  Warps are
-// specialised and the two halves of a block's work run CONCURRENTLY on
-// consecutive blocks: in interval k (between two CTA barriers)
-//   * the BULK warps sum block k+1 against the spins as they are, and
-//   * one CHAIN warp takes the sequential accept/reject decisions of block k,
-//     while the other chain warp prepares block k+1.
+// specialised: NTB = L/8 threads of BULK warps and four CHAIN warps (one per SM
+// sub-partition), coupled only through two pairs of shared-memory mbarriers, so
+// that the bulk sum of block k+1 runs while block k is being decided.
 //
-// BULK (NTB = L/8 threads).  For the 32 sites i of a block,
+// DRAW (all threads, once per sweep).  Proposals b_i, integer thresholds
+// theta_i (reading A9) and the per-site colour tables of all sites are drawn in
+// parallel from the counter-based generator; sp0 keeps the spins as they are
+// at the start of the sweep.
+//
+// BULK.  For the 32 sites i of a block,
 //   S_i = sum_j Jq[(i-j) mod L] * s'_i(c_j),   s'_i(k) = 1 + [k==a_i] - [k==b_i],
 // so that dE_i = S_i - sum_r Jq[r]  (Jq is symmetric, so (i-j) mod L indexes the
 // same coupling as |i-j|; Jq[0] = 0 drops j == i).  The 32 x L pair terms of a
 // block are split as 8 site groups (4 sites of equal parity) x L/64 ranges of
 // 64 consecutive j, one (group, range) per thread.  The range is taken RELATIVE
-// to the block start, so the 70 couplings a thread needs never change: they
-// live in registers for the whole launch as 16-bit halves packed in pairs
+// to the block start, so the couplings a thread needs never change: they live
+// in registers for the whole launch as 16-bit halves packed in pairs
 // (pt_kernels.cuh: pack_pairs_kernel).  Per 4 sites j the colour -> s' map is
 // one PRMT (the packed 4-bit colours ARE the byte selectors of a per-site 8-byte
 // table; hence q <= 8) and the multiply-accumulate is IDP.2A (16-bit x 8-bit
 // two-way dot products), all integer, exact.  The HIGH halves Jq[r] >> 16 are
-// non-zero only for r <= r_hi (71 at L=4096, sigma=0.3): with FULL_HI = false
-// the bulk warps sum the low halves only (0.5 IDP.2A per pair term) and the
-// high halves of the 224 sites around the block are summed by the preparing
-// chain warp (NEAR); FULL_HI = true keeps both halves in the bulk warps (small
-// L or small sigma, where r_hi is not small).
+// non-zero only for r <= r_hi (71 at L=4096, sigma=0.3): with NEARQ != 0 the
+// main loop sums the low halves only (0.5 IDP.2A per pair term) and each thread
+// adds the high halves of NEARQ of the 56 quads of sites within distance 95 of
+// the block (NEAR); NEARQ = 0 keeps both halves everywhere (small L or sigma).
+// Block sums are reduced with shuffles and shared-memory atomics; every bulk
+// warp then arrives on full[k&1].  Before block k a bulk warp waits on
+// done[k&1] (block k-2 decided), so it reads: blocks < k-1 final, block k-1 as
+// it was at the START of the sweep (sp0; it may still be changing), blocks >= k
+// untouched.
 //
-// Because block k+1 is summed while block k is still being decided, the bulk
-// reads block k as it was at the START of the sweep (sp0) and everything else
-// live (sp): blocks < k are final, blocks > k untouched.  The chain warp then
-// corrects for the changes accepted in block k exactly like for those inside
-// its own block:
-//
-// CHAIN (lane = site).  With dE_l valid for the stale configuration, the
-// sequential acceptance of Eq. 8 needs, for every accepted
-// change f: a_f -> b_f at an earlier site, the exact correction
-//   dE_l += Jq[l-f] * ( s'_l(b_f) - s'_l(a_f) ),
-// 32 predicated adds for the previous block (all known at once) and 32
-// dependent steps "vote on lane f, add its correction" inside the block.  The
-// 64 correction terms of a lane are computed ahead of time (PREP) while the
-// other chain warp is deciding the previous block.  Integer arithmetic makes
-// the result identical to the site-by-site order.  Proposals b_i and
-// thresholds theta_i (reading A9) of all sites are drawn in parallel at the
-// start of the sweep from the counter-based generator.
+// CHAIN (lane = site l, every chain warp holds all 32 slacks y_l = theta_l - dE_l).
+// For an accepted change a_f -> b_f at an earlier site f, dE_l changes by
+//   cm[f][l] = Jq[l-f] * ( s'_l(b_f) - s'_l(a_f) )          (exact, integer).
+// Chain warp cw computes the rows f = 8cw..8cw+7 of the previous block (whose
+// changes the bulk did not see) and of the own block from registers (CORR:
+// PRMT + IDP.4A + IMAD per entry, before it waits on full[k&1]).  The accept
+// mask a of the block is the unique solution of the triangular system
+//   a_l = [ y_l - sum_{f<l} a_f cm[f][l] >= 0 ],
+// which the site-by-site order of Eq. 8 solves by forward
+// substitution.  Here it is solved by fixed-point rounds a <- F(a) starting
+// from "no correction": after t rounds the first t bits are exact, so at most
+// 32 rounds give exactly the sequential result; measured: 2.5 rounds per block
+// for the hottest replica of configs[3], 0-1 for cold ones.  A round is a masked
+// sum of 8 rows per warp (LOP3 -> predicate, SEL, IADD3: ALU pipe only, the FMA
+// pipe is saturated by BULK), an exchange of the four partial sums through
+// shared memory (named barrier 1) and a ballot.  Chain warp 0 writes the new
+// spins and arrives on done[k&1].  Integer arithmetic makes all of this
+// independent of the order of summation (parity tests: bit-identical).
 #pragma once
 #include "pt_kernels.cuh"
 
@@ -204,7 +212,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 
 // NEARQ = 0: the bulk warps sum both 16-bit halves of every coupling.  NEARQ = 1, 2, 4: they sum the low halves
 // only, plus the high halves of NEARQ of the 56 quads of sites within distance 95 of the block (requires
-// r_hi <= 95 and NEARQ * L/64 >= 56).  NJR64: L == 4096 (64 j-ranges), one CORR row per thread, straight-line code.
+// r_hi <= 95 and NEARQ * L/64 >= 56).  NJR64: L == 4096 (64 j-ranges as a compile-time constant).
 template <int NEARQ, bool NJR64>
 __global__ void __launch_bounds__(DIRECT_MAX_THREADS, 1)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi) {
@@ -226,8 +234,8 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
     __shared__ int s_cnt[16];
     __shared__ long long s_dE;
     __shared__ int s_nacc;
-    // full[s]: the block sums and correction rows of buffer s are complete (one arrival per bulk warp);
-    // done[s]: the chain warp has decided the block of buffer s and written its spins (one arrival).
+    // full[s]: the block sums of buffer s are complete (one arrival per bulk warp);
+    // done[s]: the chain warps have decided the block of buffer s and written its spins (one arrival).
     __shared__ __align__(8) uint64_t s_full[2], s_done[2];
     __shared__ __align__(16) int s_xch[2][32][4];   // partial sums exchanged between the chain warps
 
