@@ -33,7 +33,7 @@ UNIT = "attempts/s"
 IDP_LANES_PER_CLK_PER_SM = 64
 MACS_PER_IDP_LANE = 2
 # dram__bytes_read.sum + dram__bytes_write.sum of one sweep_direct_kernel launch (ncu --set full, profiles/r1_c_direct_v5.md)
-DRAM_BYTES_PER_LAUNCH = 417.0e3
+DRAM_BYTES_PER_LAUNCH = 399.0e3
 N_SM = 148
 
 
@@ -161,7 +161,7 @@ def run_ours(args):
     import torch.distributed as dist
     from paper_1308_5426_b200 import build as ptbuild
     ptbuild.build()
-    from paper_1308_5426_b200 import pt
+    from paper_1308_5426_b200 import pt, shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -175,7 +175,8 @@ def run_ours(args):
     w = inputs.config(3)
     betas = inputs.betas(w)
     K, W_ = args.steps, args.warmup
-    g = pt.PT(w.L, w.q, w.sigma, 1, w.n_rep, betas, w.seed, ens_base=rank, variant=args.variant)
+    ens_base, n_ens_local = shard.ensemble_shard(world, world, rank)   # one configs[3] ensemble per GPU
+    g = pt.PT(w.L, w.q, w.sigma, n_ens_local, w.n_rep, betas, w.seed, ens_base=ens_base, variant=args.variant)
     variant = g.get_variant()
     stream = torch.cuda.Stream()
     g.use_torch_stream(stream)
@@ -201,9 +202,7 @@ def run_ours(args):
         clocks = sampler.result()
     ms = ev0.elapsed_time(ev1)
     if world > 1:
-        tmax = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms = float(tmax.item())
+        ms = shard.max_over_ranks(ms, dist, device="cuda")
     attempts_per_gpu = K * w.n_rep * w.L
     value = world * attempts_per_gpu / (ms * 1e-3)
     obs = g.observables()
@@ -221,9 +220,7 @@ def run_ours(args):
     barrier()
     e2e_s = time.perf_counter() - t0
     if world > 1:
-        tmax = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        e2e_s = float(tmax.item())
+        e2e_s = shard.max_over_ranks(e2e_s, dist, device="cuda")
     assert spins.shape == start.shape and E.size == w.n_rep and ob["n_samples"].min() > 0
     e2e = {"value": world * attempts_per_gpu / e2e_s, "unit": UNIT,
            "h2d_bytes_per_step": start.nbytes / K, "d2h_bytes_per_step": (spins.nbytes + E.nbytes + w.n_rep * 88) / K,

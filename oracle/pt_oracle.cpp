@@ -129,6 +129,7 @@ struct Replica {
 
 struct Ctx {
     int L, q, n_ens, n_rep;
+    int ens_base = 0;           // global index of this context's first ensemble (enters the RNG counter only)
     double sigma;
     uint64_t seed;
     uint32_t key[2];
@@ -177,7 +178,7 @@ void metropolis_cycle(Ctx& C, int e, int t, bool field) {
     const int q = C.q, L = C.L;
     for (int i = 0; i < L; ++i) {
         const uint32_t ctr[4] = {(uint32_t)i, (uint32_t)C.sweep, (uint32_t)t,
-                                 ((uint32_t)e << 4) | TAG_SWEEP};
+                                 ((uint32_t)(C.ens_base + e) << 4) | TAG_SWEEP};
         uint32_t w[4];
         philox4x32_10(ctr, C.key, w);
         const int a = R.c[i];
@@ -233,7 +234,7 @@ void swap_event(Ctx& C, int e) {
             Replica& Rb = C.rep[(size_t)e * C.n_rep + t + 1];
             Obs& O = C.obs[(size_t)e * C.n_rep + t];
             const double d = (C.beta[t] - C.beta[t + 1]) * ldexp((double)(Ra.E - Rb.E), -24);
-            const uint32_t ctr[4] = {(uint32_t)t, (uint32_t)C.sweep, 0u, ((uint32_t)e << 4) | TAG_SWAP};
+            const uint32_t ctr[4] = {(uint32_t)t, (uint32_t)C.sweep, 0u, ((uint32_t)(C.ens_base + e) << 4) | TAG_SWAP};
             uint32_t w[4];
             philox4x32_10(ctr, C.key, w);
             const double u = uniform53(w[1], w[2]);
@@ -278,7 +279,9 @@ int orc_philox(const uint32_t* ctr, const uint32_t* key, uint32_t* out) {
 double orc_uniform53(uint32_t w1, uint32_t w2) { return uniform53(w1, w2); }
 
 // Returns NULL on invalid arguments (same validity rules as include/pt.h).
-void* orc_create(int L, int q, double sigma, int n_ens, int n_rep, const double* betas, uint64_t seed) {
+void* orc_create_ex(int L, int q, double sigma, int n_ens, int n_rep, const double* betas, uint64_t seed,
+                    int ens_base) {
+    if (ens_base < 0) return nullptr;
     if (L < 2 || (L % 8) != 0 || q < 2 || q > 16 || !(sigma > 0.0) || !std::isfinite(sigma) ||
         n_ens < 1 || n_rep < 1 || !betas)
         return nullptr;
@@ -286,6 +289,7 @@ void* orc_create(int L, int q, double sigma, int n_ens, int n_rep, const double*
         if (!(betas[t] >= 0.0) || !std::isfinite(betas[t])) return nullptr;
     Ctx* C = new Ctx;
     C->L = L; C->q = q; C->sigma = sigma; C->n_ens = n_ens; C->n_rep = n_rep; C->seed = seed;
+    C->ens_base = ens_base;
     C->key[0] = (uint32_t)seed; C->key[1] = (uint32_t)(seed >> 32);
     C->beta.assign(betas, betas + n_rep);
     couplings(L, sigma, C->Jq);
@@ -300,7 +304,7 @@ void* orc_create(int L, int q, double sigma, int n_ens, int n_rep, const double*
             Replica& R = C->rep[(size_t)e * n_rep + t];
             R.c.resize(L);
             for (int i = 0; i < L; ++i) {
-                const uint32_t ctr[4] = {(uint32_t)i, 0u, (uint32_t)t, ((uint32_t)e << 4) | TAG_INIT};
+                const uint32_t ctr[4] = {(uint32_t)i, 0u, (uint32_t)t, ((uint32_t)(C->ens_base + e) << 4) | TAG_INIT};
                 uint32_t w[4];
                 philox4x32_10(ctr, C->key, w);
                 R.c[i] = (uint8_t)mulhi32(w[0], (uint32_t)q);
@@ -308,6 +312,10 @@ void* orc_create(int L, int q, double sigma, int n_ens, int n_rep, const double*
             R.E = total_energy(*C, R.c);
         }
     return C;
+}
+
+void* orc_create(int L, int q, double sigma, int n_ens, int n_rep, const double* betas, uint64_t seed) {
+    return orc_create_ex(L, q, sigma, n_ens, n_rep, betas, seed, 0);
 }
 
 void orc_destroy(void* h) { delete (Ctx*)h; }

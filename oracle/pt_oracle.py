@@ -53,6 +53,8 @@ def lib():
         L.orc_uniform53.restype = dbl
         L.orc_create.argtypes = [i32, i32, dbl, i32, i32, vp, u64]
         L.orc_create.restype = vp
+        L.orc_create_ex.argtypes = [i32, i32, dbl, i32, i32, vp, u64, i32]
+        L.orc_create_ex.restype = vp
         L.orc_destroy.argtypes = [vp]
         L.orc_destroy.restype = None
         L.orc_sweeps.argtypes = [vp, i64, i32, i32, i32]
@@ -101,13 +103,13 @@ def uniform53(w1, w2):
 class Oracle:
     """Same call names as the product binding, CPU only."""
 
-    def __init__(self, L, q, sigma, n_ens, n_rep, betas, seed):
+    def __init__(self, L, q, sigma, n_ens, n_rep, betas, seed, ens_base=0):
         b = np.ascontiguousarray(betas, dtype=np.float64)
         if b.shape != (n_rep,):
             raise ValueError("betas must have n_rep entries")
         self.L, self.q, self.n_ens, self.n_rep = L, q, n_ens, n_rep
         self.betas = b
-        self._h = lib().orc_create(L, q, float(sigma), n_ens, n_rep, _p(b), int(seed))
+        self._h = lib().orc_create_ex(L, q, float(sigma), n_ens, n_rep, _p(b), int(seed), int(ens_base))
         if not self._h:
             raise ValueError("orc_create: invalid arguments")
 

@@ -173,6 +173,9 @@ def test_ens_base_shards_ensembles(pt, oracle):
         c.sweeps(50, 1)
     np.testing.assert_array_equal(whole.get_spins(), np.concatenate([lo.get_spins(), hi.get_spins()]))
     np.testing.assert_array_equal(whole.energy(), np.concatenate([lo.energy(), hi.energy()]))
+    o_hi = oracle.Oracle(L, q, 0.5, 2, n_rep, b, 9, ens_base=2)
+    o_hi.sweeps(50, 1)
+    assert_same_state(hi, o_hi, "ens_base=2 shard against the oracle")
 
 
 def test_errors(pt):
