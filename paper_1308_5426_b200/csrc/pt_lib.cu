@@ -90,6 +90,11 @@ void free_ctx(pt_ctx* c) {
 }
 
 int recompute_energy(pt_ctx* c, long long* d_out) {
+    if (ptk::direct_applies(c->L, c->q)) {   // IDP.2A version (pt_sweep_direct.cuh), ~10x faster at L = 4096
+        int rc = ptk::launch_energy_direct(c->dev(), d_out, c->stream);
+        if (rc) return fail(PT_ECUDA, std::string("energy_direct launch: ") + cudaGetErrorString((cudaError_t)rc));
+        return PT_OK;
+    }
     const size_t smem = (size_t)(c->L + c->L / 8) * 4;
     if (smem > 48 * 1024)
         PT_CUDA(cudaFuncSetAttribute(ptk::energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -573,6 +573,92 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
     if (do_swap) arrive_and_swap(d, e, (uint32_t)(sweep0 + n_sweeps));
 }
 
+// ---------------------------------------------------------------------------
+// a6. Total energy with the bulk machinery (Eq. 2 in reading A1):
+//   E = -(1/2) sum_i S_i,   S_i = sum_j Jq[(i-j) mod L] [c_j == c_i]      (Jq[0] = 0 drops j == i).
+// Same thread mapping as BULK (4 sites x 64 j per thread, couplings in registers, both 16-bit halves), the
+// per-site table is the one-hot byte table of the site's own colour.  One CTA per replica (storage order).
+// ---------------------------------------------------------------------------
+__global__ void __launch_bounds__(DIRECT_MAX_BULK, 1)
+energy_direct_kernel(Dev d, long long* __restrict__ E_out) {
+    extern __shared__ uint32_t smem_ed[];
+    uint32_t* sp = smem_ed;   // [W]
+    __shared__ unsigned long long s_tot[DIRECT_MAX_BULK / 32];
+    const int L = d.L, W = d.W;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, NT = blockDim.x;
+    const int g = tid & 7, jr = tid >> 3;
+    const int par = g & 1, gbase = 8 * (g >> 1) + par;
+    const int NJR = L / 64, NB = L >> 5;
+    const bool active = jr < NJR;
+    uint32_t PL[DIRECT_NPAIR], PH[DIRECT_NPAIR];
+    {
+        const int H = L / 2;
+        const int R0 = ((gbase + 6 - 64 * jr) % L + L) % L;
+        const uint32_t* lo = d.Jpair + (size_t)(2 * par) * H;
+        const uint32_t* hi = lo + H;
+#pragma unroll
+        for (int tt = 0; tt < DIRECT_NPAIR; ++tt) {
+            const int r = ((R0 - 2 * tt) % L + L) % L;
+            const int mm = (r - par) / 2;
+            PL[tt] = active ? __ldg(lo + mm) : 0u;
+            PH[tt] = active ? __ldg(hi + mm) : 0u;
+        }
+    }
+    const uint32_t* g_sp = d.spins + (size_t)blockIdx.x * W;
+    for (int w = tid; w < W; w += NT) sp[w] = g_sp[w];
+    __syncthreads();
+    unsigned long long tot = 0ull;
+    if (active) {
+        int wj = 8 * jr;
+        for (int kb = 0; kb < NB; ++kb) {
+            int wj2 = wj + 4;
+            wj2 -= wj2 >= W ? W : 0;
+            const uint4 wa = *reinterpret_cast<const uint4*>(sp + wj);
+            const uint4 wb = *reinterpret_cast<const uint4*>(sp + wj2);
+            const uint32_t words[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
+            uint2 lt[4];
+#pragma unroll
+            for (int mm = 0; mm < 4; ++mm) {   // byte k of the table = [k == c_i]
+                const unsigned long long tab = 1ull << (8 * get_nibble(sp, (kb << 5) + gbase + 2 * mm));
+                lt[mm] = make_uint2((uint32_t)tab, (uint32_t)(tab >> 32));
+            }
+            uint32_t alo[4] = {0u, 0u, 0u, 0u}, alo2[4] = {0u, 0u, 0u, 0u}, ahi[4] = {0u, 0u, 0u, 0u},
+                     ahi2[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
+#pragma unroll
+                for (int mm = 0; mm < 4; ++mm) {
+                    const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
+                    const int tt = 3 - mm + 2 * u;
+                    alo[mm] = __dp2a_lo(PL[tt], S, alo[mm]);
+                    alo2[mm] = __dp2a_hi(PL[tt + 1], S, alo2[mm]);
+                    ahi[mm] = __dp2a_lo(PH[tt], S, ahi[mm]);
+                    ahi2[mm] = __dp2a_hi(PH[tt + 1], S, ahi2[mm]);
+                }
+            }
+#pragma unroll
+            for (int mm = 0; mm < 4; ++mm)
+                tot += (unsigned long long)(alo[mm] + alo2[mm]) + ((unsigned long long)(ahi[mm] + ahi2[mm]) << 16);
+            wj += 4;
+            wj -= wj >= W ? W : 0;
+        }
+    }
+    for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+    if (lane == 0) s_tot[warp] = tot;
+    __syncthreads();
+    if (tid == 0) {
+        unsigned long long t2 = 0ull;
+        for (int k = 0; k < (NT >> 5); ++k) t2 += s_tot[k];
+        E_out[blockIdx.x] = -(long long)(t2 / 2ull);   // the ordered-pair sum is even
+    }
+}
+
+inline int launch_energy_direct(const Dev& d, long long* E_out, cudaStream_t stream) {
+    energy_direct_kernel<<<d.n_ens * d.n_rep, direct_bulk_threads(d.L), (size_t)d.W * 4, stream>>>(d, E_out);
+    return (int)cudaGetLastError();
+}
+
 // Returns a cudaError_t as int.  r_hi = largest r <= L/2 with Jq[r] >= 2^16 (0 if none).
 inline int launch_sweep_direct(const Dev& d, long long sweep0, int n_sweeps, int do_swap, int r_hi,
                                cudaStream_t stream) {
