@@ -216,3 +216,48 @@ def test_dev_pointer_calls_and_torch_stream(pt):
     g.get_spins_dev(sp)
     np.testing.assert_array_equal(E.cpu().numpy().reshape(1, -1), g.energy())
     np.testing.assert_array_equal(sp.cpu().numpy().reshape(1, w.n_rep, w.L), g.get_spins())
+
+
+def _block_means(snaps, key, norm):
+    """Per-slot block means of an accumulator from cumulative snapshots [n_blocks+1][n_rep]."""
+    d = np.diff(np.stack([s[key][0] for s in snaps]).astype(np.float64), axis=0)
+    n = np.diff(np.stack([s["n_samples"][0] for s in snaps]).astype(np.float64), axis=0)
+    return d / n / norm
+
+
+def test_statistics_agree_with_independent_oracle_run(pt, oracle):
+    """configs 3-4 bar (north_star): <E> and <M> within 3 sigma of the oracle's statistics.  Here the two sides run
+    DIFFERENT seeds (different trajectories), on a cfg3-like model small enough for the CPU: L=512, q=8, sigma=0.3,
+    16 replicas; blocked errors from 16 accumulator snapshots; >= 90 % of the slots within 3 sigma, none beyond 5."""
+    L, q, sigma, n_rep = 512, 8, 0.3, 16
+    b = inputs.geometric_betas(0.8, 2.5, n_rep)
+    g = pt.PT(L, q, sigma, 1, n_rep, b, 1001)
+    o = oracle.Oracle(L, q, sigma, 1, n_rep, b, 2002)
+    burn, n_blocks, per_block = 600, 16, 250
+    g.sweeps(burn, 1)
+    o.sweeps(burn, 1, field=True, threads=THREADS)
+    gs, os_ = [g.observables()], [o.observables()]
+    for _ in range(n_blocks):
+        g.sweeps(per_block, 1)
+        o.sweeps(per_block, 1, field=True, threads=THREADS)
+        gs.append(g.observables())
+        os_.append(o.observables())
+    checked = bad3 = 0
+    for key, norm in (("sum_E", L * 16777216.0), ("sum_Nmax", float(L))):
+        bg, bo = _block_means(gs, key, norm), _block_means(os_, key, norm)
+        mg, mo = bg.mean(axis=0), bo.mean(axis=0)
+        sg, so = bg.std(axis=0, ddof=1) / np.sqrt(n_blocks), bo.std(axis=0, ddof=1) / np.sqrt(n_blocks)
+        sigma_c = np.sqrt(sg * sg + so * so) + 1e-12
+        z = np.abs(mg - mo) / sigma_c
+        assert (z < 5.0).all(), "%s: slots beyond 5 sigma: z=%s" % (key, z)
+        checked += z.size
+        bad3 += int((z >= 3.0).sum())
+    assert bad3 <= 0.1 * checked, "%d of %d slot means differ by more than 3 sigma" % (bad3, checked)
+
+
+def test_cfg3_200_sweeps_bit_exact(pt, oracle):
+    w = inputs.config(3)
+    g, o = make_pair(pt, oracle, w, "direct")
+    g.sweeps(200, w.swap_every)
+    o.sweeps(200, w.swap_every, field=True, threads=THREADS)
+    assert_same_state(g, o, "cfg3 after 200 sweeps")
