@@ -59,7 +59,7 @@ typedef enum {
  *                     (PAPER.md:118-124), for blocks of 32 consecutive sites at a
  *                     time, with exact integer corrections for the changes
  *                     accepted inside the block.  Needs L % 64 == 0,
- *                     64 <= L <= 4096, q <= 8 and sum_r Jq[r] < 2^30 - 1.
+ *                     64 <= L <= 4096 and sum_r Jq[r] < 2^30 - 1.
  *  PT_VARIANT_AUTO  : DIRECT where it applies, else FIELD. */
 enum { PT_VARIANT_AUTO = 0, PT_VARIANT_FIELD = 1, PT_VARIANT_DIRECT = 2 };
 

@@ -121,8 +121,8 @@ int resolve_variant(int L, int q, long long rowsum, int variant, int* out) {
     if (variant == PT_VARIANT_AUTO) variant = direct_ok ? PT_VARIANT_DIRECT : PT_VARIANT_FIELD;
     if (variant == PT_VARIANT_DIRECT) {
         if (!direct_ok)
-            return fail(PT_EINVAL, "direct variant needs L % 64 == 0, 64 <= L <= 4096, q <= 8 and sum_r Jq[r] < 2^30 - 1");
-        if (ptk::direct_smem_bytes(L) + 256 > kSmemLimit)
+            return fail(PT_EINVAL, "direct variant needs L % 64 == 0, 64 <= L <= 4096 and sum_r Jq[r] < 2^30 - 1");
+        if (ptk::direct_smem_bytes(L, q) + 256 > kSmemLimit)
             return fail(PT_ECAPACITY, "direct variant does not fit in shared memory for this L");
     } else if (variant == PT_VARIANT_FIELD) {
         if (!field_fits(L, q)) return fail(PT_ECAPACITY, "local-field table (L*q*4 bytes) does not fit in shared memory");

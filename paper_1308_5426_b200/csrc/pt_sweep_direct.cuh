@@ -65,7 +65,7 @@ constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: the 224 sites (56
 constexpr int DIRECT_NEAR_QUADS = 56;
 
 __host__ __device__ inline bool direct_applies(int L, int q) {
-    return (L % 64) == 0 && L >= 64 && L <= 64 * (DIRECT_MAX_BULK / 8) && q <= 8;
+    return (L % 64) == 0 && L >= 64 && L <= 64 * (DIRECT_MAX_BULK / 8) && q <= 16;
 }
 __host__ __device__ inline int direct_bulk_threads(int L) {
     const int t = 8 * (L / 64);
@@ -79,9 +79,9 @@ __host__ __device__ inline int direct_nearq(int L, int r_hi) {
     if (r_hi > DIRECT_NEAR_R || L < 256 || nq > 4) return 0;
     return nq == 3 ? 4 : nq;
 }
-// dynamic smem (32-bit words): theta[L] | lut[2L] | sp[W] | sp0[W] | bq[W] | selb[L/4] | part[64] | Jz[96]
-__host__ __device__ inline size_t direct_smem_bytes(int L) {
-    return (size_t)(3 * L + 3 * (L / 8) + L / 4 + 64 + 96) * 4;
+// dynamic smem (32-bit words): theta[L] | lut[2L] | lutb[2L] (q > 8 only) | sp[W] | sp0[W] | bq[W] | selb[L/4] | part[64] | Jz[96]
+__host__ __device__ inline size_t direct_smem_bytes(int L, int q) {
+    return (size_t)((q > 8 ? 5 : 3) * L + 3 * (L / 8) + L / 4 + 64 + 96) * 4;
 }
 
 __device__ __forceinline__ int dp4a_s32_u32(int a, uint32_t b, int c) {
@@ -95,6 +95,17 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
     uint32_t d;
     asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
     return d;
+}
+
+// Colour -> s' lookup of 4 sites at once: the 4 colour nibbles of `sel` select bytes of the site's table.  Colours
+// 8..15 (Q16) live in a second 8-byte table: a selector nibble with bit 3 set makes PRMT return the replicated sign
+// bit of the selected byte, i.e. 0 for table bytes 0..2, so each PRMT contributes only its own half and the two
+// results are OR-ed (selx = sel ^ 0x8888).
+template <bool Q16>
+__device__ __forceinline__ uint32_t tab_lookup(const uint2& ta, const uint2& tb, uint32_t sel, uint32_t selx) {
+    uint32_t v = prmt(ta.x, ta.y, sel);
+    if (Q16) v |= prmt(tb.x, tb.y, selx);
+    return v;
 }
 
 // 8 accept bits -> 8 nibbles of 0xF
@@ -111,7 +122,8 @@ __device__ __forceinline__ void cta_sync() { asm volatile("bar.sync 0;" ::: "mem
 
 struct DirectSmem {
     int32_t* theta;   // [L]  acceptance thresholds of the running sweep
-    uint2* lut;       // [L]  per-site colour -> s' byte table
+    uint2* lut;       // [L]  per-site colour -> s' byte table, colours 0..7
+    uint2* lutb;      // [L]  colours 8..15 (q > 8 only)
     uint32_t* sp;     // [W]  live packed spins
     uint32_t* sp0;    // [W]  spins at the start of the running sweep
     uint32_t* bq;     // [W]  proposed colours
@@ -138,9 +150,11 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
             bword |= b << (4 * n);
             if (n < 4) s0 |= (a | (b << 4)) << (8 * n); else s1 |= (a | (b << 4)) << (8 * (n - 4));
             m.theta[i] = min(accept_threshold(uniform53(p.w1, p.w2), scale), 1 << 30);  // |dE| < 2^30: same decisions
-            const unsigned long long tab =
-                0x0101010101010101ull + (1ull << (8 * a)) - (1ull << (8 * b));  // byte k = s'(k)
-            m.lut[i] = make_uint2((uint32_t)tab, (uint32_t)(tab >> 32));
+            unsigned long long ta = 0x0101010101010101ull, tb = ta;   // byte k = s'(k), k = 0..7 | 8..15
+            if (a < 8u) ta += 1ull << (8 * a); else tb += 1ull << (8 * (a - 8u));
+            if (b < 8u) ta -= 1ull << (8 * b); else tb -= 1ull << (8 * (b - 8u));
+            m.lut[i] = make_uint2((uint32_t)ta, (uint32_t)(ta >> 32));
+            if (q > 8) m.lutb[i] = make_uint2((uint32_t)tb, (uint32_t)(tb >> 32));
         }
         m.bq[w] = bword;
         m.sp0[w] = word;
@@ -213,7 +227,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 // NEARQ = 0: the bulk warps sum both 16-bit halves of every coupling.  NEARQ = 1, 2, 4: they sum the low halves
 // only, plus the high halves of NEARQ of the 56 quads of sites within distance 95 of the block (requires
 // r_hi <= 95 and NEARQ * L/64 >= 56).  NJR64: L == 4096 (64 j-ranges as a compile-time constant).
-template <int NEARQ, bool NJR64>
+template <int NEARQ, bool NJR64, bool Q16>
 __global__ void __launch_bounds__(DIRECT_MAX_THREADS, 1)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi) {
     constexpr bool FULL_HI = NEARQ == 0;
@@ -225,7 +239,8 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
     DirectSmem m;
     m.theta = (int32_t*)smem_d;
     m.lut = (uint2*)(m.theta + L);
-    m.sp = (uint32_t*)(m.lut + L);
+    m.lutb = m.lut + L;
+    m.sp = (uint32_t*)(m.lut + (Q16 ? 2 * L : L));
     m.sp0 = m.sp + W;
     m.bq = m.sp0 + W;
     m.selb = (uint8_t*)(m.bq + W);
@@ -327,7 +342,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
             PT_ACC(0, t_draw);
             PT_T0(t_loop);
             // per-thread cursors, advanced by one block (32 sites = 4 words) per block
-            const uint2* lutp = m.lut + gbase;
+            const uint2* lutp = m.lut + gbase;   // (table of colours 8..15: L entries further)
             int wj = 8 * jr;                                    // first word of this thread's j-range
             // the second half of the last range is block kb-1, which is being decided: sweep-start copy
             const uint32_t* sp2 = (jr == NJR - 1) ? m.sp0 : m.sp;
@@ -349,9 +364,12 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                     const uint4 wa = *reinterpret_cast<const uint4*>(m.sp + wj);
                     const uint4 wb = *reinterpret_cast<const uint4*>(sp2 + wj2);
                     const uint32_t words[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
-                    uint2 lt[4];
+                    uint2 lt[4], ltb[4];
 #pragma unroll
-                    for (int mm = 0; mm < 4; ++mm) lt[mm] = lutp[2 * mm];
+                    for (int mm = 0; mm < 4; ++mm) {
+                        lt[mm] = lutp[2 * mm];
+                        ltb[mm] = Q16 ? lutp[L + 2 * mm] : make_uint2(0u, 0u);
+                    }
                     uint32_t nword[NQ];
 #pragma unroll
                     for (int iq = 0; iq < NQ; ++iq) {   // quads 16..23 are block kb-1: sweep-start copy
@@ -363,9 +381,10 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
 #pragma unroll
                     for (int u = 0; u < 16; ++u) {
                         const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
+                        const uint32_t selx = sel ^ 0x8888u;
 #pragma unroll
                         for (int mm = 0; mm < 4; ++mm) {
-                            const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
+                            const uint32_t S = tab_lookup<Q16>(lt[mm], ltb[mm], sel, selx);
                             const int tt = 3 - mm + 2 * u;
                             alo[mm] = __dp2a_lo(PL[tt], S, alo[mm]);
                             alo2[mm] = __dp2a_hi(PL[tt + 1], S, alo2[mm]);
@@ -383,7 +402,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                             const uint32_t sel = (n & 1) ? (nword[iq] >> 16) : nword[iq];
 #pragma unroll
                             for (int mm = 0; mm < 4; ++mm) {
-                                const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
+                                const uint32_t S = tab_lookup<Q16>(lt[mm], ltb[mm], sel, sel ^ 0x8888u);
                                 ahi[mm] = __dp2a_lo(NP[iq][mm][0], S, ahi[mm]);
                                 ahi[mm] = __dp2a_hi(NP[iq][mm][1], S, ahi[mm]);
                             }
@@ -481,6 +500,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                 const int wsp = (i0 >> 3) + (lane & 3);
                 const uint32_t w_old = m.sp[wsp], w_new = m.bq[wsp];
                 const uint2 tab = m.lut[i0 + lane];
+                const uint2 tabb = Q16 ? m.lutb[i0 + lane] : make_uint2(0u, 0u);
                 int ipv = i0 - 32 + 8 * cw;
                 ipv += ipv < 0 ? L : 0;
                 const uint2 sfp = *reinterpret_cast<const uint2*>(m.selb + ipv);            // a | b << 4 of 8 sites
@@ -491,8 +511,9 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                     const uint32_t wp = j < 4 ? sfp.x : sfp.y, wo = j < 4 ? sfo.x : sfo.y;
                     // selector byte j: nibble 0 = a_f, nibble 1 = b_f (the two higher nibbles pick bytes that the
                     // dot product weights with 0); byte 0 of the result = s'_l(a_f), byte 1 = s'_l(b_f)
-                    cp[j] = Jp[j] * dp4a_s32_u32(0x000001ff, prmt(tab.x, tab.y, wp >> (8 * (j & 3))), 0);
-                    co[j] = Jo[j] * dp4a_s32_u32(0x000001ff, prmt(tab.x, tab.y, wo >> (8 * (j & 3))), 0);
+                    const uint32_t sp_ = wp >> (8 * (j & 3)), so_ = wo >> (8 * (j & 3));
+                    cp[j] = Jp[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, sp_, sp_ ^ 0x8888u), 0);
+                    co[j] = Jo[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, so_, so_ ^ 0x8888u), 0);
                 }
                 const int4 cp0 = make_int4(cp[0], cp[1], cp[2], cp[3]), cp1 = make_int4(cp[4], cp[5], cp[6], cp[7]);
                 const int4 co0 = make_int4(co[0], co[1], co[2], co[3]), co1 = make_int4(co[4], co[5], co[6], co[7]);
@@ -579,6 +600,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
 // Same thread mapping as BULK (4 sites x 64 j per thread, couplings in registers, both 16-bit halves), the
 // per-site table is the one-hot byte table of the site's own colour.  One CTA per replica (storage order).
 // ---------------------------------------------------------------------------
+template <bool Q16>
 __global__ void __launch_bounds__(DIRECT_MAX_BULK, 1)
 energy_direct_kernel(Dev d, long long* __restrict__ E_out) {
     extern __shared__ uint32_t smem_ed[];
@@ -616,20 +638,24 @@ energy_direct_kernel(Dev d, long long* __restrict__ E_out) {
             const uint4 wa = *reinterpret_cast<const uint4*>(sp + wj);
             const uint4 wb = *reinterpret_cast<const uint4*>(sp + wj2);
             const uint32_t words[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
-            uint2 lt[4];
+            uint2 lt[4], ltb[4];
 #pragma unroll
-            for (int mm = 0; mm < 4; ++mm) {   // byte k of the table = [k == c_i]
-                const unsigned long long tab = 1ull << (8 * get_nibble(sp, (kb << 5) + gbase + 2 * mm));
-                lt[mm] = make_uint2((uint32_t)tab, (uint32_t)(tab >> 32));
+            for (int mm = 0; mm < 4; ++mm) {   // byte k of the table = [k == c_i], colours 0..7 | 8..15
+                const int ci = get_nibble(sp, (kb << 5) + gbase + 2 * mm);
+                const unsigned long long ta = ci < 8 ? 1ull << (8 * ci) : 0ull;
+                const unsigned long long tb = ci < 8 ? 0ull : 1ull << (8 * (ci - 8));
+                lt[mm] = make_uint2((uint32_t)ta, (uint32_t)(ta >> 32));
+                ltb[mm] = make_uint2((uint32_t)tb, (uint32_t)(tb >> 32));
             }
             uint32_t alo[4] = {0u, 0u, 0u, 0u}, alo2[4] = {0u, 0u, 0u, 0u}, ahi[4] = {0u, 0u, 0u, 0u},
                      ahi2[4] = {0u, 0u, 0u, 0u};
 #pragma unroll
             for (int u = 0; u < 16; ++u) {
                 const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
+                const uint32_t selx = sel ^ 0x8888u;
 #pragma unroll
                 for (int mm = 0; mm < 4; ++mm) {
-                    const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
+                    const uint32_t S = tab_lookup<Q16>(lt[mm], ltb[mm], sel, selx);
                     const int tt = 3 - mm + 2 * u;
                     alo[mm] = __dp2a_lo(PL[tt], S, alo[mm]);
                     alo2[mm] = __dp2a_hi(PL[tt + 1], S, alo2[mm]);
@@ -655,21 +681,33 @@ energy_direct_kernel(Dev d, long long* __restrict__ E_out) {
 }
 
 inline int launch_energy_direct(const Dev& d, long long* E_out, cudaStream_t stream) {
-    energy_direct_kernel<<<d.n_ens * d.n_rep, direct_bulk_threads(d.L), (size_t)d.W * 4, stream>>>(d, E_out);
+    if (d.q > 8)
+        energy_direct_kernel<true><<<d.n_ens * d.n_rep, direct_bulk_threads(d.L), (size_t)d.W * 4, stream>>>(d, E_out);
+    else
+        energy_direct_kernel<false><<<d.n_ens * d.n_rep, direct_bulk_threads(d.L), (size_t)d.W * 4, stream>>>(d, E_out);
     return (int)cudaGetLastError();
 }
 
 // Returns a cudaError_t as int.  r_hi = largest r <= L/2 with Jq[r] >= 2^16 (0 if none).
 inline int launch_sweep_direct(const Dev& d, long long sweep0, int n_sweeps, int do_swap, int r_hi,
                                cudaStream_t stream) {
-    const size_t smem = direct_smem_bytes(d.L);
+    const size_t smem = direct_smem_bytes(d.L, d.q);
     void (*kern)(Dev, long long, int, int, int) = nullptr;
     const bool l4096 = d.L == 4096;
-    switch (direct_nearq(d.L, r_hi)) {
-        case 1: kern = l4096 ? sweep_direct_kernel<1, true> : sweep_direct_kernel<1, false>; break;
-        case 2: kern = sweep_direct_kernel<2, false>; break;
-        case 4: kern = sweep_direct_kernel<4, false>; break;
-        default: kern = l4096 ? sweep_direct_kernel<0, true> : sweep_direct_kernel<0, false>; break;
+    if (d.q <= 8) {
+        switch (direct_nearq(d.L, r_hi)) {
+            case 1: kern = l4096 ? sweep_direct_kernel<1, true, false> : sweep_direct_kernel<1, false, false>; break;
+            case 2: kern = sweep_direct_kernel<2, false, false>; break;
+            case 4: kern = sweep_direct_kernel<4, false, false>; break;
+            default: kern = l4096 ? sweep_direct_kernel<0, true, false> : sweep_direct_kernel<0, false, false>; break;
+        }
+    } else {
+        switch (direct_nearq(d.L, r_hi)) {
+            case 1: kern = sweep_direct_kernel<1, false, true>; break;
+            case 2: kern = sweep_direct_kernel<2, false, true>; break;
+            case 4: kern = sweep_direct_kernel<4, false, true>; break;
+            default: kern = sweep_direct_kernel<0, false, true>; break;
+        }
     }
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return (int)err;

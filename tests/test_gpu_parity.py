@@ -261,3 +261,19 @@ def test_cfg3_200_sweeps_bit_exact(pt, oracle):
     g.sweeps(200, w.swap_every)
     o.sweeps(200, w.swap_every, field=True, threads=THREADS)
     assert_same_state(g, o, "cfg3 after 200 sweeps")
+
+
+@pytest.mark.parametrize("L,q,sigma", [(128, 16, 0.6), (256, 9, 0.2), (1024, 12, 0.9), (2048, 9, 0.5)])
+def test_direct_variant_with_more_than_8_colours(pt, oracle, L, q, sigma):
+    """Colours 8..15 use the second 8-byte table of a site (two PRMTs OR-ed); both variants against the oracle."""
+    n_rep = 6
+    b = inputs.geometric_betas(0.5, 2.5, n_rep)
+    for variant in ("direct", "field"):
+        g = pt.PT(L, q, sigma, 2, n_rep, b, 31, variant=variant)
+        assert g.get_variant() == variant
+        o = oracle.Oracle(L, q, sigma, 2, n_rep, b, 31)
+        for n in (3, 20):
+            g.sweeps(n, 1)
+            o.sweeps(n, 1, field=True, threads=THREADS)
+            assert_same_state(g, o, "L=%d q=%d %s" % (L, q, variant))
+        g.close()
