@@ -134,6 +134,7 @@ struct DirectSmem {
 
 // Start of a sweep, all threads: proposals, thresholds and colour tables of all sites (A6, A7, A9) and the
 // snapshot of the spins.
+template <bool Q16>
 __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, uint32_t sweep, int t, uint32_t c3,
                                             double scale) {
     const int W = d.W, q = d.q;
@@ -151,10 +152,10 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
             if (n < 4) s0 |= (a | (b << 4)) << (8 * n); else s1 |= (a | (b << 4)) << (8 * (n - 4));
             m.theta[i] = min(accept_threshold(uniform53(p.w1, p.w2), scale), 1 << 30);  // |dE| < 2^30: same decisions
             unsigned long long ta = 0x0101010101010101ull, tb = ta;   // byte k = s'(k), k = 0..7 | 8..15
-            if (a < 8u) ta += 1ull << (8 * a); else tb += 1ull << (8 * (a - 8u));
-            if (b < 8u) ta -= 1ull << (8 * b); else tb -= 1ull << (8 * (b - 8u));
+            if (!Q16 || a < 8u) ta += 1ull << (8 * a); else tb += 1ull << (8 * (a - 8u));
+            if (!Q16 || b < 8u) ta -= 1ull << (8 * b); else tb -= 1ull << (8 * (b - 8u));
             m.lut[i] = make_uint2((uint32_t)ta, (uint32_t)(ta >> 32));
-            if (q > 8) m.lutb[i] = make_uint2((uint32_t)tb, (uint32_t)(tb >> 32));
+            if (Q16) m.lutb[i] = make_uint2((uint32_t)tb, (uint32_t)(tb >> 32));
         }
         m.bq[w] = bword;
         m.sp0[w] = word;
@@ -333,7 +334,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
 
         for (int s = 0; s < n_sweeps; ++s) {
             PT_T0(t_draw);
-            direct_draw(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
+            direct_draw<Q16>(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
             if (tid == 0) {
                 mbar_init(&s_full[0], NTB >> 5); mbar_init(&s_full[1], NTB >> 5);
                 mbar_init(&s_done[0], 1); mbar_init(&s_done[1], 1);
@@ -394,7 +395,6 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                             }
                         }
                     }
-#ifndef PT_EXP_NOEXTRA
                     if (NEARQ) {
 #pragma unroll
                         for (int iq = 0; iq < NQ; ++iq) {
@@ -408,7 +408,6 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                             }
                         }
                     }
-#endif
 #pragma unroll
                     for (int mm = 0; mm < 4; ++mm) val[mm] = alo[mm] + alo2[mm] + (ahi[mm] << 16);
                     // advance the cursors
@@ -487,7 +486,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
         int xb = 0;   // exchange buffer in use
 
         for (int s = 0; s < n_sweeps; ++s) {
-            direct_draw(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
+            direct_draw<Q16>(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
             cta_sync();
             long long dE_acc = 0;
             int n_acc = 0;
