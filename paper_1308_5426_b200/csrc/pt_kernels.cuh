@@ -14,6 +14,7 @@ using namespace ptdev;
 struct Dev {
     int L, W, q, n_ens, n_rep, ens_base;
     uint32_t key0, key1;
+    uint32_t rowsum;          // sum_r Jq[r] (< 2^31)
     const int32_t* Jq;        // [L]
     const uint32_t* Jpair;    // direct variant: [4][L/2] packed 16-bit halves, see pack_pairs_kernel
     const double* beta;       // [n_rep]

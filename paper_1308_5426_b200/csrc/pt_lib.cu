@@ -69,7 +69,7 @@ struct pt_ctx {
     ptk::Dev dev() const {
         ptk::Dev d;
         d.L = L; d.W = L / 8; d.q = q; d.n_ens = n_ens; d.n_rep = n_rep; d.ens_base = ens_base;
-        d.key0 = (uint32_t)seed; d.key1 = (uint32_t)(seed >> 32);
+        d.key0 = (uint32_t)seed; d.key1 = (uint32_t)(seed >> 32); d.rowsum = (uint32_t)rowsum;
         d.Jq = d_Jq; d.Jpair = d_Jpair; d.beta = d_beta; d.thr_scale = d_scale;
         d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done; d.dbg = d_dbg;
         return d;

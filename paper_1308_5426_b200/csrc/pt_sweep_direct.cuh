@@ -273,6 +273,8 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
 #ifdef PT_TIMING
     long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     PT_T0(t_kernel);
+    unsigned long long gt_start;   // wall clock (ns) at the first instruction: launch gaps = start(n+1) - end(n)
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_start));
 #endif
 
     for (int n = tid; n < 96; n += NT) m.Jz[n] = n < 32 ? 0 : d.Jq[n - 32];
@@ -295,12 +297,14 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
             const int R0 = ((gbase + 6 - 64 * jr) % L + L) % L;
             const uint32_t* lo = d.Jpair + (size_t)(2 * par) * H;
             const uint32_t* hi = lo + H;
+            int r = R0;   // r = R0 - 2 tt (mod L) keeps the parity of `par`: no division or modulo per load
 #pragma unroll
             for (int tt = 0; tt < DIRECT_NPAIR; ++tt) {
-                const int r = ((R0 - 2 * tt) % L + L) % L;
-                const int mm = (r - par) / 2;
+                const int mm = (r - par) >> 1;
                 PL[tt] = active ? __ldg(lo + mm) : 0u;
                 if (FULL_HI) PH[tt] = active ? __ldg(hi + mm) : 0u;
+                r -= 2;
+                r += r < 0 ? L : 0;
             }
             if (!FULL_HI) PH[0] = 0u;
         }
@@ -327,7 +331,9 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                 }
             }
         }
+        PT_T0(t_w);
         PT_AFTER_PREVIOUS_GRID();
+        PT_ACC(6, t_w);
         long long E = d.E[x];
         ObsAcc oa;
         cta_sync();
@@ -461,13 +467,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
         // slack y_l of all 32 sites (lane = site); warp cw owns the correction rows f = 8cw..8cw+7 and adds
         // their part of every masked sum; the parts are exchanged through shared memory (named barrier 1).
         const int cw = warp - (NTB >> 5);
-        // sum_r Jq[r]
-        uint32_t rowsum;
-        {
-            uint32_t acc = 0;
-            for (int r = lane; r < L; r += 32) acc += (uint32_t)d.Jq[r];
-            rowsum = __reduce_add_sync(0xffffffffu, acc);
-        }
+        const uint32_t rowsum = d.rowsum;   // sum_r Jq[r], known to the host since pt_create
         // CORR: this warp's correction rows for lane = site l.  If site f of the previous block (rows f = 8cw+j)
         // or of the own block (rows 32 + 8cw + j) accepts a_f -> b_f, dE_l changes by
         //   Jq[dist] (s'_l(b_f) - s'_l(a_f)),   dist = l + 32 - f  resp.  l - f  (nothing for dist <= 0).
@@ -591,6 +591,17 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
     cta_sync();
     for (int w = tid; w < W; w += NT) g_sp[w] = m.sp[w];
     if (do_swap) arrive_and_swap(d, e, (uint32_t)(sweep0 + n_sweeps));
+#ifdef PT_TIMING
+    if (tid == 0 && d.dbg) {   // per CTA: [31][0] first start, [31][1] last end, [31][2] sum of (end - start), [31][3] launches
+        unsigned long long gt_end;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_end));
+        long long* g = d.dbg + ((size_t)blockIdx.x * 32 + 31) * 8;
+        if (g[3] == 0) g[0] = (long long)gt_start;
+        g[1] = (long long)gt_end;
+        g[2] += (long long)(gt_end - gt_start);
+        g[3] += 1;
+    }
+#endif
 }
 
 // ---------------------------------------------------------------------------
@@ -617,12 +628,14 @@ energy_direct_kernel(Dev d, long long* __restrict__ E_out) {
         const int R0 = ((gbase + 6 - 64 * jr) % L + L) % L;
         const uint32_t* lo = d.Jpair + (size_t)(2 * par) * H;
         const uint32_t* hi = lo + H;
+        int r = R0;
 #pragma unroll
         for (int tt = 0; tt < DIRECT_NPAIR; ++tt) {
-            const int r = ((R0 - 2 * tt) % L + L) % L;
-            const int mm = (r - par) / 2;
+            const int mm = (r - par) >> 1;
             PL[tt] = active ? __ldg(lo + mm) : 0u;
             PH[tt] = active ? __ldg(hi + mm) : 0u;
+            r -= 2;
+            r += r < 0 ? L : 0;
         }
     }
     const uint32_t* g_sp = d.spins + (size_t)blockIdx.x * W;
