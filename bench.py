@@ -228,19 +228,20 @@ def run_ours(args):
 
     if rank == 0:
         f_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
-        macs_per_launch = w.n_rep * w.L * w.L                # one multiply-accumulate per pair term (i, j)
-        launch_s = ms * 1e-3 / max(1, launches)              # CUDA events on the launching stream, K launches
+        # one multiply-accumulate per pair term (i, j); a persistent launch covers all K sweeps (swap events inside)
+        macs_per_launch = K * w.n_rep * w.L * w.L / max(1, launches)
+        launch_s = ms * 1e-3 / max(1, launches)              # CUDA events on the launching stream
         achieved = macs_per_launch / launch_s / 1e12
         peak = N_SM * IDP_LANES_PER_CLK_PER_SM * MACS_PER_IDP_LANE * f_hz / 1e12
         roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tmac/s", "frac": achieved / peak,
                     "traffic": DRAM_BYTES_PER_LAUNCH if variant == "direct" else None,
                     "kernel": "sweep_%s_kernel" % variant,
-                    "note": "algorithmic work = n_rep*L^2 = %.3e integer multiply-accumulates per launch (one per "
-                            "pair term); peak = 148 SMs x 64 IDP.2A lanes/clk/SM (measured issue rate) x 2 MAC x "
+                    "note": "algorithmic work = sweeps*n_rep*L^2 = %.3e integer multiply-accumulates per launch (one per "
+                            "pair term; %d sweeps per launch); peak = 148 SMs x 64 IDP.2A lanes/clk/SM (measured issue rate) x 2 MAC x "
                             "sampled SM clock %.0f MHz -- a derived ALU peak, not MEASURED_PEAKS.json (its HBM and "
                             "tensor figures do not bound this path: %.0f KB of DRAM traffic per launch = %.2f GB/s "
                             "of the measured %.0f GB/s); 128 of 148 SMs carry a replica"
-                            % (macs_per_launch, f_hz / 1e6, DRAM_BYTES_PER_LAUNCH / 1e3,
+                            % (macs_per_launch, K // max(1, launches), f_hz / 1e6, DRAM_BYTES_PER_LAUNCH / 1e3,
                                DRAM_BYTES_PER_LAUNCH / launch_s / 1e9, measured_hbm_gbs())}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

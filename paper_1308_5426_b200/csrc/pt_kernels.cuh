@@ -25,6 +25,8 @@ struct Dev {
     pt_obs* obs;              // [n_ens][n_rep]     slot order
     int32_t* h;               // [n_ens*n_rep][q][L] storage order (field variant)
     unsigned* done;           // [n_ens] arrival counters of the swap event
+    unsigned* gen;            // [n_ens] arrivals at the swap events of the running persistent launch
+    long long* Epub;          // [2][n_ens][n_rep] energies published for those events, by storage index
     long long* dbg;           // PT_TIMING builds: [n_ens*n_rep][32 warps][8] clock sums (else unused)
 };
 
@@ -196,6 +198,8 @@ __global__ void __launch_bounds__(256) build_fields_kernel(Dev d) {
 //   d = (beta_t - beta_{t+1}) (E_t - E_{t+1}) 2^-24 >= 0  or  u < exp(d),
 // u from Philox(t, sweep, 0, e<<4|SWAP).  fp64 throughout, one rounding in d.
 // ---------------------------------------------------------------------------
+// All global reads of state that another CTA may have written go to L2 (__ldcg / atomics): inside a persistent
+// launch the event is run by a different CTA every time and L1 is not coherent.
 __device__ inline void swap_event(const Dev& d, int e, uint32_t sweep) {
     int* perm = d.perm + (size_t)e * d.n_rep;
     const long long* E = d.E + (size_t)e * d.n_rep;
@@ -203,19 +207,20 @@ __device__ inline void swap_event(const Dev& d, int e, uint32_t sweep) {
     const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_SWAP;
     for (int stage = 0; stage < 2; ++stage) {
         for (int t = stage + 2 * (int)threadIdx.x; t + 1 < d.n_rep; t += 2 * (int)blockDim.x) {
-            const int sa = perm[t], sb = perm[t + 1];
+            const int sa = __ldcg(perm + t), sb = __ldcg(perm + t + 1);
             const long long Ea = __ldcg(E + sa), Eb = __ldcg(E + sb);
             const double dd = __dmul_rn(d.beta[t] - d.beta[t + 1], ldexp((double)(Ea - Eb), -24));
             const Philox4 p = philox4x32_10((uint32_t)t, sweep, 0u, c3, d.key0, d.key1);
             const double u = uniform53(p.w1, p.w2);
-            obs[t].swap_attempts += 1;
+            atomicAdd((unsigned long long*)&obs[t].swap_attempts, 1ull);
             if (dd >= 0.0 || u < exp(dd)) {
-                perm[t] = sb;
-                perm[t + 1] = sa;
-                obs[t].swap_accepts += 1;
+                __stcg(perm + t, sb);
+                __stcg(perm + t + 1, sa);
+                atomicAdd((unsigned long long*)&obs[t].swap_accepts, 1ull);
             }
         }
-        __syncthreads();
+        __threadfence_block();
+        asm volatile("bar.sync 0;" ::: "memory");   // all threads of the CTA, also from role-specialised code
     }
 }
 
@@ -273,13 +278,15 @@ struct ObsAcc {
         n += 1; sE += E; sN += nmax; sN2 += (long long)nmax * nmax;
         add_square_128(e2lo, e2hi, E);
     }
+    // Single writer at a time per slot, but successive writers may be different CTAs (persistent launches):
+    // read-modify-write in L2 with atomics.
     __device__ void flush(pt_obs* o) const {
-        o->n_samples += n; o->sum_E += sE; o->sum_Nmax += sN; o->sum_Nmax2 += sN2;
-        o->flip_attempts += att; o->flip_accepts += acc;
-        const unsigned long long nlo = o->sum_E2_lo + e2lo;
-        o->sum_E2_hi = (long long)((unsigned long long)o->sum_E2_hi + (unsigned long long)e2hi +
-                                   (nlo < e2lo ? 1ull : 0ull));
-        o->sum_E2_lo = nlo;
+        typedef unsigned long long u64;
+        atomicAdd((u64*)&o->n_samples, (u64)n); atomicAdd((u64*)&o->sum_E, (u64)sE);
+        atomicAdd((u64*)&o->sum_Nmax, (u64)sN); atomicAdd((u64*)&o->sum_Nmax2, (u64)sN2);
+        atomicAdd((u64*)&o->flip_attempts, (u64)att); atomicAdd((u64*)&o->flip_accepts, (u64)acc);
+        const u64 old = atomicAdd((u64*)&o->sum_E2_lo, e2lo);
+        atomicAdd((u64*)&o->sum_E2_hi, (u64)e2hi + ((old + e2lo < old) ? 1ull : 0ull));
     }
 };
 

@@ -64,6 +64,10 @@ struct pt_ctx {
     unsigned* d_done = nullptr;
     int* d_flag = nullptr;
     long long* d_dbg = nullptr;
+    unsigned* d_gen = nullptr;
+    long long* d_Epub = nullptr;
+    int coresident = -1;   // direct variant: CTAs that fit on the device at once (-1: not asked yet)
+    bool allow_persistent = true;
 
     int R() const { return n_ens * n_rep; }
     ptk::Dev dev() const {
@@ -71,7 +75,7 @@ struct pt_ctx {
         d.L = L; d.W = L / 8; d.q = q; d.n_ens = n_ens; d.n_rep = n_rep; d.ens_base = ens_base;
         d.key0 = (uint32_t)seed; d.key1 = (uint32_t)(seed >> 32); d.rowsum = (uint32_t)rowsum;
         d.Jq = d_Jq; d.Jpair = d_Jpair; d.beta = d_beta; d.thr_scale = d_scale;
-        d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done; d.dbg = d_dbg;
+        d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done; d.dbg = d_dbg; d.gen = d_gen; d.Epub = d_Epub;
         return d;
     }
 };
@@ -85,7 +89,7 @@ void free_ctx(pt_ctx* c) {
     if (!c) return;
     cudaFree(c->d_Jq); cudaFree(c->d_Jpair); cudaFree(c->d_beta); cudaFree(c->d_scale);
     cudaFree(c->d_spins); cudaFree(c->d_E); cudaFree(c->d_Etmp); cudaFree(c->d_Eout);
-    cudaFree(c->d_perm); cudaFree(c->d_obs); cudaFree(c->d_h); cudaFree(c->d_done); cudaFree(c->d_flag); cudaFree(c->d_dbg);
+    cudaFree(c->d_perm); cudaFree(c->d_obs); cudaFree(c->d_h); cudaFree(c->d_done); cudaFree(c->d_flag); cudaFree(c->d_dbg); cudaFree(c->d_gen); cudaFree(c->d_Epub);
     delete c;
 }
 
@@ -133,8 +137,9 @@ int resolve_variant(int L, int q, long long rowsum, int variant, int* out) {
     return PT_OK;
 }
 
-// Enqueue one launch covering n_sweeps sweeps, optionally closed by a swap event.
-int launch_sweeps(pt_ctx* c, int n_sweeps, bool do_swap) {
+// Enqueue one launch covering n_sweeps sweeps.  swap_mode 0: no swap event, 1: one at the end of the launch,
+// 2 (direct variant only): persistent launch with an event after every sweep whose index divides by swap_every.
+int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
     if (c->variant == PT_VARIANT_FIELD) {
         int rc = ensure_fields(c);
         if (rc) return rc;
@@ -144,15 +149,22 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, bool do_swap) {
         const size_t smem = ptk::field_smem_bytes(c->L, c->q);
         PT_CUDA(cudaFuncSetAttribute(ptk::sweep_field_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         ptk::sweep_field_kernel<<<c->R(), ptk::FIELD_THREADS, smem, c->stream>>>(d, (long long)c->sweep, n_sweeps,
-                                                                                 do_swap ? 1 : 0);
+                                                                                 swap_mode == 1 ? 1 : 0);
     } else {
         c->fields_valid = false;
-        int rc = ptk::launch_sweep_direct(d, (long long)c->sweep, n_sweeps, do_swap ? 1 : 0, c->r_hi, c->stream);
+        int rc = ptk::launch_sweep_direct(d, (long long)c->sweep, n_sweeps, swap_mode, swap_every, c->r_hi, c->stream);
         if (rc) return fail(PT_ECUDA, std::string("sweep_direct launch: ") + cudaGetErrorString((cudaError_t)rc));
     }
     PT_CUDA(cudaGetLastError());
     c->sweep += n_sweeps;
     return PT_OK;
+}
+
+// Direct variant: can all replicas be resident at once (persistent launches with in-kernel swap events)?
+bool persistent_ok(pt_ctx* c) {
+    if (c->variant != PT_VARIANT_DIRECT || !c->allow_persistent) return false;
+    if (c->coresident < 0) c->coresident = ptk::direct_max_coresident(c->dev(), c->r_hi, c->device);
+    return c->R() <= c->coresident && c->n_rep <= ptk::DIRECT_MAX_PERSIST_REP;
 }
 
 }  // namespace
@@ -224,6 +236,13 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
     PT_CUDA_C(cudaMalloc(&c->d_flag, sizeof(int)));
     PT_CUDA_C(cudaMemset(c->d_obs, 0, (size_t)R * sizeof(pt_obs)));
     PT_CUDA_C(cudaMemset(c->d_done, 0, (size_t)n_ens * sizeof(unsigned)));
+    PT_CUDA_C(cudaMalloc(&c->d_gen, (size_t)n_ens * sizeof(unsigned)));
+    PT_CUDA_C(cudaMemset(c->d_gen, 0, (size_t)n_ens * sizeof(unsigned)));
+    PT_CUDA_C(cudaMalloc(&c->d_Epub, (size_t)2 * R * sizeof(long long)));
+    {
+        const char* env = getenv("PT_PERSISTENT");   // PT_PERSISTENT=0: one launch per swap interval (A/B, debugging)
+        c->allow_persistent = !(env && env[0] == '0');
+    }
 #ifdef PT_TIMING
     PT_CUDA_C(cudaMalloc(&c->d_dbg, (size_t)R * 32 * 8 * sizeof(long long)));
     PT_CUDA_C(cudaMemset(c->d_dbg, 0, (size_t)R * 32 * 8 * sizeof(long long)));
@@ -288,15 +307,19 @@ int pt_sweeps_async(pt_ctx* c, int64_t n, int swap_every, int64_t* n_launches) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");
     if (n < 0 || swap_every < 0) return fail(PT_EINVAL, "n and swap_every must be >= 0");
     int64_t launches = 0;
-    constexpr int64_t kMaxChunk = 1 << 16;  // sweeps per launch when no swap event intervenes
+    constexpr int64_t kMaxChunk = 1 << 16;  // sweeps per launch
+    const bool persistent = swap_every > 0 && persistent_ok(c);
     while (n > 0) {
         int64_t chunk = n < kMaxChunk ? n : kMaxChunk;
-        bool do_swap = false;
-        if (swap_every > 0) {
+        int swap_mode = 0;
+        if (persistent) {
+            swap_mode = 2;
+        } else if (swap_every > 0) {
             const int64_t to_event = swap_every - (c->sweep % swap_every);
-            if (to_event <= chunk) { chunk = to_event; do_swap = true; }
+            if (to_event <= chunk) { chunk = to_event; swap_mode = 1; }
         }
-        int rc = launch_sweeps(c, (int)chunk, do_swap);
+        if (swap_mode == 2) PT_CUDA(cudaMemsetAsync(c->d_gen, 0, (size_t)c->n_ens * sizeof(unsigned), c->stream));
+        int rc = launch_sweeps(c, (int)chunk, swap_mode, swap_every);
         if (rc) return rc;
         launches += 1;
         n -= chunk;

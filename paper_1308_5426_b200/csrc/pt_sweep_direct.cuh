@@ -63,6 +63,7 @@ constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 32 * DIRECT_CHAIN_WARPS;
 constexpr int DIRECT_NPAIR = 35;   // packed coupling pairs per thread and half
 constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: the 224 sites (56 quads) around a block
 constexpr int DIRECT_NEAR_QUADS = 56;
+constexpr int DIRECT_MAX_PERSIST_REP = 256;   // replicas per ensemble in a persistent launch (static shared arrays)
 
 __host__ __device__ inline bool direct_applies(int L, int q) {
     return (L % 64) == 0 && L >= 64 && L <= 64 * (DIRECT_MAX_BULK / 8) && q <= 16;
@@ -181,6 +182,60 @@ __device__ __forceinline__ int direct_nmax(const uint32_t* sp, int W, int q, int
     return nmax;
 }
 
+// Swap event inside a persistent launch (all CTAs of the ensemble co-resident: cooperative launch; n_rep <=
+// DIRECT_MAX_PERSIST_REP).  Nothing is serialised in one CTA: every CTA publishes its energy (Epub, double buffered by
+// event parity), arrives on the ensemble's counter gen[e] (zeroed by the host before the launch), waits until all
+// n_rep arrivals of this event are in, fetches all energies and evaluates the whole event (Eq. 9; even pairs, then odd
+// pairs) on its OWN copy of the slot -> storage permutation in shared memory: the decisions are a pure
+// function of (energies, permutation, Philox(slot, sweep)), so all copies stay identical.  The CTA that holds storage 0
+// also counts the attempts/acceptances.  Returns the slot the configuration with storage index st now occupies.
+// Called by ALL threads of the CTA.
+struct PersistSmem {
+    int* perm;          // [n_rep] slot -> storage
+    long long* Eall;    // [n_rep] energies by storage index
+    int* slot;          // result
+};
+__device__ __forceinline__ int direct_swap_in_kernel(const Dev& d, const PersistSmem& ps, int e, uint32_t sweep, int st,
+                                                     long long E_mine, int event) {
+    const int n_rep = d.n_rep;
+    long long* Epub = d.Epub + ((size_t)(event & 1) * d.n_ens + e) * n_rep;
+    if (threadIdx.x == 0) {
+        __stcg(Epub + st, E_mine);
+        __threadfence();
+        atomicAdd(d.gen + e, 1u);
+        const unsigned target = (unsigned)n_rep * (unsigned)(event + 1);
+        unsigned g = 0u, spins = 0u;
+        while (true) {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(g) : "l"(d.gen + e) : "memory");
+            if (g >= target) break;
+            if (++spins > (1u << 22)) __trap();   // seconds: a CTA of the ensemble is missing
+        }
+    }
+    cta_sync();
+    for (int t2 = threadIdx.x; t2 < n_rep; t2 += blockDim.x) ps.Eall[t2] = __ldcg(Epub + t2);
+    cta_sync();
+    const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_SWAP;
+    pt_obs* obs = d.obs + (size_t)e * n_rep;
+    for (int stage = 0; stage < 2; ++stage) {
+        for (int t2 = stage + 2 * (int)threadIdx.x; t2 + 1 < n_rep; t2 += 2 * (int)blockDim.x) {
+            const int sa = ps.perm[t2], sb = ps.perm[t2 + 1];
+            const double dd = __dmul_rn(d.beta[t2] - d.beta[t2 + 1], ldexp((double)(ps.Eall[sa] - ps.Eall[sb]), -24));
+            const Philox4 p = philox4x32_10((uint32_t)t2, sweep, 0u, c3, d.key0, d.key1);
+            const bool acc = dd >= 0.0 || uniform53(p.w1, p.w2) < exp(dd);
+            if (acc) { ps.perm[t2] = sb; ps.perm[t2 + 1] = sa; }
+            if (st == 0) {
+                atomicAdd((unsigned long long*)&obs[t2].swap_attempts, 1ull);
+                if (acc) atomicAdd((unsigned long long*)&obs[t2].swap_accepts, 1ull);
+            }
+        }
+        cta_sync();
+    }
+    for (int t2 = threadIdx.x; t2 < n_rep; t2 += blockDim.x)
+        if (ps.perm[t2] == st) *ps.slot = t2;
+    cta_sync();
+    return *ps.slot;
+}
+
 #ifdef PT_TIMING
 #define PT_T0(v) const long long v = clock64()
 #define PT_ACC(slot, v) tacc[slot] += clock64() - (v)
@@ -230,7 +285,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 // r_hi <= 95 and NEARQ * L/64 >= 56).  NJR64: L == 4096 (64 j-ranges as a compile-time constant).
 template <int NEARQ, bool NJR64, bool Q16>
 __global__ void __launch_bounds__(DIRECT_MAX_THREADS, 1)
-sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi) {
+sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi) {
+    // swap_mode 0: no swap event; 1: one event at the end of the launch (last-arriving CTA, nobody waits);
+    // 2: persistent launch, an event inside the kernel after every sweep whose index is a multiple of swap_every.
     constexpr bool FULL_HI = NEARQ == 0;
     constexpr int NQ = NEARQ ? NEARQ : 1;
     extern __shared__ uint32_t smem_d[];
@@ -250,25 +307,40 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
     __shared__ int s_cnt[16];
     __shared__ long long s_dE;
     __shared__ int s_nacc;
+    __shared__ int s_slot;
+    __shared__ int s_perm[DIRECT_MAX_PERSIST_REP];
+    __shared__ long long s_Eall[DIRECT_MAX_PERSIST_REP];
+    __shared__ double s_scale[DIRECT_MAX_PERSIST_REP];
+    PersistSmem ps;
+    ps.perm = s_perm; ps.Eall = s_Eall; ps.slot = &s_slot;
+    int event = 0;   // swap events so far in this (persistent) launch
     // full[s]: the block sums of buffer s are complete (one arrival per bulk warp);
     // done[s]: the chain warps have decided the block of buffer s and written its spins (one arrival).
     __shared__ __align__(8) uint64_t s_full[2], s_done[2];
     __shared__ __align__(16) int s_xch[2][32][4];   // partial sums exchanged between the chain warps
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int e = blockIdx.x / d.n_rep, t = blockIdx.x % d.n_rep;
+    const int e = blockIdx.x / d.n_rep;
+    int t = blockIdx.x % d.n_rep;   // slot (temperature) of this CTA's configuration; moves in swap_mode 2
     // Programmatic dependent launch: this grid may start while the previous sweep launch is still draining, and
     // everything up to PT_AFTER_PREVIOUS_GRID (coupling registers, tables) overlaps with it; what the previous
     // launch writes (perm, spins, E, obs) is only read behind griddepcontrol.wait.
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     size_t x = 0;
+    int st = 0;
     uint32_t* g_sp = nullptr;
 #define PT_AFTER_PREVIOUS_GRID()                                             \
     do {                                                                     \
         asm volatile("griddepcontrol.wait;" ::: "memory");                   \
-        x = (size_t)e * d.n_rep + d.perm[blockIdx.x];                        \
+        st = d.perm[blockIdx.x];                                             \
+        x = (size_t)e * d.n_rep + st;                                        \
         g_sp = d.spins + x * W;                                              \
         for (int w = tid; w < W; w += NT) m.sp[w] = g_sp[w];                 \
+        if (swap_mode == 2)                                                  \
+            for (int t2 = tid; t2 < d.n_rep; t2 += NT) {                     \
+                s_perm[t2] = d.perm[(size_t)e * d.n_rep + t2];               \
+                s_scale[t2] = d.thr_scale[t2];                               \
+            }                                                                \
     } while (0)
 #ifdef PT_TIMING
     long long tacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -279,7 +351,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
 
     for (int n = tid; n < 96; n += NT) m.Jz[n] = n < 32 ? 0 : d.Jq[n - 32];
     if (tid < 64) m.part[tid] = 0u;
-    const double scale = d.thr_scale[t];
+    double scale = d.thr_scale[t];
     const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_SWEEP;
 
     if (tid < NTB) {
@@ -451,9 +523,20 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
                 oa.sample(E, nmax);
             }
             cta_sync();
+            if (swap_mode == 2 && (sweep0 + s + 1) % swap_every == 0) {
+                const int t_new = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, E, event++);
+                if (t_new != t) {   // the accumulators belong to the slot: hand them over when the slot changes
+                    if (tid == 0) {
+                        oa.flush(d.obs + (size_t)e * d.n_rep + t);
+                        oa = ObsAcc();
+                    }
+                    t = t_new;
+                    scale = s_scale[t];
+                }
+            }
             PT_ACC(3, t_end);
         }
-        if (tid == 0) { d.E[x] = E; oa.flush(d.obs + blockIdx.x); }
+        if (tid == 0) { d.E[x] = E; oa.flush(d.obs + (size_t)e * d.n_rep + t); }
 #ifdef PT_TIMING
         if (lane == 0 && d.dbg) {
             tacc[4] = clock64() - t_kernel;
@@ -579,6 +662,10 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
             cta_sync();
             direct_nmax(m.sp, W, q, s_cnt);
             cta_sync();
+            if (swap_mode == 2 && (sweep0 + s + 1) % swap_every == 0) {
+                t = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, 0, event++);
+                scale = s_scale[t];
+            }
         }
 #ifdef PT_TIMING
         if (lane == 0 && d.dbg && warp < 32) {
@@ -590,7 +677,9 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap, int r_hi
 
     cta_sync();
     for (int w = tid; w < W; w += NT) g_sp[w] = m.sp[w];
-    if (do_swap) arrive_and_swap(d, e, (uint32_t)(sweep0 + n_sweeps));
+    if (swap_mode == 1) arrive_and_swap(d, e, (uint32_t)(sweep0 + n_sweeps));
+    if (swap_mode == 2 && st == 0)   // all copies are identical: one CTA per ensemble writes the permutation back
+        for (int t2 = tid; t2 < d.n_rep; t2 += NT) d.perm[(size_t)e * d.n_rep + t2] = s_perm[t2];
 #ifdef PT_TIMING
     if (tid == 0 && d.dbg) {   // per CTA: [31][0] first start, [31][1] last end, [31][2] sum of (end - start), [31][3] launches
         unsigned long long gt_end;
@@ -700,41 +789,65 @@ inline int launch_energy_direct(const Dev& d, long long* E_out, cudaStream_t str
     return (int)cudaGetLastError();
 }
 
-// Returns a cudaError_t as int.  r_hi = largest r <= L/2 with Jq[r] >= 2^16 (0 if none).
-inline int launch_sweep_direct(const Dev& d, long long sweep0, int n_sweeps, int do_swap, int r_hi,
-                               cudaStream_t stream) {
-    const size_t smem = direct_smem_bytes(d.L, d.q);
-    void (*kern)(Dev, long long, int, int, int) = nullptr;
+typedef void (*direct_kernel_t)(Dev, long long, int, int, int, int);
+
+// r_hi = largest r <= L/2 with Jq[r] >= 2^16 (0 if none).
+inline direct_kernel_t select_direct_kernel(const Dev& d, int r_hi) {
     const bool l4096 = d.L == 4096;
     if (d.q <= 8) {
         switch (direct_nearq(d.L, r_hi)) {
-            case 1: kern = l4096 ? sweep_direct_kernel<1, true, false> : sweep_direct_kernel<1, false, false>; break;
-            case 2: kern = sweep_direct_kernel<2, false, false>; break;
-            case 4: kern = sweep_direct_kernel<4, false, false>; break;
-            default: kern = l4096 ? sweep_direct_kernel<0, true, false> : sweep_direct_kernel<0, false, false>; break;
-        }
-    } else {
-        switch (direct_nearq(d.L, r_hi)) {
-            case 1: kern = sweep_direct_kernel<1, false, true>; break;
-            case 2: kern = sweep_direct_kernel<2, false, true>; break;
-            case 4: kern = sweep_direct_kernel<4, false, true>; break;
-            default: kern = sweep_direct_kernel<0, false, true>; break;
+            case 1: return l4096 ? sweep_direct_kernel<1, true, false> : sweep_direct_kernel<1, false, false>;
+            case 2: return sweep_direct_kernel<2, false, false>;
+            case 4: return sweep_direct_kernel<4, false, false>;
+            default: return l4096 ? sweep_direct_kernel<0, true, false> : sweep_direct_kernel<0, false, false>;
         }
     }
+    switch (direct_nearq(d.L, r_hi)) {
+        case 1: return sweep_direct_kernel<1, false, true>;
+        case 2: return sweep_direct_kernel<2, false, true>;
+        case 4: return sweep_direct_kernel<4, false, true>;
+        default: return sweep_direct_kernel<0, false, true>;
+    }
+}
+
+// Number of CTAs of the sweep kernel that can be resident on the device at once (0 on error): a persistent launch
+// (swap_mode 2) needs all n_ens * n_rep of them.
+inline int direct_max_coresident(const Dev& d, int r_hi, int device) {
+    direct_kernel_t kern = select_direct_kernel(d, r_hi);
+    const size_t smem = direct_smem_bytes(d.L, d.q);
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
+    int per_sm = 0, n_sm = 0, coop = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, direct_threads(d.L), smem) != cudaSuccess) return 0;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return 0;
+    if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device) != cudaSuccess || !coop) return 0;
+    return per_sm * n_sm;
+}
+
+// Returns a cudaError_t as int.  swap_mode 0/1: one launch of n_sweeps sweeps, optionally closed by a swap event,
+// with programmatic dependent launch (successive launches of a stream overlap prologue and epilogue).
+// swap_mode 2: cooperative (all CTAs co-resident) persistent launch with the swap events inside the kernel.
+inline int launch_sweep_direct(const Dev& d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi,
+                               cudaStream_t stream) {
+    const size_t smem = direct_smem_bytes(d.L, d.q);
+    direct_kernel_t kern = select_direct_kernel(d, r_hi);
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return (int)err;
-    // programmatic dependent launch: successive sweep launches of a stream overlap their prologue/epilogue
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(d.n_ens * d.n_rep));
     cfg.blockDim = dim3((unsigned)direct_threads(d.L));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    if (swap_mode == 2) {
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+    } else {
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+    }
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    err = cudaLaunchKernelEx(&cfg, kern, d, sweep0, n_sweeps, do_swap, r_hi);
+    err = cudaLaunchKernelEx(&cfg, kern, d, sweep0, n_sweeps, swap_mode, swap_every, r_hi);
     if (err != cudaSuccess) return (int)err;
     return (int)cudaGetLastError();
 }
