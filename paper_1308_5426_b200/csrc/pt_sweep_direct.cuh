@@ -201,8 +201,8 @@ __device__ __forceinline__ int direct_swap_in_kernel(const Dev& d, const Persist
     long long* Epub = d.Epub + ((size_t)(event & 1) * d.n_ens + e) * n_rep;
     if (threadIdx.x == 0) {
         __stcg(Epub + st, E_mine);
-        __threadfence();
-        atomicAdd(d.gen + e, 1u);
+        // release: the energy is visible to whoever observes the arrival (cheaper than a full __threadfence)
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(d.gen + e) : "memory");
         const unsigned target = (unsigned)n_rep * (unsigned)(event + 1);
         unsigned g = 0u, spins = 0u;
         while (true) {
@@ -403,9 +403,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 }
             }
         }
-        PT_T0(t_w);
         PT_AFTER_PREVIOUS_GRID();
-        PT_ACC(6, t_w);
         long long E = d.E[x];
         ObsAcc oa;
         cta_sync();
@@ -514,6 +512,8 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             PT_ACC(2, t_loop);
             PT_T0(t_end);
             cta_sync();  // the chain warp has decided the last block and published its sums
+            PT_ACC(6, t_end);
+            PT_T0(t_nm);
             // a8: sample after the sweep, before the swap event (A15)
             const int nmax = direct_nmax(m.sp, W, q, s_cnt);
             if (tid == 0) {
@@ -523,6 +523,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 oa.sample(E, nmax);
             }
             cta_sync();
+            PT_ACC(7, t_nm);
             if (swap_mode == 2 && (sweep0 + s + 1) % swap_every == 0) {
                 const int t_new = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, E, event++);
                 if (t_new != t) {   // the accumulators belong to the slot: hand them over when the slot changes
