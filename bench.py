@@ -32,8 +32,9 @@ UNIT = "attempts/s"
 # 64 lanes/clk/SM on the FMA-heavy pipe (profiles/r1_a_direct_v1a.md), so peak = 148 SMs x 64 x 2 MAC x f_SM.
 IDP_LANES_PER_CLK_PER_SM = 64
 MACS_PER_IDP_LANE = 2
-# dram__bytes_read.sum + dram__bytes_write.sum of one sweep_direct_kernel launch (ncu --set full, profiles/r1_c_direct_v5.md)
-DRAM_BYTES_PER_LAUNCH = 399.0e3
+# dram__bytes_read.sum + dram__bytes_write.sum per sweep of a persistent sweep_direct_kernel launch
+# (ncu --set full on a 40-sweep launch: 683 KB, profiles/r1_d_direct_v6.md)
+DRAM_BYTES_PER_SWEEP = 17.1e3
 N_SM = 148
 
 
@@ -232,17 +233,18 @@ def run_ours(args):
         macs_per_launch = K * w.n_rep * w.L * w.L / max(1, launches)
         launch_s = ms * 1e-3 / max(1, launches)              # CUDA events on the launching stream
         achieved = macs_per_launch / launch_s / 1e12
+        dram_per_launch = DRAM_BYTES_PER_SWEEP * K / max(1, launches)
         peak = N_SM * IDP_LANES_PER_CLK_PER_SM * MACS_PER_IDP_LANE * f_hz / 1e12
         roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tmac/s", "frac": achieved / peak,
-                    "traffic": DRAM_BYTES_PER_LAUNCH if variant == "direct" else None,
+                    "traffic": dram_per_launch if variant == "direct" else None,
                     "kernel": "sweep_%s_kernel" % variant,
                     "note": "algorithmic work = sweeps*n_rep*L^2 = %.3e integer multiply-accumulates per launch (one per "
                             "pair term; %d sweeps per launch); peak = 148 SMs x 64 IDP.2A lanes/clk/SM (measured issue rate) x 2 MAC x "
                             "sampled SM clock %.0f MHz -- a derived ALU peak, not MEASURED_PEAKS.json (its HBM and "
                             "tensor figures do not bound this path: %.0f KB of DRAM traffic per launch = %.2f GB/s "
                             "of the measured %.0f GB/s); 128 of 148 SMs carry a replica"
-                            % (macs_per_launch, K // max(1, launches), f_hz / 1e6, DRAM_BYTES_PER_LAUNCH / 1e3,
-                               DRAM_BYTES_PER_LAUNCH / launch_s / 1e9, measured_hbm_gbs())}
+                            % (macs_per_launch, K // max(1, launches), f_hz / 1e6, dram_per_launch / 1e3,
+                               dram_per_launch / launch_s / 1e9, measured_hbm_gbs())}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "int32", "data": "synthetic", "config": workload_config(w, variant, world),
