@@ -600,33 +600,31 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 }
                 const int4 cp0 = make_int4(cp[0], cp[1], cp[2], cp[3]), cp1 = make_int4(cp[4], cp[5], cp[6], cp[7]);
                 const int4 co0 = make_int4(co[0], co[1], co[2], co[3]), co1 = make_int4(co[4], co[5], co[6], co[7]);
+                // changes accepted in block k-1, which the bulk sum saw as it was before: this warp's rows, known
+                // before the wait; they ride along with the first round below (one exchange less per block)
+                int pc = 0;
+                if (mp) {
+                    const unsigned mv = (mp >> (8 * cw)) ^ lz;
+                    pc = masked_add4(masked_add4(0, mv, 0, cp0), mv, 4, cp1);
+                }
                 mbar_wait(&s_full[k & 1], (k >> 1) & 1);
                 PT_T0(t_c);
                 const uint32_t S = m.part[(k & 1) * 32 + lane];
                 // slack y = theta - dE: the site accepts iff y >= 0 (theta <= 2^30 and |dE| < 2^30: no overflow)
                 int y = th - (int)(S - rowsum);
-                if (mp) {   // changes accepted in block k-1, which the bulk sum saw as it was before
-                    const unsigned mv = (mp >> (8 * cw)) ^ lz;
-                    const int part = masked_add4(masked_add4(0, mv, 0, cp0), mv, 4, cp1);
-                    s_xch[xb][lane][cw] = part;
-                    asm volatile("bar.sync 1, 128;" ::: "memory");
-                    const int4 pv = *reinterpret_cast<const int4*>(&s_xch[xb][lane][0]);
-                    xb ^= 1;
-                    y -= (pv.x + pv.y) + (pv.z + pv.w);
-                }
                 PT_ACC(1, t_c);
                 PT_T0(t_s);
                 // The accept mask a of the block is the unique solution of the triangular system
                 //   a_l = [ y_l - sum_{f<l} a_f cm[32+f][l] >= 0 ]      (cm[32+f][l] = 0 for f >= l),
                 // which the site-by-site order solves by forward substitution.  Here: fixed-point iteration
                 // a <- F(a) from the guess "no correction"; after t rounds the first t bits are exact, so it ends
-                // after at most 32 rounds with exactly the sequential result, and in practice after two or three.
-                unsigned mask = __ballot_sync(0xffffffffu, y >= 0);
+                // after at most 33 rounds with exactly the sequential result, and in practice after two or three.
+                unsigned mask = __ballot_sync(0xffffffffu, y >= 0);   // first guess: no correction at all
                 int yy = y;
-                if (mask) {   // nothing accepted at first sight: nothing to correct, the guess is the solution
-                    for (int it = 0; it < 32; ++it) {
+                if (mask | mp) {   // nothing accepted here or in block k-1: nothing to correct
+                    for (int it = 0; it < 33; ++it) {
                         const unsigned mv = (mask >> (8 * cw)) ^ lz;
-                        const int part = masked_add4(masked_add4(0, mv, 0, co0), mv, 4, co1);
+                        const int part = masked_add4(masked_add4(pc, mv, 0, co0), mv, 4, co1);
                         s_xch[xb][lane][cw] = part;
                         asm volatile("bar.sync 1, 128;" ::: "memory");
                         const int4 pv = *reinterpret_cast<const int4*>(&s_xch[xb][lane][0]);
