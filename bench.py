@@ -217,14 +217,14 @@ def run_ours(args):
     g.sweeps(K, w.swap_every)
     spins = g.get_spins()                    # D2H: n_rep*L bytes
     E = g.energy()                           # D2H: n_rep*8 bytes
-    ob = g.observables()                     # D2H: n_rep*88 bytes
+    ob = g.observables()                     # D2H: n_rep*144 bytes
     barrier()
     e2e_s = time.perf_counter() - t0
     if world > 1:
         e2e_s = shard.max_over_ranks(e2e_s, dist, device="cuda")
     assert spins.shape == start.shape and E.size == w.n_rep and ob["n_samples"].min() > 0
     e2e = {"value": world * attempts_per_gpu / e2e_s, "unit": UNIT,
-           "h2d_bytes_per_step": start.nbytes / K, "d2h_bytes_per_step": (spins.nbytes + E.nbytes + w.n_rep * 88) / K,
+           "h2d_bytes_per_step": start.nbytes / K, "d2h_bytes_per_step": (spins.nbytes + E.nbytes + w.n_rep * 144) / K,
            "what": "pt_set_spins(host) + pt_sweeps(K) + pt_get_spins + pt_energy + pt_observables (host buffers), wall clock"}
 
     if rank == 0:

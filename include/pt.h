@@ -82,6 +82,13 @@ typedef struct {
     int64_t swap_attempts; /* Eq. 9, pair (t,t+1) recorded at slot t */
     int64_t swap_accepts;
     int64_t near_ties;     /* -1: not counted by this library (the CPU oracle counts them) */
+    /* Higher moments for the cumulants U_E = <E^4>/<E^2>^2 (Eq. 11) and
+     * V_M = 1 - <M^4>/(3<M^2>^2) (Eq. 12); M^4 is a polynomial of degree 4 in Nmax (Eq. 10).
+     * Valid while Nmax^3 sums fit int64 (L <= 2^14 for any realistic number of samples). */
+    uint64_t sum_E4[4];    /* sum of E^4 as a 256-bit unsigned integer, little-endian 64-bit limbs */
+    int64_t sum_Nmax3;
+    uint64_t sum_Nmax4_lo; /* sum of Nmax^4 as a 128-bit integer: low 64 bits ... */
+    int64_t sum_Nmax4_hi;  /* ... high 64 bits */
 } pt_obs;
 
 /* Create a context on the current CUDA device: evaluates J* (Eqs. 5-7) on the

@@ -119,6 +119,10 @@ struct Obs {              // same field order as include/pt.h's pt_obs (declared
     int64_t flip_attempts, flip_accepts;
     int64_t swap_attempts, swap_accepts;
     int64_t near_ties;
+    // higher moments for the cumulants of Eqs. 11-12
+    uint64_t sum_E4[4];                          // sum of E^4 as a 256-bit integer, little-endian 64-bit limbs
+    int64_t sum_Nmax3;
+    uint64_t sum_Nmax4_lo; int64_t sum_Nmax4_hi; // sum of Nmax^4 as a 128-bit integer
 };
 
 struct Replica {
@@ -224,6 +228,32 @@ void measure(Ctx& C, int e, int t) {
     O.sum_E2_hi = (int64_t)(uint64_t)(acc >> 64);
     O.sum_Nmax += nmax;
     O.sum_Nmax2 += nmax * nmax;
+    // Eq. 11 needs <E^4>: E^4 = (E^2)^2 with E^2 = hi 2^64 + lo, added limb by limb (schoolbook, base 2^64)
+    {
+        const unsigned __int128 e2 = (unsigned __int128)((__int128)R.E * (__int128)R.E);
+        const uint64_t lo = (uint64_t)e2, hi = (uint64_t)(e2 >> 64);
+        const unsigned __int128 ll = (unsigned __int128)lo * lo, lh = (unsigned __int128)lo * hi,
+                                hh = (unsigned __int128)hi * hi;
+        uint64_t add[4] = {(uint64_t)ll, 0, 0, 0};
+        unsigned __int128 c = (ll >> 64) + (uint64_t)lh + (uint64_t)lh;     // limb 1: carry of ll + 2 low(lh)
+        add[1] = (uint64_t)c;
+        c = (c >> 64) + (lh >> 64) + (lh >> 64) + (uint64_t)hh;             // limb 2
+        add[2] = (uint64_t)c;
+        c = (c >> 64) + (hh >> 64);                                         // limb 3
+        add[3] = (uint64_t)c;
+        unsigned __int128 carry = 0;
+        for (int k = 0; k < 4; ++k) {
+            carry += (unsigned __int128)O.sum_E4[k] + add[k];
+            O.sum_E4[k] = (uint64_t)carry;
+            carry >>= 64;
+        }
+    }
+    // Eq. 12 needs <M^4>, a polynomial in Nmax of degree 4 (Eq. 10)
+    O.sum_Nmax3 += nmax * nmax * nmax;
+    unsigned __int128 n4 = ((unsigned __int128)(uint64_t)O.sum_Nmax4_hi << 64) | O.sum_Nmax4_lo;
+    n4 += (unsigned __int128)((uint64_t)(nmax * nmax)) * (uint64_t)(nmax * nmax);
+    O.sum_Nmax4_lo = (uint64_t)n4;
+    O.sum_Nmax4_hi = (int64_t)(uint64_t)(n4 >> 64);
 }
 
 // Eq. 9 in two stages, even pairs then odd pairs (A11).

@@ -33,7 +33,9 @@ class Obs(ctypes.Structure):
                 ("sum_Nmax", ctypes.c_int64), ("sum_Nmax2", ctypes.c_int64),
                 ("flip_attempts", ctypes.c_int64), ("flip_accepts", ctypes.c_int64),
                 ("swap_attempts", ctypes.c_int64), ("swap_accepts", ctypes.c_int64),
-                ("near_ties", ctypes.c_int64)]
+                ("near_ties", ctypes.c_int64),
+                ("sum_E4", ctypes.c_uint64 * 4), ("sum_Nmax3", ctypes.c_int64),
+                ("sum_Nmax4_lo", ctypes.c_uint64), ("sum_Nmax4_hi", ctypes.c_int64)]
 
 
 OBS_FIELDS = [f[0] for f in Obs._fields_]
@@ -135,7 +137,10 @@ class Oracle:
         lib().orc_observables(self._h, ctypes.byref(arr))
         out = {}
         for name in OBS_FIELDS:
-            dt = np.uint64 if name == "sum_E2_lo" else np.int64
+            if name == "sum_E4":   # [n_ens, n_rep, 4] little-endian 64-bit limbs
+                out[name] = np.array([list(o.sum_E4) for o in arr], dtype=np.uint64).reshape(self.n_ens, self.n_rep, 4)
+                continue
+            dt = np.uint64 if name in ("sum_E2_lo", "sum_Nmax4_lo") else np.int64
             out[name] = np.array([getattr(o, name) for o in arr], dtype=dt).reshape(self.n_ens, self.n_rep)
         return out
 

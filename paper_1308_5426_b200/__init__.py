@@ -3,4 +3,4 @@
 library `libpt.so` (include/pt.h); `paper_1308_5426_b200.inputs` holds the seeded
 workload recipes.  Nothing here falls back to a CPU path: importing `.pt` without a
 built `libpt.so` raises."""
-__all__ = ["inputs", "pt", "build", "shard"]
+__all__ = ["inputs", "pt", "pt_math", "build", "shard"]

@@ -68,4 +68,40 @@ __device__ __forceinline__ void add_square_128(unsigned long long& lo, long long
     lo = nlo;
 }
 
+// Adds x^4 to the 256-bit accumulator a[0..3] (little-endian limbs): x^2 = hi 2^64 + lo, x^4 = lo^2 + 2 lo hi 2^64
+// + hi^2 2^128, schoolbook in base 2^64.
+__device__ __forceinline__ void add_fourth_256(unsigned long long a[4], long long x) {
+    const unsigned long long ax = (unsigned long long)(x < 0 ? -x : x);
+    const unsigned long long lo = ax * ax, hi = __umul64hi(ax, ax);
+    const unsigned long long ll_lo = lo * lo, ll_hi = __umul64hi(lo, lo);
+    const unsigned long long lh_lo = lo * hi, lh_hi = __umul64hi(lo, hi);
+    const unsigned long long hh_lo = hi * hi, hh_hi = __umul64hi(hi, hi);
+    unsigned long long add[4];
+    add[0] = ll_lo;
+    // limb 1 = ll_hi + 2 lh_lo (three 64-bit terms: carry in 0..2)
+    unsigned long long s1 = ll_hi + lh_lo;
+    unsigned long long c1 = s1 < ll_hi ? 1ull : 0ull;
+    unsigned long long s1b = s1 + lh_lo;
+    c1 += s1b < s1 ? 1ull : 0ull;
+    add[1] = s1b;
+    // limb 2 = c1 + 2 lh_hi + hh_lo
+    unsigned long long s2 = c1 + lh_hi;
+    unsigned long long c2 = s2 < lh_hi ? 1ull : 0ull;
+    unsigned long long s2b = s2 + lh_hi;
+    c2 += s2b < s2 ? 1ull : 0ull;
+    unsigned long long s2c = s2b + hh_lo;
+    c2 += s2c < s2b ? 1ull : 0ull;
+    add[2] = s2c;
+    add[3] = c2 + hh_hi;
+    unsigned long long carry = 0ull;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const unsigned long long t = a[k] + carry;
+        const unsigned long long c0 = t < carry ? 1ull : 0ull;
+        const unsigned long long u = t + add[k];
+        carry = c0 + (u < t ? 1ull : 0ull);
+        a[k] = u;
+    }
+}
+
 }  // namespace ptdev

@@ -271,24 +271,50 @@ __device__ inline int count_nmax(const uint32_t* sp, int W, int q, int* s_cnt) {
 
 // Per-launch accumulators kept by thread 0 of a sweep CTA.
 struct ObsAcc {
-    long long n = 0, sE = 0, sN = 0, sN2 = 0, acc = 0, att = 0;
+    long long n = 0, sE = 0, sN = 0, sN2 = 0, sN3 = 0, acc = 0, att = 0;
     unsigned long long e2lo = 0;
     long long e2hi = 0;
+    unsigned long long e4[4] = {0, 0, 0, 0};
+    unsigned long long n4lo = 0;
+    long long n4hi = 0;
     __device__ void sample(long long E, int nmax) {
-        n += 1; sE += E; sN += nmax; sN2 += (long long)nmax * nmax;
+        const long long nm = nmax, nm2 = nm * nm;
+        n += 1; sE += E; sN += nm; sN2 += nm2; sN3 += nm2 * nm;
         add_square_128(e2lo, e2hi, E);
+        add_fourth_256(e4, E);
+        add_square_128(n4lo, n4hi, nm2);
     }
-    // Single writer at a time per slot, but successive writers may be different CTAs (persistent launches):
-    // read-modify-write in L2 with atomics.
+    // Adds the accumulators to the slot's pt_obs.  One writer at a time per slot, but successive writers may be
+    // different CTAs (persistent launches, ordered by the swap barrier): all loads and stores go to L2; the loads are
+    // independent, so the whole flush costs one L2 round trip.  The swap counters (words 8, 9) are not touched here.
     __device__ void flush(pt_obs* o) const {
         typedef unsigned long long u64;
-        atomicAdd((u64*)&o->n_samples, (u64)n); atomicAdd((u64*)&o->sum_E, (u64)sE);
-        atomicAdd((u64*)&o->sum_Nmax, (u64)sN); atomicAdd((u64*)&o->sum_Nmax2, (u64)sN2);
-        atomicAdd((u64*)&o->flip_attempts, (u64)att); atomicAdd((u64*)&o->flip_accepts, (u64)acc);
-        const u64 old = atomicAdd((u64*)&o->sum_E2_lo, e2lo);
-        atomicAdd((u64*)&o->sum_E2_hi, (u64)e2hi + ((old + e2lo < old) ? 1ull : 0ull));
+        // Nothing gathered (the configuration moved into this slot at the last swap event of the launch): the slot's
+        // previous holder may be flushing right now, and it is the only one with something to add.
+        if (n == 0 && att == 0) return;
+        u64* p = (u64*)o;
+        u64 v[18];
+#pragma unroll
+        for (int k = 0; k < 18; ++k) v[k] = (k >= 8 && k <= 10) ? 0ull : __ldcg(p + k);
+        v[0] += (u64)n; v[1] += (u64)sE; v[4] += (u64)sN; v[5] += (u64)sN2; v[6] += (u64)att; v[7] += (u64)acc;
+        { const u64 lo = v[2] + e2lo; v[3] += (u64)e2hi + (lo < v[2] ? 1ull : 0ull); v[2] = lo; }
+        u64 carry = 0ull;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const u64 t = v[11 + k] + carry;
+            const u64 c0 = t < carry ? 1ull : 0ull;
+            const u64 u = t + e4[k];
+            carry = c0 + (u < t ? 1ull : 0ull);
+            v[11 + k] = u;
+        }
+        v[15] += (u64)sN3;
+        { const u64 lo = v[16] + n4lo; v[17] += (u64)n4hi + (lo < v[16] ? 1ull : 0ull); v[16] = lo; }
+#pragma unroll
+        for (int k = 0; k < 18; ++k)
+            if (k < 8 || k > 10) __stcg(p + k, v[k]);
     }
 };
+static_assert(sizeof(pt_obs) == 18 * 8, "ObsAcc::flush addresses pt_obs as 18 64-bit words");
 
 // ---------------------------------------------------------------------------
 // I/O kernels (slot order outside, storage order inside).

@@ -177,8 +177,7 @@ __device__ __forceinline__ int direct_nmax(const uint32_t* sp, int W, int q, int
     }
     cta_sync();
     int nmax = 0;
-    if (threadIdx.x == 0)
-        for (int k = 0; k < q; ++k) nmax = max(nmax, s_cnt[k]);
+    for (int k = 0; k < q; ++k) nmax = max(nmax, s_cnt[k]);   // every thread: whoever needs it has it
     return nmax;
 }
 
@@ -196,11 +195,11 @@ struct PersistSmem {
     int* slot;          // result
 };
 __device__ __forceinline__ int direct_swap_in_kernel(const Dev& d, const PersistSmem& ps, int e, uint32_t sweep, int st,
-                                                     long long E_mine, int event) {
+                                                     const long long* s_E, int event) {
     const int n_rep = d.n_rep;
     long long* Epub = d.Epub + ((size_t)(event & 1) * d.n_ens + e) * n_rep;
     if (threadIdx.x == 0) {
-        __stcg(Epub + st, E_mine);
+        __stcg(Epub + st, *s_E);
         // release: the energy is visible to whoever observes the arrival (cheaper than a full __threadfence)
         asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(d.gen + e) : "memory");
         const unsigned target = (unsigned)n_rep * (unsigned)(event + 1);
@@ -305,9 +304,9 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     m.part = (uint32_t*)(m.selb + L);
     m.Jz = (int32_t*)(m.part + 64);
     __shared__ int s_cnt[16];
-    __shared__ long long s_dE;
-    __shared__ int s_nacc;
+    __shared__ long long s_E;   // running energy of this configuration (owner: lane 0 of chain warp 0)
     __shared__ int s_slot;
+    __shared__ ObsAcc s_oa;
     __shared__ int s_perm[DIRECT_MAX_PERSIST_REP];
     __shared__ long long s_Eall[DIRECT_MAX_PERSIST_REP];
     __shared__ double s_scale[DIRECT_MAX_PERSIST_REP];
@@ -404,8 +403,6 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             }
         }
         PT_AFTER_PREVIOUS_GRID();
-        long long E = d.E[x];
-        ObsAcc oa;
         cta_sync();
 
         for (int s = 0; s < n_sweeps; ++s) {
@@ -514,30 +511,16 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             cta_sync();  // the chain warp has decided the last block and published its sums
             PT_ACC(6, t_end);
             PT_T0(t_nm);
-            // a8: sample after the sweep, before the swap event (A15)
-            const int nmax = direct_nmax(m.sp, W, q, s_cnt);
-            if (tid == 0) {
-                E += s_dE;
-                oa.acc += s_nacc;
-                oa.att += L;
-                oa.sample(E, nmax);
-            }
+            // a8 (the chain warps' owner thread samples the observables; every thread helps counting colours)
+            direct_nmax(m.sp, W, q, s_cnt);
             cta_sync();
             PT_ACC(7, t_nm);
             if (swap_mode == 2 && (sweep0 + s + 1) % swap_every == 0) {
-                const int t_new = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, E, event++);
-                if (t_new != t) {   // the accumulators belong to the slot: hand them over when the slot changes
-                    if (tid == 0) {
-                        oa.flush(d.obs + (size_t)e * d.n_rep + t);
-                        oa = ObsAcc();
-                    }
-                    t = t_new;
-                    scale = s_scale[t];
-                }
+                t = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, &s_E, event++);
+                scale = s_scale[t];
             }
             PT_ACC(3, t_end);
         }
-        if (tid == 0) { d.E[x] = E; oa.flush(d.obs + (size_t)e * d.n_rep + t); }
 #ifdef PT_TIMING
         if (lane == 0 && d.dbg) {
             tacc[4] = clock64() - t_kernel;
@@ -563,6 +546,11 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             Jo[j] = dn > 0 ? __ldg(d.Jq + dn) : 0;
         }
         PT_AFTER_PREVIOUS_GRID();
+        // Owner of the configuration's running energy and of the slot's accumulators (a8): lane 0 of chain warp 0.
+        // They live in shared memory, so nothing of this costs registers in the bulk path.
+        const bool owner = cw == 0 && lane == 0;
+        ObsAcc& oa = s_oa;
+        if (owner) { oa = ObsAcc(); s_E = d.E[x]; }
         cta_sync();
         // A per-lane zero the compiler cannot see through: xor-ed into the accept masks it keeps the bit tests
         // on the ALU pipe (LOP3 -> predicate, SEL) instead of shift pairs on the FMA or uniform pipes.
@@ -657,14 +645,43 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 PT_ACC(0, t_c);
             }
             for (int o = 16; o > 0; o >>= 1) dE_acc += __shfl_xor_sync(0xffffffffu, dE_acc, o);
-            if (cw == 0 && lane == 0) { s_dE = dE_acc; s_nacc = n_acc; }
+            if (owner) s_E += dE_acc;
             cta_sync();
-            direct_nmax(m.sp, W, q, s_cnt);
+            // a8: sample after the sweep, before the swap event (A15)
+            const int nmax = direct_nmax(m.sp, W, q, s_cnt);
+            if (owner) {
+                oa.acc += n_acc;
+                oa.att += L;
+                oa.sample(s_E, nmax);
+            }
             cta_sync();
             if (swap_mode == 2 && (sweep0 + s + 1) % swap_every == 0) {
-                t = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, 0, event++);
-                scale = s_scale[t];
+                const int t_new = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, &s_E, event++);
+                if (t_new != t) {   // the accumulators belong to the slot: hand them over when the slot changes
+                    if (owner) {
+                        oa.flush(d.obs + (size_t)e * d.n_rep + t);
+                        oa = ObsAcc();
+                    }
+                    t = t_new;
+                    scale = s_scale[t];
+                }
             }
+        }
+        if (owner) {
+            d.E[x] = s_E;
+            if (swap_mode == 2) {
+                // The observables of a slot are read-modify-written by one CTA at a time; a last counter barrier
+                // orders this final flush behind the flush of whoever left the slot at an earlier event.
+                asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(d.gen + e) : "memory");
+                const unsigned target = (unsigned)d.n_rep * (unsigned)(event + 1);
+                unsigned g = 0u, spins = 0u;
+                while (true) {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(g) : "l"(d.gen + e) : "memory");
+                    if (g >= target) break;
+                    if (++spins > (1u << 22)) __trap();
+                }
+            }
+            oa.flush(d.obs + (size_t)e * d.n_rep + t);
         }
 #ifdef PT_TIMING
         if (lane == 0 && d.dbg && warp < 32) {

@@ -36,7 +36,9 @@ class Obs(ctypes.Structure):  # pt_obs
                 ("sum_Nmax", ctypes.c_int64), ("sum_Nmax2", ctypes.c_int64),
                 ("flip_attempts", ctypes.c_int64), ("flip_accepts", ctypes.c_int64),
                 ("swap_attempts", ctypes.c_int64), ("swap_accepts", ctypes.c_int64),
-                ("near_ties", ctypes.c_int64)]
+                ("near_ties", ctypes.c_int64),
+                ("sum_E4", ctypes.c_uint64 * 4), ("sum_Nmax3", ctypes.c_int64),
+                ("sum_Nmax4_lo", ctypes.c_uint64), ("sum_Nmax4_hi", ctypes.c_int64)]
 
 
 OBS_FIELDS = [f[0] for f in Obs._fields_]
@@ -138,7 +140,10 @@ class PT:
         _check(_lib.pt_observables(self._h, ctypes.byref(arr)))
         out = {}
         for name in OBS_FIELDS:
-            dt = np.uint64 if name == "sum_E2_lo" else np.int64
+            if name == "sum_E4":   # [n_ens, n_rep, 4] little-endian 64-bit limbs of a 256-bit integer
+                out[name] = np.array([list(o.sum_E4) for o in arr], dtype=np.uint64).reshape(self.n_ens, self.n_rep, 4)
+                continue
+            dt = np.uint64 if name in ("sum_E2_lo", "sum_Nmax4_lo") else np.int64
             out[name] = np.array([getattr(o, name) for o in arr], dtype=dt).reshape(self.n_ens, self.n_rep)
         return out
 
@@ -184,12 +189,4 @@ class PT:
         return s
 
 
-def derived(obs, L, q):
-    """<E>/L, <M>, <M^2> from the integer accumulators (one fixed fp64 formula; Eq. 10)."""
-    n = obs["n_samples"].astype(np.float64)
-    e = obs["sum_E"].astype(np.float64) / (n * L * 16777216.0)
-    m1 = obs["sum_Nmax"].astype(np.float64) / (n * L)
-    m2 = obs["sum_Nmax2"].astype(np.float64) / (n * float(L) * float(L))
-    M = (q * m1 - 1.0) / (q - 1.0)
-    M2 = (q * q * m2 - 2.0 * q * m1 + 1.0) / ((q - 1.0) ** 2)
-    return {"E_per_spin": e, "M": M, "M2": M2}
+from .pt_math import cumulants, derived, obs_diff  # noqa: E402,F401  (pure-Python reporting helpers)

@@ -33,7 +33,7 @@ def test_header_symbols_are_exported(lib_path):
 def test_binding_lists_every_symbol(lib_path):
     from paper_1308_5426_b200 import pt
     assert sorted(pt.SYMBOLS) == declared_symbols()
-    assert ctypes.sizeof(pt.Obs) == 88
+    assert ctypes.sizeof(pt.Obs) == 144
 
 
 def test_no_cpu_fallback(lib_path):

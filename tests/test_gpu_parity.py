@@ -16,7 +16,8 @@ pytestmark = pytest.mark.gpu
 THREADS = max(1, min(32, os.cpu_count() or 1))
 FULL = os.environ.get("PT_FULL", "0") == "1"
 CMP_FIELDS = ["n_samples", "sum_E", "sum_E2_lo", "sum_E2_hi", "sum_Nmax", "sum_Nmax2",
-              "flip_attempts", "flip_accepts", "swap_attempts", "swap_accepts"]
+              "flip_attempts", "flip_accepts", "swap_attempts", "swap_accepts",
+              "sum_E4", "sum_Nmax3", "sum_Nmax4_lo", "sum_Nmax4_hi"]
 
 
 @pytest.fixture(scope="module")
