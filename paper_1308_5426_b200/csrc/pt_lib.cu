@@ -67,7 +67,7 @@ struct pt_ctx {
     unsigned* d_gen = nullptr;
     long long* d_Epub = nullptr;
     int coresident = -1;   // direct variant: CTAs that fit on the device at once (-1: not asked yet)
-    bool allow_persistent = true;
+    int persistent_policy = 1;   // 0 never, 1 when the context fills the device and the call is long enough, 2 whenever possible
 
     int R() const { return n_ens * n_rep; }
     ptk::Dev dev() const {
@@ -162,9 +162,15 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
 
 // Direct variant: can all replicas be resident at once (persistent launches with in-kernel swap events)?
 bool persistent_ok(pt_ctx* c) {
-    if (c->variant != PT_VARIANT_DIRECT || !c->allow_persistent) return false;
+    if (c->variant != PT_VARIANT_DIRECT || c->persistent_policy == 0) return false;
     if (c->coresident < 0) c->coresident = ptk::direct_max_coresident(c->dev(), c->r_hi, c->device);
-    return c->R() <= c->coresident && c->n_rep <= ptk::DIRECT_MAX_PERSIST_REP;
+    // A small context (e.g. one of the 40 handles of configs[4]) shares the GPU with others: launches per swap
+    // interval interleave their CTAs better than resident kernels that wait at their own barriers (measured:
+    // 4.2e9 against 3.6e9 attempts/s on configs[4]).  Persistent launches are for contexts that fill the device.
+    int n_sm = 0;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) return false;
+    return c->R() <= c->coresident && (2 * c->R() >= n_sm || c->persistent_policy == 2) &&
+           c->n_rep <= ptk::DIRECT_MAX_PERSIST_REP;
 }
 
 }  // namespace
@@ -240,8 +246,10 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
     PT_CUDA_C(cudaMemset(c->d_gen, 0, (size_t)n_ens * sizeof(unsigned)));
     PT_CUDA_C(cudaMalloc(&c->d_Epub, (size_t)2 * R * sizeof(long long)));
     {
-        const char* env = getenv("PT_PERSISTENT");   // PT_PERSISTENT=0: one launch per swap interval (A/B, debugging)
-        c->allow_persistent = !(env && env[0] == '0');
+        // PT_PERSISTENT=0: one launch per swap interval; =2: persistent launches whenever all replicas can be
+        // co-resident (tests); default: only for contexts that fill the device (see persistent_ok)
+        const char* env = getenv("PT_PERSISTENT");
+        c->persistent_policy = (env && env[0] == '0') ? 0 : (env && env[0] == '2') ? 2 : 1;
     }
 #ifdef PT_TIMING
     PT_CUDA_C(cudaMalloc(&c->d_dbg, (size_t)R * 32 * 8 * sizeof(long long)));
@@ -308,7 +316,8 @@ int pt_sweeps_async(pt_ctx* c, int64_t n, int swap_every, int64_t* n_launches) {
     if (n < 0 || swap_every < 0) return fail(PT_EINVAL, "n and swap_every must be >= 0");
     int64_t launches = 0;
     constexpr int64_t kMaxChunk = 1 << 16;  // sweeps per launch
-    const bool persistent = swap_every > 0 && persistent_ok(c);
+    // a persistent launch pays a counter reset and a cooperative launch: worth it from a handful of sweeps per call
+    const bool persistent = swap_every > 0 && (n >= 8 || c->persistent_policy == 2) && persistent_ok(c);
     while (n > 0) {
         int64_t chunk = n < kMaxChunk ? n : kMaxChunk;
         int swap_mode = 0;

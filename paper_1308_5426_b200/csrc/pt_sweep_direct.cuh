@@ -321,16 +321,12 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int e = blockIdx.x / d.n_rep;
     int t = blockIdx.x % d.n_rep;   // slot (temperature) of this CTA's configuration; moves in swap_mode 2
-    // Programmatic dependent launch: this grid may start while the previous sweep launch is still draining, and
-    // everything up to PT_AFTER_PREVIOUS_GRID (coupling registers, tables) overlaps with it; what the previous
-    // launch writes (perm, spins, E, obs) is only read behind griddepcontrol.wait.
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    // state that the previous launch wrote (perm, spins, E) and, for persistent launches, the ensemble's tables
     size_t x = 0;
     int st = 0;
     uint32_t* g_sp = nullptr;
-#define PT_AFTER_PREVIOUS_GRID()                                             \
+#define PT_LOAD_STATE()                                             \
     do {                                                                     \
-        asm volatile("griddepcontrol.wait;" ::: "memory");                   \
         st = d.perm[blockIdx.x];                                             \
         x = (size_t)e * d.n_rep + st;                                        \
         g_sp = d.spins + x * W;                                              \
@@ -402,7 +398,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 }
             }
         }
-        PT_AFTER_PREVIOUS_GRID();
+        PT_LOAD_STATE();
         cta_sync();
 
         for (int s = 0; s < n_sweeps; ++s) {
@@ -545,7 +541,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             Jp[j] = __ldg(d.Jq + dp);               // 1 <= dp <= 63 < L
             Jo[j] = dn > 0 ? __ldg(d.Jq + dn) : 0;
         }
-        PT_AFTER_PREVIOUS_GRID();
+        PT_LOAD_STATE();
         // Owner of the configuration's running energy and of the slot's accumulators (a8): lane 0 of chain warp 0.
         // They live in shared memory, so nothing of this costs registers in the bulk path.
         const bool owner = cw == 0 && lane == 0;
@@ -839,9 +835,12 @@ inline int direct_max_coresident(const Dev& d, int r_hi, int device) {
     return per_sm * n_sm;
 }
 
-// Returns a cudaError_t as int.  swap_mode 0/1: one launch of n_sweeps sweeps, optionally closed by a swap event,
-// with programmatic dependent launch (successive launches of a stream overlap prologue and epilogue).
-// swap_mode 2: cooperative (all CTAs co-resident) persistent launch with the swap events inside the kernel.
+// Returns a cudaError_t as int.  swap_mode 0/1: one ordinary launch of n_sweeps sweeps, optionally closed by a swap
+// event.  swap_mode 2: cooperative (all CTAs co-resident) persistent launch with the swap events inside the kernel.
+// (Programmatic dependent launch was tried for swap_mode 1 and removed: streams with thousands of dependent
+// launches of this kernel queued back to back occasionally never finished on this driver, and for the small
+// contexts that still use swap_mode 1 it was slower than ordinary launches: 0.41-0.48 s against 0.39 s for 10000
+// sweeps of configs[2].)
 inline int launch_sweep_direct(const Dev& d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi,
                                cudaStream_t stream) {
     const size_t smem = direct_smem_bytes(d.L, d.q);
@@ -857,12 +856,9 @@ inline int launch_sweep_direct(const Dev& d, long long sweep0, int n_sweeps, int
     if (swap_mode == 2) {
         attr[0].id = cudaLaunchAttributeCooperative;
         attr[0].val.cooperative = 1;
-    } else {
-        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[0].val.programmaticStreamSerializationAllowed = 1;
     }
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
+    cfg.numAttrs = swap_mode == 2 ? 1 : 0;
     err = cudaLaunchKernelEx(&cfg, kern, d, sweep0, n_sweeps, swap_mode, swap_every, r_hi);
     if (err != cudaSuccess) return (int)err;
     return (int)cudaGetLastError();

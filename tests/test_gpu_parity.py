@@ -278,3 +278,22 @@ def test_direct_variant_with_more_than_8_colours(pt, oracle, L, q, sigma):
             o.sweeps(n, 1, field=True, threads=THREADS)
             assert_same_state(g, o, "L=%d q=%d %s" % (L, q, variant))
         g.close()
+
+
+@pytest.mark.parametrize("policy", ["0", "2"])
+def test_persistent_and_per_interval_launches_agree_with_the_oracle(pt, oracle, policy, monkeypatch):
+    """PT_PERSISTENT=2 forces persistent launches (swap events inside the kernel, slots moving between resident CTAs)
+    wherever all replicas can be co-resident, =0 forbids them: both must reproduce the oracle, for several ensembles,
+    an odd replica count, swap periods 1 and 3, short and split calls, and more than 8 colours."""
+    monkeypatch.setenv("PT_PERSISTENT", policy)
+    for (L, q, sigma, n_ens, n_rep, swap_every) in [(128, 4, 0.6, 3, 5, 1), (128, 4, 0.6, 3, 5, 3), (64, 3, 0.5, 1, 8, 1),
+                                                    (256, 12, 0.4, 2, 7, 2), (1024, 8, 0.3, 1, 16, 1)]:
+        b = inputs.geometric_betas(0.7, 2.4, n_rep)
+        g = pt.PT(L, q, sigma, n_ens, n_rep, b, 4242, variant="direct")
+        o = oracle.Oracle(L, q, sigma, n_ens, n_rep, b, 4242)
+        for n in (1, 2, 9, 40):
+            g.sweeps(n, swap_every)
+            o.sweeps(n, swap_every, field=True, threads=THREADS)
+            assert_same_state(g, o, "policy %s L=%d q=%d swap_every=%d after +%d" % (policy, L, q, swap_every, n))
+        assert int(o.observables()["swap_accepts"].sum()) > 0
+        g.close()
