@@ -63,7 +63,7 @@ constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 32 * DIRECT_CHAIN_WARPS;
 constexpr int DIRECT_NPAIR = 35;   // packed coupling pairs per thread and half
 constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: the 224 sites (56 quads) around a block
 constexpr int DIRECT_NEAR_QUADS = 56;
-constexpr int DIRECT_MAX_PERSIST_REP = 256;   // replicas per ensemble in a persistent launch (static shared arrays)
+constexpr int DIRECT_MAX_PERSIST_REP = 512;   // replicas per ensemble in a persistent launch (static shared arrays)
 
 __host__ __device__ inline bool direct_applies(int L, int q) {
     return (L % 64) == 0 && L >= 64 && L <= 64 * (DIRECT_MAX_BULK / 8) && q <= 16;
