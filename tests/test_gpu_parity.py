@@ -25,6 +25,8 @@ def pt():
     import torch
     if not torch.cuda.is_available():
         pytest.fail("gpu-marked test on a box without CUDA")
+    from paper_1308_5426_b200 import build
+    build.build()   # no-op when libpt.so is up to date; the binding raises if the library is missing
     from paper_1308_5426_b200 import pt as ptmod
     return ptmod
 
