@@ -166,10 +166,11 @@ bool persistent_ok(pt_ctx* c) {
     if (c->coresident < 0) c->coresident = ptk::direct_max_coresident(c->dev(), c->r_hi, c->device);
     // A small context (e.g. one of the 40 handles of configs[4]) shares the GPU with others: launches per swap
     // interval interleave their CTAs better than resident kernels that wait at their own barriers (measured:
-    // 4.2e9 against 3.6e9 attempts/s on configs[4]).  Persistent launches are for contexts that fill the device.
+    // 4.2e9 against 3.6e9 attempts/s on configs[4]).  Persistent launches are for contexts that take at least a
+    // third of the SMs (configs[2] alone: 32 us per sweep persistent, 39 us with ordinary launches).
     int n_sm = 0;
     if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess) return false;
-    return c->R() <= c->coresident && (2 * c->R() >= n_sm || c->persistent_policy == 2) &&
+    return c->R() <= c->coresident && (3 * c->R() >= n_sm || c->persistent_policy == 2) &&
            c->n_rep <= ptk::DIRECT_MAX_PERSIST_REP;
 }
 
