@@ -52,6 +52,16 @@
 // shared memory (named barrier 1) and a ballot.  Chain warp 0 writes the new
 // spins and arrives on done[k&1].  Integer arithmetic makes all of this
 // independent of the order of summation (parity tests: bit-identical).
+//
+// OBSERVABLES, SWAPS.  Lane 0 of chain warp 0 owns the configuration's running
+// energy and the slot's accumulators (shared memory); it samples them after
+// every sweep (A15).  swap_mode 1: the launch ends with one swap event, run by
+// the CTA that arrives last (nobody waits).  swap_mode 2 (persistent,
+// cooperative launch, all replicas co-resident): the launch runs many sweeps;
+// at a swap event every CTA publishes its energy, meets the others at a counter
+// barrier in global memory, and evaluates the whole event on its own copy of the
+// slot -> storage permutation (direct_swap_in_kernel); the configuration keeps
+// its CTA and shared memory, the temperature, RNG slot and accumulators move.
 #pragma once
 #include "pt_kernels.cuh"
 
