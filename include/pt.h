@@ -114,6 +114,30 @@ int pt_create(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
 int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
                  const double* betas, uint64_t seed, int ens_base);
 
+/* Slot-sharded context: ONE ensemble of n_rep replicas spread over several processes / GPUs.
+ * Every process creates the context with the same arguments except (rep_base, n_local): it sweeps the n_local
+ * configurations with storage index rep_base .. rep_base + n_local - 1 (at creation storage index = slot), and keeps
+ * a full copy of the slot -> storage permutation.  Configurations never leave their process; at a swap event
+ * (Eq. 9) only energies are exchanged: every process passes the energies of ALL configurations, in
+ * storage order (an all-gather of pt_energy_storage_dev), to pt_swap_external, which takes the same decisions
+ * everywhere from the slot-keyed random stream and moves the temperature labels.  pt_sweeps must be called with
+ * swap_every = 0.  The accumulators of a slot are gathered by whichever process holds its configuration: the
+ * ensemble's observables are the field-wise sums over the processes (swap counters: process with rep_base = 0).
+ * Needs the direct variant (PT_EINVAL otherwise), 0 <= rep_base, n_local >= 1, rep_base + n_local <= n_rep. */
+int pt_create_shard(pt_ctx** out, int L, int q, double sigma, int n_rep, const double* betas, uint64_t seed,
+                    int ens_base, int rep_base, int n_local);
+
+/* Slot-sharded contexts: running energies of the local configurations, E_out_dev[n_local] (DEVICE pointer),
+ * storage order. */
+int pt_energy_storage_dev(pt_ctx* ctx, int64_t* E_out_dev);
+
+/* Slot-sharded contexts: one swap event (even pairs, then odd pairs) after the current sweep, from the energies of
+ * all n_rep configurations in storage order, E_all_dev[n_rep] (DEVICE pointer). */
+int pt_swap_external(pt_ctx* ctx, const int64_t* E_all_dev);
+
+/* perm[n_ens*n_rep]: storage index (inside the ensemble) of the configuration at each slot. */
+int pt_get_perm(pt_ctx* ctx, int32_t* perm);
+
 void pt_destroy(pt_ctx* ctx); /* NULL is allowed */
 
 /* Advance every replica by n >= 0 sweeps.  With swap_every > 0 a swap event

@@ -13,6 +13,9 @@ using namespace ptdev;
 // Everything a kernel needs to know about a context (passed by value).
 struct Dev {
     int L, W, q, n_ens, n_rep, ens_base;
+    int rep_base, n_local;    // slot-sharded contexts (pt_create_shard): this process sweeps the configurations with
+                              // storage index rep_base .. rep_base + n_local - 1; otherwise 0, n_rep
+    int count_swaps;          // 0: this shard leaves the swap counters to the shard with rep_base = 0
     uint32_t key0, key1;
     uint32_t rowsum;          // sum_r Jq[r] (< 2^31)
     const int32_t* Jq;        // [L]
@@ -212,11 +215,11 @@ __device__ inline void swap_event(const Dev& d, int e, uint32_t sweep) {
             const double dd = __dmul_rn(d.beta[t] - d.beta[t + 1], ldexp((double)(Ea - Eb), -24));
             const Philox4 p = philox4x32_10((uint32_t)t, sweep, 0u, c3, d.key0, d.key1);
             const double u = uniform53(p.w1, p.w2);
-            atomicAdd((unsigned long long*)&obs[t].swap_attempts, 1ull);
+            if (d.count_swaps) atomicAdd((unsigned long long*)&obs[t].swap_attempts, 1ull);
             if (dd >= 0.0 || u < exp(dd)) {
                 __stcg(perm + t, sb);
                 __stcg(perm + t + 1, sa);
-                atomicAdd((unsigned long long*)&obs[t].swap_accepts, 1ull);
+                if (d.count_swaps) atomicAdd((unsigned long long*)&obs[t].swap_accepts, 1ull);
             }
         }
         __threadfence_block();

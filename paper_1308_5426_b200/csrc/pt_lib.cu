@@ -49,6 +49,7 @@ struct pt_ctx {
     bool fields_valid = false;
     int64_t sweep = 0;
     long long rowsum = 0;  // sum_r Jq[r]
+    int rep_base = 0, n_local = 0;   // slot-sharded context: local storage indices (n_local = 0: not sharded)
     int r_hi = 0;  // largest r <= L/2 with Jq[r] >= 2^16 (direct variant: reach of the high halves)
     int32_t* d_Jq = nullptr;
     uint32_t* d_Jpair = nullptr;
@@ -76,6 +77,7 @@ struct pt_ctx {
         d.key0 = (uint32_t)seed; d.key1 = (uint32_t)(seed >> 32); d.rowsum = (uint32_t)rowsum;
         d.Jq = d_Jq; d.Jpair = d_Jpair; d.beta = d_beta; d.thr_scale = d_scale;
         d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done; d.dbg = d_dbg; d.gen = d_gen; d.Epub = d_Epub;
+        d.rep_base = rep_base; d.n_local = n_local ? n_local : n_rep; d.count_swaps = rep_base == 0 ? 1 : 0;
         return d;
     }
 };
@@ -162,7 +164,7 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
 
 // Direct variant: can all replicas be resident at once (persistent launches with in-kernel swap events)?
 bool persistent_ok(pt_ctx* c) {
-    if (c->variant != PT_VARIANT_DIRECT || c->persistent_policy == 0) return false;
+    if (c->variant != PT_VARIANT_DIRECT || c->persistent_policy == 0 || c->n_local) return false;
     if (c->coresident < 0) c->coresident = ptk::direct_max_coresident(c->dev(), c->r_hi, c->device);
     // A small context (e.g. one of the 40 handles of configs[4]) shares the GPU with others: launches per swap
     // interval interleave their CTAs better than resident kernels that wait at their own barriers (measured:
@@ -315,13 +317,15 @@ void pt_destroy(pt_ctx* ctx) {
 int pt_sweeps_async(pt_ctx* c, int64_t n, int swap_every, int64_t* n_launches) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");
     if (n < 0 || swap_every < 0) return fail(PT_EINVAL, "n and swap_every must be >= 0");
+    if (c->n_local && swap_every != 0)
+        return fail(PT_EINVAL, "slot-sharded context: call pt_sweeps with swap_every = 0 and pt_swap_external");
     int64_t launches = 0;
     constexpr int64_t kMaxChunk = 1 << 16;  // sweeps per launch
     // a persistent launch pays a counter reset and a cooperative launch: worth it from a handful of sweeps per call
     const bool persistent = swap_every > 0 && (n >= 8 || c->persistent_policy == 2) && persistent_ok(c);
     while (n > 0) {
         int64_t chunk = n < kMaxChunk ? n : kMaxChunk;
-        int swap_mode = 0;
+        int swap_mode = c->n_local ? 3 : 0;
         if (persistent) {
             swap_mode = 2;
         } else if (swap_every > 0) {
@@ -438,6 +442,50 @@ int pt_get_couplings(pt_ctx* c, int32_t* Jq) {
 
 int64_t pt_sweep_counter(pt_ctx* c) { return c ? c->sweep : -1; }
 
+int pt_create_shard(pt_ctx** out, int L, int q, double sigma, int n_rep, const double* betas, uint64_t seed,
+                    int ens_base, int rep_base, int n_local) {
+    if (out) *out = nullptr;
+    if (rep_base < 0 || n_local < 1 || n_rep < 1 || (long long)rep_base + n_local > n_rep)
+        return fail(PT_EINVAL, "need 0 <= rep_base, n_local >= 1 and rep_base + n_local <= n_rep");
+    pt_ctx* c = nullptr;
+    int rc = pt_create_ex(&c, L, q, sigma, 1, n_rep, betas, seed, ens_base);
+    if (rc) return rc;
+    if (c->variant != PT_VARIANT_DIRECT) {
+        pt_destroy(c);
+        return fail(PT_EINVAL, "slot-sharded contexts need the direct variant (L % 64 == 0, 64 <= L <= 4096)");
+    }
+    c->rep_base = rep_base;
+    c->n_local = n_local;
+    *out = c;
+    return PT_OK;
+}
+
+int pt_energy_storage_dev(pt_ctx* c, int64_t* E_out_dev) {
+    if (!c || !E_out_dev) return fail(PT_EINVAL, "NULL argument");
+    const int n = c->n_local ? c->n_local : c->R();
+    PT_CUDA(cudaMemcpyAsync(E_out_dev, c->d_E + c->rep_base, (size_t)n * sizeof(long long), cudaMemcpyDeviceToDevice,
+                            c->stream));
+    return pt_sync(c);
+}
+
+int pt_swap_external(pt_ctx* c, const int64_t* E_all_dev) {
+    if (!c || !E_all_dev) return fail(PT_EINVAL, "NULL argument");
+    if (!c->n_local) return fail(PT_EINVAL, "pt_swap_external is for slot-sharded contexts (pt_create_shard)");
+    PT_CUDA(cudaMemcpyAsync(c->d_E, E_all_dev, (size_t)c->n_rep * sizeof(long long), cudaMemcpyDeviceToDevice,
+                            c->stream));
+    ptk::swap_kernel<<<1, 256, 0, c->stream>>>(c->dev(), (uint32_t)c->sweep);
+    PT_CUDA(cudaGetLastError());
+    return pt_sync(c);
+}
+
+int pt_get_perm(pt_ctx* c, int32_t* perm) {
+    if (!c || !perm) return fail(PT_EINVAL, "NULL argument");
+    int rc = pt_sync(c);
+    if (rc) return rc;
+    PT_CUDA(cudaMemcpy(perm, c->d_perm, (size_t)c->R() * sizeof(int), cudaMemcpyDeviceToHost));
+    return PT_OK;
+}
+
 #ifdef PT_TIMING
 // Development builds only (-DPT_TIMING): per-warp clock sums of the sweep kernel, [R][32][8].
 int pt_debug_timing(pt_ctx* c, long long* out) {
@@ -450,6 +498,7 @@ int pt_debug_timing(pt_ctx* c, long long* out) {
 
 int pt_set_variant(pt_ctx* c, int variant) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");
+    if (c->n_local && variant == PT_VARIANT_FIELD) return fail(PT_EINVAL, "slot-sharded contexts need the direct variant");
     int v = 0;
     int rc = resolve_variant(c->L, c->q, c->rowsum, variant, &v);
     if (rc) return rc;

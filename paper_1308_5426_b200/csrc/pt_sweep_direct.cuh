@@ -296,7 +296,9 @@ template <int NEARQ, bool NJR64, bool Q16>
 __global__ void __launch_bounds__(DIRECT_MAX_THREADS, 1)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi) {
     // swap_mode 0: no swap event; 1: one event at the end of the launch (last-arriving CTA, nobody waits);
-    // 2: persistent launch, an event inside the kernel after every sweep whose index is a multiple of swap_every.
+    // 2: persistent launch, an event inside the kernel after every sweep whose index is a multiple of swap_every;
+    // 3: slot-sharded context (one ensemble): CTA b sweeps the configuration with storage index rep_base + b at
+    //    whatever slot it occupies now; no swap event (the caller exchanges energies and calls pt_swap_external).
     constexpr bool FULL_HI = NEARQ == 0;
     constexpr int NQ = NEARQ ? NEARQ : 1;
     extern __shared__ uint32_t smem_d[];
@@ -329,7 +331,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     __shared__ __align__(16) int s_xch[2][32][4];   // partial sums exchanged between the chain warps
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int e = blockIdx.x / d.n_rep;
+    const int e = swap_mode == 3 ? 0 : blockIdx.x / d.n_rep;
     int t = blockIdx.x % d.n_rep;   // slot (temperature) of this CTA's configuration; moves in swap_mode 2
     // state that the previous launch wrote (perm, spins, E) and, for persistent launches, the ensemble's tables
     size_t x = 0;
@@ -337,7 +339,10 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     uint32_t* g_sp = nullptr;
 #define PT_LOAD_STATE()                                             \
     do {                                                                     \
-        st = d.perm[blockIdx.x];                                             \
+        st = swap_mode == 3 ? d.rep_base + (int)blockIdx.x : d.perm[blockIdx.x];  \
+        if (swap_mode == 3)                                                  \
+            for (int t2 = tid; t2 < d.n_rep; t2 += NT)                       \
+                if (d.perm[t2] == st) s_slot = t2;                           \
         x = (size_t)e * d.n_rep + st;                                        \
         g_sp = d.spins + x * W;                                              \
         for (int w = tid; w < W; w += NT) m.sp[w] = g_sp[w];                 \
@@ -410,6 +415,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         }
         PT_LOAD_STATE();
         cta_sync();
+        if (swap_mode == 3) { t = s_slot; scale = d.thr_scale[t]; }
 
         for (int s = 0; s < n_sweeps; ++s) {
             PT_T0(t_draw);
@@ -558,6 +564,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         ObsAcc& oa = s_oa;
         if (owner) { oa = ObsAcc(); s_E = d.E[x]; }
         cta_sync();
+        if (swap_mode == 3) { t = s_slot; scale = d.thr_scale[t]; }
         // A per-lane zero the compiler cannot see through: xor-ed into the accept masks it keeps the bit tests
         // on the ALU pipe (LOP3 -> predicate, SEL) instead of shift pairs on the FMA or uniform pipes.
         const unsigned lz = (unsigned)m.Jz[lane];
@@ -858,7 +865,7 @@ inline int launch_sweep_direct(const Dev& d, long long sweep0, int n_sweeps, int
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return (int)err;
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)(d.n_ens * d.n_rep));
+    cfg.gridDim = dim3((unsigned)(swap_mode == 3 ? d.n_local : d.n_ens * d.n_rep));
     cfg.blockDim = dim3((unsigned)direct_threads(d.L));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;

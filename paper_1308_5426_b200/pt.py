@@ -21,7 +21,8 @@ STATUS = {0: "PT_OK", -1: "PT_EINVAL", -2: "PT_EOVERFLOW", -3: "PT_ENOMEM", -4: 
 SYMBOLS = ["pt_create", "pt_create_ex", "pt_destroy", "pt_sweeps", "pt_energy", "pt_energy_dev",
            "pt_observables", "pt_get_spins", "pt_get_spins_dev", "pt_set_spins", "pt_get_couplings",
            "pt_sweep_counter", "pt_set_variant", "pt_get_variant", "pt_set_stream", "pt_sweeps_async",
-           "pt_sync", "pt_last_error"]
+           "pt_sync", "pt_last_error", "pt_create_shard", "pt_energy_storage_dev", "pt_swap_external",
+           "pt_get_perm"]
 
 
 class PTError(RuntimeError):
@@ -51,6 +52,10 @@ _lib = ctypes.CDLL(LIB_PATH)
 _vp, _i32, _i64, _u64, _dbl = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_uint64, ctypes.c_double
 _lib.pt_create.argtypes = [ctypes.POINTER(_vp), _i32, _i32, _dbl, _i32, _i32, _vp, _u64]
 _lib.pt_create_ex.argtypes = [ctypes.POINTER(_vp), _i32, _i32, _dbl, _i32, _i32, _vp, _u64, _i32]
+_lib.pt_create_shard.argtypes = [ctypes.POINTER(_vp), _i32, _i32, _dbl, _i32, _vp, _u64, _i32, _i32, _i32]
+_lib.pt_energy_storage_dev.argtypes = [_vp, _vp]
+_lib.pt_swap_external.argtypes = [_vp, _vp]
+_lib.pt_get_perm.argtypes = [_vp, _vp]
 _lib.pt_destroy.argtypes = [_vp]
 _lib.pt_destroy.restype = None
 _lib.pt_sweeps.argtypes = [_vp, _i64, _i32]
@@ -83,15 +88,23 @@ def _p(a):
 class PT:
     """One libpt context: n_ens ensembles x n_rep replicas of the (L, q, sigma) model."""
 
-    def __init__(self, L, q, sigma, n_ens, n_rep, betas, seed, ens_base=0, variant="auto"):
+    def __init__(self, L, q, sigma, n_ens, n_rep, betas, seed, ens_base=0, variant="auto", shard=None):
+        """shard = (rep_base, n_local): slot-sharded context (pt_create_shard; one ensemble)."""
         b = np.ascontiguousarray(betas, dtype=np.float64)
         if b.ndim != 1 or b.shape[0] != n_rep:
             raise ValueError("betas must have n_rep entries")
         self.L, self.q, self.n_ens, self.n_rep = int(L), int(q), int(n_ens), int(n_rep)
         self.betas = b
+        self.shard = None if shard is None else (int(shard[0]), int(shard[1]))
         self._h = _vp()
-        _check(_lib.pt_create_ex(ctypes.byref(self._h), int(L), int(q), float(sigma), int(n_ens), int(n_rep),
-                                 _p(b), int(seed) & 0xFFFFFFFFFFFFFFFF, int(ens_base)))
+        if self.shard is None:
+            _check(_lib.pt_create_ex(ctypes.byref(self._h), int(L), int(q), float(sigma), int(n_ens), int(n_rep),
+                                     _p(b), int(seed) & 0xFFFFFFFFFFFFFFFF, int(ens_base)))
+        else:
+            if n_ens != 1:
+                raise ValueError("a slot-sharded context holds one ensemble")
+            _check(_lib.pt_create_shard(ctypes.byref(self._h), int(L), int(q), float(sigma), int(n_rep), _p(b),
+                                        int(seed) & 0xFFFFFFFFFFFFFFFF, int(ens_base), self.shard[0], self.shard[1]))
         if variant != "auto":
             self.set_variant(variant)
 
@@ -134,6 +147,22 @@ class PT:
         assert out.is_cuda and out.numel() == self.n_ens * self.n_rep and out.element_size() == 8
         _check(_lib.pt_energy_dev(self._h, ctypes.c_void_p(out.data_ptr()), int(bool(recompute))))
         return out
+
+    def energy_storage_dev(self, out):
+        """Slot-sharded contexts: out = torch int64 CUDA tensor with n_local elements (storage order)."""
+        assert out.is_cuda and out.element_size() == 8
+        _check(_lib.pt_energy_storage_dev(self._h, ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    def swap_external(self, E_all):
+        """Slot-sharded contexts: E_all = torch int64 CUDA tensor, energies of all n_rep configurations, storage order."""
+        assert E_all.is_cuda and E_all.numel() == self.n_rep and E_all.element_size() == 8 and E_all.is_contiguous()
+        _check(_lib.pt_swap_external(self._h, ctypes.c_void_p(E_all.data_ptr())))
+
+    def get_perm(self):
+        perm = np.zeros((self.n_ens, self.n_rep), dtype=np.int32)
+        _check(_lib.pt_get_perm(self._h, _p(perm)))
+        return perm
 
     def observables(self):
         arr = (Obs * (self.n_ens * self.n_rep))()

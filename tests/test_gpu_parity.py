@@ -299,3 +299,71 @@ def test_persistent_and_per_interval_launches_agree_with_the_oracle(pt, oracle, 
             assert_same_state(g, o, "policy %s L=%d q=%d swap_every=%d after +%d" % (policy, L, q, swap_every, n))
         assert int(o.observables()["swap_accepts"].sum()) > 0
         g.close()
+
+
+@pytest.mark.parametrize("cuts", [(0, 7), (0, 3, 7), (0, 2, 4, 7)])
+def test_slot_sharded_ensemble_reproduces_the_oracle(pt, oracle, cuts):
+    """one ensemble spread over several processes, emulated here by several slot-sharded contexts
+    on one GPU.  Each shard sweeps its own configurations; at a swap event only the energies are exchanged (the
+    all-gather is a concatenation here) and every shard takes the same decisions.  Assembled spins and energies, and the
+    summed accumulators, must equal the unsharded oracle run bit for bit."""
+    import torch
+    from paper_1308_5426_b200 import shard
+    L, q, sigma, n_rep, seed = 256, 5, 0.6, 7, 99
+    b = inputs.geometric_betas(0.7, 2.4, n_rep)
+    bases = list(cuts[:-1])
+    counts = [cuts[i + 1] - cuts[i] for i in range(len(cuts) - 1)]
+    gs = [pt.PT(L, q, sigma, 1, n_rep, b, seed, shard=(bs, c)) for bs, c in zip(bases, counts)]
+    o = oracle.Oracle(L, q, sigma, 1, n_rep, b, seed)
+    loc = [torch.zeros(c, dtype=torch.int64, device="cuda") for c in counts]
+    for n_sweeps, swap_every in ((5, 1), (9, 2), (20, 1)):
+        for _ in range(n_sweeps):
+            for g in gs:
+                g.sweeps(1, 0)
+            if gs[0].sweep_counter() % swap_every == 0:
+                E_all = torch.cat([g.energy_storage_dev(x) for g, x in zip(gs, loc)])   # the exchange step
+                for g in gs:
+                    g.swap_external(E_all)
+        # the oracle's swap period is tested on its global sweep counter, like ours
+        o.sweeps(n_sweeps, swap_every)
+        perms = [g.get_perm()[0] for g in gs]
+        for p_ in perms[1:]:
+            np.testing.assert_array_equal(p_, perms[0])
+        spins = shard.merge_shards([g.get_spins()[0] for g in gs], perms, bases, counts)
+        E = shard.merge_shards([g.energy()[0] for g in gs], perms, bases, counts)
+        np.testing.assert_array_equal(spins, o.get_spins()[0])
+        np.testing.assert_array_equal(E, o.energy()[0])
+        tot, oo = shard.sum_observables([g.observables() for g in gs]), o.observables()
+        for f in CMP_FIELDS:
+            np.testing.assert_array_equal(tot[f], oo[f], err_msg="sharded: " + f)
+    with pytest.raises(pt.PTError):
+        gs[0].sweeps(1, 1)   # swap events of a sharded context go through swap_external
+    for g in gs:
+        g.close()
+
+
+def test_sharded_ensemble_driver_single_rank_nccl(pt, oracle):
+    """shard.ShardedEnsemble (sweeps -> all-gather of the energies -> pt_swap_external) with a one-rank NCCL group
+    and without a group; both must follow the oracle."""
+    import socket
+    import torch
+    import torch.distributed as dist
+    from paper_1308_5426_b200 import shard
+    L, q, sigma, n_rep, seed = 128, 4, 0.5, 6, 5
+    b = inputs.geometric_betas(0.8, 2.2, n_rep)
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    dist.init_process_group("nccl", init_method="tcp://127.0.0.1:%d" % port, rank=0, world_size=1,
+                            device_id=torch.device("cuda", torch.cuda.current_device()))
+    try:
+        for group in (dist, None):
+            ens = shard.ShardedEnsemble(pt, L, q, sigma, n_rep, b, seed, dist=group)
+            o = oracle.Oracle(L, q, sigma, 1, n_rep, b, seed)
+            for n, swap_every in ((7, 1), (10, 3)):
+                ens.sweeps(n, swap_every)
+                o.sweeps(n, swap_every)
+                assert_same_state(ens.g, o, "ShardedEnsemble, group %s" % ("nccl" if group else "none"))
+            ens.close()
+    finally:
+        dist.destroy_process_group()

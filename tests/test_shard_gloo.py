@@ -39,6 +39,15 @@ def _worker(rank, world, port, n_ens_total, out_dir):
         E_all = shard.gather_ensembles(E, n_ens_total, dist)
         acc_all = shard.gather_ensembles(acc, n_ens_total, dist)
         sE_all = shard.gather_ensembles(sE, n_ens_total, dist)
+        # exchange step of a slot-sharded ensemble: uneven blocks, padded all_gather, global order
+        import torch
+        for n_total in (7, 8, 2):
+            b0, nl = shard.ensemble_shard(n_total, world, rank)
+            n_max = -(-n_total // world)
+            loc = torch.full((n_max,), -1, dtype=torch.int64)
+            loc[:nl] = torch.arange(b0, b0 + nl) * 1000003
+            got = shard.all_gather_blocks(loc, n_total, dist)
+            assert torch.equal(got, torch.arange(n_total) * 1000003), (rank, n_total, got)
         t_max = shard.max_over_ranks(10.0 + rank, dist)
         assert t_max == 10.0 + world - 1
         if rank == 0:
