@@ -367,3 +367,17 @@ def test_sharded_ensemble_driver_single_rank_nccl(pt, oracle):
             ens.close()
     finally:
         dist.destroy_process_group()
+
+
+def test_more_replicas_than_sms(pt, oracle):
+    """400 replicas (the paper's replica count) on 148 SMs: several waves of CTAs per launch, swap event
+    by the last CTA to arrive; and 2 x 100 replicas as two ensembles."""
+    for (L, q, n_ens, n_rep) in [(128, 3, 1, 400), (64, 3, 2, 100)]:
+        T = np.linspace(0.5, 3.0, n_rep)   # uniform ladder as in the paper
+        g = pt.PT(L, q, 0.5, n_ens, n_rep, 1.0 / T, 400)
+        o = oracle.Oracle(L, q, 0.5, n_ens, n_rep, 1.0 / T, 400)
+        for n in (3, 25):
+            g.sweeps(n, 1)
+            o.sweeps(n, 1, field=True, threads=THREADS)
+            assert_same_state(g, o, "L=%d, %d x %d replicas" % (L, n_ens, n_rep))
+        g.close()
