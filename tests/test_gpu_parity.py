@@ -369,9 +369,11 @@ def test_sharded_ensemble_driver_single_rank_nccl(pt, oracle):
         dist.destroy_process_group()
 
 
-def test_more_replicas_than_sms(pt, oracle):
-    """400 replicas (the paper's replica count) on 148 SMs: several waves of CTAs per launch, swap event
+@pytest.mark.parametrize("policy", ["0", "1"])
+def test_more_replicas_than_sms(pt, oracle, policy, monkeypatch):
+    """(PT_PERSISTENT=0: one ordinary launch per sweep; 1: default policy, persistent where co-resident.)  400 replicas (the paper's replica count) on 148 SMs: several waves of CTAs per launch, swap event
     by the last CTA to arrive; and 2 x 100 replicas as two ensembles."""
+    monkeypatch.setenv("PT_PERSISTENT", policy)
     for (L, q, n_ens, n_rep) in [(128, 3, 1, 400), (64, 3, 2, 100)]:
         T = np.linspace(0.5, 3.0, n_rep)   # uniform ladder as in the paper
         g = pt.PT(L, q, 0.5, n_ens, n_rep, 1.0 / T, 400)
