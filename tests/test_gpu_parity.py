@@ -383,3 +383,27 @@ def test_more_replicas_than_sms(pt, oracle, policy, monkeypatch):
             o.sweeps(n, 1, field=True, threads=THREADS)
             assert_same_state(g, o, "L=%d, %d x %d replicas" % (L, n_ens, n_rep))
         g.close()
+
+
+def test_binder_crossing_reproduces_the_papers_critical_temperature(pt):
+    """Physics check of the whole path (not parity): the Binder cumulants V_M (Eq. 12) of two sizes cross at the
+    critical temperature; the paper's Table 1 gives T_c = 2.085(5) for q=3, sigma=0.4.  64 replicas on
+    a uniform ladder T in [1.95, 2.25], 2e4 + 6e4 sweeps, swap every sweep, L = 256 and 512 (about 3 s of GPU time)."""
+    from paper_1308_5426_b200 import pt_math
+    q, sigma, n_rep = 3, 0.4, 64
+    T = np.linspace(1.95, 2.25, n_rep)
+    V = {}
+    for L in (256, 512):
+        g = pt.PT(L, q, sigma, 1, n_rep, 1.0 / T, 1234 + L)
+        g.sweeps(20000, 1)
+        base = g.observables()
+        g.sweeps(60000, 1)
+        V[L] = pt_math.cumulants(pt_math.obs_diff(g.observables(), base), L, q)["V_M"][0]
+        g.close()
+        assert 0.6 < V[L][0] < 2.0 / 3.0 and V[L][-1] < 0.3      # ordered (V_M -> 2/3) ... disordered
+    d = V[256] - V[512]
+    idx = np.where(np.sign(d[:-1]) != np.sign(d[1:]))[0]
+    crossings = [T[i] + (T[i + 1] - T[i]) * d[i] / (d[i] - d[i + 1]) for i in idx]
+    assert crossings, "the cumulants of L=256 and L=512 do not cross"
+    best = min(crossings, key=lambda x: abs(x - 2.085))
+    assert abs(best - 2.085) < 0.01, crossings
