@@ -60,7 +60,10 @@ typedef enum {
  *                     time, with exact integer corrections for the changes
  *                     accepted inside the block.  Needs L % 64 == 0,
  *                     64 <= L <= 4096 and sum_r Jq[r] < 2^30 - 1.
- *  PT_VARIANT_AUTO  : DIRECT where it applies, else FIELD. */
+ *  PT_VARIANT_AUTO  : DIRECT where it applies, else FIELD.
+ * Environment: PT_VARIANT=direct|field|auto sets the variant chosen by pt_create; PT_PERSISTENT=0|1|2 the launch
+ * policy of the direct variant (0: one launch per swap interval; 1, default: persistent launches with the swap events
+ * inside the kernel for contexts that take at least a third of the SMs; 2: whenever all replicas can be co-resident). */
 enum { PT_VARIANT_AUTO = 0, PT_VARIANT_FIELD = 1, PT_VARIANT_DIRECT = 2 };
 
 /* Cumulative per-slot accumulators since pt_create (the caller differences two

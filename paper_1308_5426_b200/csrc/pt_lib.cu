@@ -276,7 +276,12 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
         if (Jq[r] >= 65536) c->r_hi = r;
     c->rowsum = rowsum;
     {
-        int rc = resolve_variant(L, q, rowsum, PT_VARIANT_AUTO, &c->variant);
+        // PT_VARIANT=direct|field|auto overrides the default choice (an impossible request is an error)
+        int want = PT_VARIANT_AUTO;
+        const char* env = getenv("PT_VARIANT");
+        if (env && !strcmp(env, "direct")) want = PT_VARIANT_DIRECT;
+        else if (env && !strcmp(env, "field")) want = PT_VARIANT_FIELD;
+        int rc = resolve_variant(L, q, rowsum, want, &c->variant);
         if (rc) { free_ctx(c); return rc; }
     }
     if (bad || rowsum >= (1ll << 31)) {
