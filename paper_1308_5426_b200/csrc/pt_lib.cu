@@ -68,6 +68,7 @@ struct pt_ctx {
     unsigned* d_gen = nullptr;
     long long* d_Epub = nullptr;
     int coresident = -1;   // direct variant: CTAs that fit on the device at once (-1: not asked yet)
+    ptk::direct_kernel_t direct_kern = nullptr;   // the sweep kernel instantiation this context uses
     int persistent_policy = 1;   // 0 never, 1 when the context fills the device and the call is long enough, 2 whenever possible
 
     int R() const { return n_ens * n_rep; }
@@ -154,7 +155,9 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
                                                                                  swap_mode == 1 ? 1 : 0);
     } else {
         c->fields_valid = false;
-        int rc = ptk::launch_sweep_direct(d, (long long)c->sweep, n_sweeps, swap_mode, swap_every, c->r_hi, c->stream);
+        if (!c->direct_kern) c->direct_kern = ptk::select_direct_kernel(d, c->r_hi, c->device, &c->coresident);
+        int rc = ptk::launch_sweep_direct(c->direct_kern, d, (long long)c->sweep, n_sweeps, swap_mode, swap_every,
+                                          c->r_hi, c->stream);
         if (rc) return fail(PT_ECUDA, std::string("sweep_direct launch: ") + cudaGetErrorString((cudaError_t)rc));
     }
     PT_CUDA(cudaGetLastError());
@@ -165,7 +168,7 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
 // Direct variant: can all replicas be resident at once (persistent launches with in-kernel swap events)?
 bool persistent_ok(pt_ctx* c) {
     if (c->variant != PT_VARIANT_DIRECT || c->persistent_policy == 0 || c->n_local) return false;
-    if (c->coresident < 0) c->coresident = ptk::direct_max_coresident(c->dev(), c->r_hi, c->device);
+    if (!c->direct_kern) c->direct_kern = ptk::select_direct_kernel(c->dev(), c->r_hi, c->device, &c->coresident);
     // A small context (e.g. one of the 40 handles of configs[4]) shares the GPU with others: launches per swap
     // interval interleave their CTAs better than resident kernels that wait at their own barriers (measured:
     // 4.2e9 against 3.6e9 attempts/s on configs[4]).  Persistent launches are for contexts that take at least a

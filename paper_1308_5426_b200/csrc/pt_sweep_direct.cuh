@@ -67,18 +67,24 @@
 
 namespace ptk {
 
-constexpr int DIRECT_MAX_BULK = 512;
+constexpr int DIRECT_SITES = 8;     // sites of a block per bulk thread (4 threads x 8 sites = 32)
+constexpr int DIRECT_MAX_BULK = 256;
 constexpr int DIRECT_CHAIN_WARPS = 4;                       // one per SM sub-partition
 constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 32 * DIRECT_CHAIN_WARPS;
-constexpr int DIRECT_NPAIR = 35;   // packed coupling pairs per thread and half
+constexpr int DIRECT_NPAIR = 39;   // packed coupling pairs per thread and half: 64 + 2*7 couplings
+constexpr int ENERGY_MAX_THREADS = 512, ENERGY_NPAIR = 35;   // energy_direct_kernel: 4 sites x 64 j per thread
 constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: the 224 sites (56 quads) around a block
 constexpr int DIRECT_NEAR_QUADS = 56;
 constexpr int DIRECT_MAX_PERSIST_REP = 512;   // replicas per ensemble in a persistent launch (static shared arrays)
 
 __host__ __device__ inline bool direct_applies(int L, int q) {
-    return (L % 64) == 0 && L >= 64 && L <= 64 * (DIRECT_MAX_BULK / 8) && q <= 16;
+    return (L % 64) == 0 && L >= 64 && L <= 64 * (DIRECT_MAX_BULK / 4) && q <= 16;
 }
 __host__ __device__ inline int direct_bulk_threads(int L) {
+    const int t = 4 * (L / 64);
+    return t < 32 ? 32 : (t + 31) / 32 * 32;
+}
+__host__ __device__ inline int energy_threads(int L) {
     const int t = 8 * (L / 64);
     return t < 32 ? 32 : (t + 31) / 32 * 32;
 }
@@ -292,8 +298,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 // NEARQ = 0: the bulk warps sum both 16-bit halves of every coupling.  NEARQ = 1, 2, 4: they sum the low halves
 // only, plus the high halves of NEARQ of the 56 quads of sites within distance 95 of the block (requires
 // r_hi <= 95 and NEARQ * L/64 >= 56).  NJR64: L == 4096 (64 j-ranges as a compile-time constant).
-template <int NEARQ, bool NJR64, bool Q16>
-__global__ void __launch_bounds__(DIRECT_MAX_THREADS, 1)
+// MINB: minimum CTAs per SM the register allocation must allow (1: up to 168 registers, for large L; 2: 80 registers,
+// so that several hundred small replicas can be co-resident for persistent launches).
+template <int NEARQ, bool NJR64, bool Q16, int MINB>
+__global__ void __launch_bounds__(DIRECT_MAX_THREADS, MINB)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi) {
     // swap_mode 0: no swap event; 1: one event at the end of the launch (last-arriving CTA, nobody waits);
     // 2: persistent launch, an event inside the kernel after every sweep whose index is a multiple of swap_every;
@@ -366,9 +374,9 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
 
     if (tid < NTB) {
         // =========================== BULK warps ===========================
-        // thread -> (site group g, j-range jr); group g = sites 8(g>>1) + (g&1) + {0,2,4,6}
-        const int g = tid & 7, jr = tid >> 3;
-        const int par = g & 1, gbase = 8 * (g >> 1) + par;
+        // thread -> (site group g, j-range jr); group g = the 8 sites 16(g>>1) + (g&1) + {0,2,..,14}
+        const int g = tid & 3, jr = tid >> 2;
+        const int par = g & 1, gbase = 16 * (g >> 1) + par;
         const int NJR = NJR64 ? 64 : L / 64;
         const bool active = jr < NJR;
         // couplings of this thread: pair tt holds Jq[r], Jq[r-1] with r = R0 - 2 tt  (mod L)
@@ -376,7 +384,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         uint32_t PH[FULL_HI ? DIRECT_NPAIR : 1];
         {
             const int H = L / 2;
-            const int R0 = ((gbase + 6 - 64 * jr) % L + L) % L;
+            const int R0 = ((gbase + 14 - 64 * jr) % L + L) % L;
             const uint32_t* lo = d.Jpair + (size_t)(2 * par) * H;
             const uint32_t* hi = lo + H;
             int r = R0;   // r = R0 - 2 tt (mod L) keeps the parity of `par`: no division or modulo per load
@@ -393,13 +401,13 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         // NEAR: high halves of quad n = jr + NJR*iq (sites i0 - 96 + 4n + {0..3}) for this thread's 4 sites:
         // NP[iq][mm][0] = hi(|r|) | hi(|r-1|) << 16, [1] = hi(|r-2|) | hi(|r-3|) << 16, r = gbase + 2mm + 96 - 4n,
         // hi(x) = Jq[x] >> 16 for 1 <= x <= r_hi, else 0.
-        uint32_t NP[NQ][4][2];
+        uint32_t NP[NQ][DIRECT_SITES][2];
         if (NEARQ) {
 #pragma unroll
             for (int iq = 0; iq < NQ; ++iq) {
                 const int n = jr + NJR * iq;
 #pragma unroll
-                for (int mm = 0; mm < 4; ++mm) {
+                for (int mm = 0; mm < DIRECT_SITES; ++mm) {
                     uint32_t hv[4];
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
@@ -443,16 +451,16 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 // also frees buffer kb&1), block kb-1 as at the start of the sweep, blocks >= kb untouched
                 if (kb >= 2) mbar_wait(&s_done[kb & 1], ((kb >> 1) - 1) & 1);
                 PT_T0(t_b);
-                uint32_t val[4] = {0u, 0u, 0u, 0u};
+                uint32_t val[DIRECT_SITES] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
                 if (active) {
                     int wj2 = wj + 4;
                     wj2 -= wj2 >= W ? W : 0;
                     const uint4 wa = *reinterpret_cast<const uint4*>(m.sp + wj);
                     const uint4 wb = *reinterpret_cast<const uint4*>(sp2 + wj2);
                     const uint32_t words[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
-                    uint2 lt[4], ltb[4];
+                    uint2 lt[DIRECT_SITES], ltb[DIRECT_SITES];
 #pragma unroll
-                    for (int mm = 0; mm < 4; ++mm) {
+                    for (int mm = 0; mm < DIRECT_SITES; ++mm) {
                         lt[mm] = lutp[2 * mm];
                         ltb[mm] = Q16 ? lutp[L + 2 * mm] : make_uint2(0u, 0u);
                     }
@@ -463,15 +471,17 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                         nword[iq] = NEARQ ? ((n >= 16 && n < 24) ? m.sp0 : m.sp)[wn[iq]] : 0u;
                     }
                     // two accumulators per site (even / odd pair of j) keep the IDP.2A chains short
-                    uint32_t alo[4] = {0u, 0u, 0u, 0u}, alo2[4] = {0u, 0u, 0u, 0u}, ahi[4] = {0u, 0u, 0u, 0u};
+                    uint32_t alo[DIRECT_SITES], alo2[DIRECT_SITES], ahi[DIRECT_SITES];
+#pragma unroll
+                    for (int mm = 0; mm < DIRECT_SITES; ++mm) { alo[mm] = 0u; alo2[mm] = 0u; ahi[mm] = 0u; }
 #pragma unroll
                     for (int u = 0; u < 16; ++u) {
                         const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
                         const uint32_t selx = sel ^ 0x8888u;
 #pragma unroll
-                        for (int mm = 0; mm < 4; ++mm) {
+                        for (int mm = 0; mm < DIRECT_SITES; ++mm) {
                             const uint32_t S = tab_lookup<Q16>(lt[mm], ltb[mm], sel, selx);
-                            const int tt = 3 - mm + 2 * u;
+                            const int tt = 7 - mm + 2 * u;
                             alo[mm] = __dp2a_lo(PL[tt], S, alo[mm]);
                             alo2[mm] = __dp2a_hi(PL[tt + 1], S, alo2[mm]);
                             if (FULL_HI) {
@@ -486,7 +496,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                             const int n = jr + NJR * iq;
                             const uint32_t sel = (n & 1) ? (nword[iq] >> 16) : nword[iq];
 #pragma unroll
-                            for (int mm = 0; mm < 4; ++mm) {
+                            for (int mm = 0; mm < DIRECT_SITES; ++mm) {
                                 const uint32_t S = tab_lookup<Q16>(lt[mm], ltb[mm], sel, sel ^ 0x8888u);
                                 ahi[mm] = __dp2a_lo(NP[iq][mm][0], S, ahi[mm]);
                                 ahi[mm] = __dp2a_hi(NP[iq][mm][1], S, ahi[mm]);
@@ -494,7 +504,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                         }
                     }
 #pragma unroll
-                    for (int mm = 0; mm < 4; ++mm) val[mm] = alo[mm] + alo2[mm] + (ahi[mm] << 16);
+                    for (int mm = 0; mm < DIRECT_SITES; ++mm) val[mm] = alo[mm] + alo2[mm] + (ahi[mm] << 16);
                     // advance the cursors
                     lutp += 32;
                     wj += 4;
@@ -505,14 +515,21 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                         wn[iq] -= wn[iq] >= W ? W : 0;
                     }
                 }
+                // block sums: transpose-reduce over the 8 lanes of a warp that hold the same site group (lane bits
+                // 2..4 = j-range): 4 + 2 + 1 shuffles leave one site per lane, m = lane bits (2,3,4), then one
+                // shared-memory atomic per lane (32 different sites per warp)
+                {
+                    uint32_t v4[4], v2[2];
+                    const bool u4 = lane & 16, u3 = lane & 8, u2 = lane & 4;
 #pragma unroll
-                for (int mm = 0; mm < 4; ++mm) {
-                    val[mm] += __shfl_xor_sync(0xffffffffu, val[mm], 8);
-                    val[mm] += __shfl_xor_sync(0xffffffffu, val[mm], 16);
-                }
-                if (lane < 8) {
+                    for (int i = 0; i < 4; ++i)
+                        v4[i] = (u4 ? val[i + 4] : val[i]) + __shfl_xor_sync(0xffffffffu, u4 ? val[i] : val[i + 4], 16);
 #pragma unroll
-                    for (int mm = 0; mm < 4; ++mm) atomicAdd(&m.part[(kb & 1) * 32 + gbase + 2 * mm], val[mm]);
+                    for (int i = 0; i < 2; ++i)
+                        v2[i] = (u3 ? v4[i + 2] : v4[i]) + __shfl_xor_sync(0xffffffffu, u3 ? v4[i] : v4[i + 2], 8);
+                    const uint32_t v1 = (u2 ? v2[1] : v2[0]) + __shfl_xor_sync(0xffffffffu, u2 ? v2[0] : v2[1], 4);
+                    const int msite = (u2 ? 1 : 0) + (u3 ? 2 : 0) + (u4 ? 4 : 0);
+                    atomicAdd(&m.part[(kb & 1) * 32 + gbase + 2 * msite], v1);
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&s_full[kb & 1]);
@@ -640,16 +657,16 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                     }
                 }
                 PT_ACC(2, t_s);
-                if (cw == 0) {
-                    if (lane < 4) {
-                        const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
-                        m.sp[wsp] = (w_old & ~nm) | (w_new & nm);
-                    }
-                    m.part[(k & 1) * 32 + lane] = 0u;
+                if (cw == 0 && lane < 4) {
+                    const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
+                    m.sp[wsp] = (w_old & ~nm) | (w_new & nm);
                 }
-                // every chain warp has read the buffers of block k before buffer k&1 is handed back
+                // every chain warp has read the block sums of buffer k&1 (without rounds there is no other barrier
+                // between a slow warp's read and this point) before they are cleared and the buffer is handed back
                 asm volatile("bar.sync 1, 128;" ::: "memory");
                 if (cw == 0) {
+                    m.part[(k & 1) * 32 + lane] = 0u;
+                    __syncwarp();
                     if (lane == 0) mbar_arrive(&s_done[k & 1]);   // block k is final, buffer k&1 is free
                     if ((mask >> lane) & 1u) dE_acc += th - yy;   // yy: slack of every site at its own turn
                     n_acc += __popc(mask);
@@ -729,18 +746,18 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
 // per-site table is the one-hot byte table of the site's own colour.  One CTA per replica (storage order).
 // ---------------------------------------------------------------------------
 template <bool Q16>
-__global__ void __launch_bounds__(DIRECT_MAX_BULK, 1)
+__global__ void __launch_bounds__(ENERGY_MAX_THREADS, 1)
 energy_direct_kernel(Dev d, long long* __restrict__ E_out) {
     extern __shared__ uint32_t smem_ed[];
     uint32_t* sp = smem_ed;   // [W]
-    __shared__ unsigned long long s_tot[DIRECT_MAX_BULK / 32];
+    __shared__ unsigned long long s_tot[ENERGY_MAX_THREADS / 32];
     const int L = d.L, W = d.W;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, NT = blockDim.x;
     const int g = tid & 7, jr = tid >> 3;
     const int par = g & 1, gbase = 8 * (g >> 1) + par;
     const int NJR = L / 64, NB = L >> 5;
     const bool active = jr < NJR;
-    uint32_t PL[DIRECT_NPAIR], PH[DIRECT_NPAIR];
+    uint32_t PL[ENERGY_NPAIR], PH[ENERGY_NPAIR];
     {
         const int H = L / 2;
         const int R0 = ((gbase + 6 - 64 * jr) % L + L) % L;
@@ -748,7 +765,7 @@ energy_direct_kernel(Dev d, long long* __restrict__ E_out) {
         const uint32_t* hi = lo + H;
         int r = R0;
 #pragma unroll
-        for (int tt = 0; tt < DIRECT_NPAIR; ++tt) {
+        for (int tt = 0; tt < ENERGY_NPAIR; ++tt) {
             const int mm = (r - par) >> 1;
             PL[tt] = active ? __ldg(lo + mm) : 0u;
             PH[tt] = active ? __ldg(hi + mm) : 0u;
@@ -812,37 +829,43 @@ energy_direct_kernel(Dev d, long long* __restrict__ E_out) {
 
 inline int launch_energy_direct(const Dev& d, long long* E_out, cudaStream_t stream) {
     if (d.q > 8)
-        energy_direct_kernel<true><<<d.n_ens * d.n_rep, direct_bulk_threads(d.L), (size_t)d.W * 4, stream>>>(d, E_out);
+        energy_direct_kernel<true><<<d.n_ens * d.n_rep, energy_threads(d.L), (size_t)d.W * 4, stream>>>(d, E_out);
     else
-        energy_direct_kernel<false><<<d.n_ens * d.n_rep, direct_bulk_threads(d.L), (size_t)d.W * 4, stream>>>(d, E_out);
+        energy_direct_kernel<false><<<d.n_ens * d.n_rep, energy_threads(d.L), (size_t)d.W * 4, stream>>>(d, E_out);
     return (int)cudaGetLastError();
 }
 
 typedef void (*direct_kernel_t)(Dev, long long, int, int, int, int);
 
 // r_hi = largest r <= L/2 with Jq[r] >= 2^16 (0 if none).
-inline direct_kernel_t select_direct_kernel(const Dev& d, int r_hi) {
+// minb = 1: up to 168 registers per thread (fastest block sums); minb = 2: 80 registers, twice the CTAs per SM.
+inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb) {
     const bool l4096 = d.L == 4096;
+    const int nq = direct_nearq(d.L, r_hi);
     if (d.q <= 8) {
-        switch (direct_nearq(d.L, r_hi)) {
-            case 1: return l4096 ? sweep_direct_kernel<1, true, false> : sweep_direct_kernel<1, false, false>;
-            case 2: return sweep_direct_kernel<2, false, false>;
-            case 4: return sweep_direct_kernel<4, false, false>;
-            default: return l4096 ? sweep_direct_kernel<0, true, false> : sweep_direct_kernel<0, false, false>;
+        if (minb == 1) {
+            switch (nq) {
+                case 1: return l4096 ? sweep_direct_kernel<1, true, false, 1> : sweep_direct_kernel<1, false, false, 1>;
+                case 2: return sweep_direct_kernel<2, false, false, 1>;
+                case 4: return sweep_direct_kernel<4, false, false, 1>;
+                default: return l4096 ? sweep_direct_kernel<0, true, false, 1> : sweep_direct_kernel<0, false, false, 1>;
+            }
+        }
+        return nq == 4 ? sweep_direct_kernel<4, false, false, 2> : sweep_direct_kernel<0, false, false, 2>;
+    }
+    if (minb == 1) {
+        switch (nq) {
+            case 1: return sweep_direct_kernel<1, false, true, 1>;
+            case 2: return sweep_direct_kernel<2, false, true, 1>;
+            case 4: return sweep_direct_kernel<4, false, true, 1>;
+            default: return sweep_direct_kernel<0, false, true, 1>;
         }
     }
-    switch (direct_nearq(d.L, r_hi)) {
-        case 1: return sweep_direct_kernel<1, false, true>;
-        case 2: return sweep_direct_kernel<2, false, true>;
-        case 4: return sweep_direct_kernel<4, false, true>;
-        default: return sweep_direct_kernel<0, false, true>;
-    }
+    return nq == 4 ? sweep_direct_kernel<4, false, true, 2> : sweep_direct_kernel<0, false, true, 2>;
 }
 
-// Number of CTAs of the sweep kernel that can be resident on the device at once (0 on error): a persistent launch
-// (swap_mode 2) needs all n_ens * n_rep of them.
-inline int direct_max_coresident(const Dev& d, int r_hi, int device) {
-    direct_kernel_t kern = select_direct_kernel(d, r_hi);
+// CTAs of a sweep kernel variant that can be resident on the device at once (0 on error).
+inline int direct_coresident(direct_kernel_t kern, const Dev& d, int device) {
     const size_t smem = direct_smem_bytes(d.L, d.q);
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
     int per_sm = 0, n_sm = 0, coop = 0;
@@ -852,16 +875,30 @@ inline int direct_max_coresident(const Dev& d, int r_hi, int device) {
     return per_sm * n_sm;
 }
 
+// The kernel a context uses, and how many of its CTAs fit on the device at once (a persistent launch, swap_mode 2,
+// needs all n_ens * n_rep of them).  The 168-register variant unless only the 80-register one (L < 2048) makes all
+// replicas co-resident.
+inline direct_kernel_t select_direct_kernel(const Dev& d, int r_hi, int device, int* coresident) {
+    direct_kernel_t k1 = direct_kernel_variant(d, r_hi, 1);
+    int c1 = direct_coresident(k1, d, device);
+    if (d.n_ens * d.n_rep > c1 && d.L < 2048) {
+        direct_kernel_t k2 = direct_kernel_variant(d, r_hi, 2);
+        const int c2 = direct_coresident(k2, d, device);
+        if (d.n_ens * d.n_rep <= c2) { k1 = k2; c1 = c2; }
+    }
+    if (coresident) *coresident = c1;
+    return k1;
+}
+
 // Returns a cudaError_t as int.  swap_mode 0/1: one ordinary launch of n_sweeps sweeps, optionally closed by a swap
 // event.  swap_mode 2: cooperative (all CTAs co-resident) persistent launch with the swap events inside the kernel.
 // (Programmatic dependent launch was tried for swap_mode 1 and removed: streams with thousands of dependent
 // launches of this kernel queued back to back occasionally never finished on this driver, and for the small
 // contexts that still use swap_mode 1 it was slower than ordinary launches: 0.41-0.48 s against 0.39 s for 10000
 // sweeps of configs[2].)
-inline int launch_sweep_direct(const Dev& d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi,
-                               cudaStream_t stream) {
+inline int launch_sweep_direct(direct_kernel_t kern, const Dev& d, long long sweep0, int n_sweeps, int swap_mode,
+                               int swap_every, int r_hi, cudaStream_t stream) {
     const size_t smem = direct_smem_bytes(d.L, d.q);
-    direct_kernel_t kern = select_direct_kernel(d, r_hi);
     cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (err != cudaSuccess) return (int)err;
     cudaLaunchConfig_t cfg = {};
