@@ -155,18 +155,20 @@ template <bool Q16>
 __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, uint32_t sweep, int t, uint32_t c3,
                                             double scale) {
     const int W = d.W, q = d.q;
-    for (int w = threadIdx.x; w < W; w += blockDim.x) {
+    // one work item = 4 sites (half a packed word): 2W items over all threads of the CTA
+    for (int hw = threadIdx.x; hw < 2 * W; hw += blockDim.x) {
+        const int w = hw >> 1, h4 = (hw & 1) << 2;
         const uint32_t word = m.sp[w];
-        uint32_t bword = 0, s0 = 0, s1 = 0;
+        uint32_t bhalf = 0, s4 = 0;
 #pragma unroll
-        for (int n = 0; n < 8; ++n) {
-            const int i = 8 * w + n;
+        for (int n = 0; n < 4; ++n) {
+            const int i = 8 * w + h4 + n;
             const Philox4 p = philox4x32_10((uint32_t)i, sweep, (uint32_t)t, c3, d.key0, d.key1);
-            const uint32_t a = (word >> (4 * n)) & 15u;
+            const uint32_t a = (word >> (4 * (h4 + n))) & 15u;
             const uint32_t k = __umulhi(p.w0, (uint32_t)(q - 1));
             const uint32_t b = k + (k >= a ? 1u : 0u);
-            bword |= b << (4 * n);
-            if (n < 4) s0 |= (a | (b << 4)) << (8 * n); else s1 |= (a | (b << 4)) << (8 * (n - 4));
+            bhalf |= b << (4 * n);
+            s4 |= (a | (b << 4)) << (8 * n);
             m.theta[i] = min(accept_threshold(uniform53(p.w1, p.w2), scale), 1 << 30);  // |dE| < 2^30: same decisions
             unsigned long long ta = 0x0101010101010101ull, tb = ta;   // byte k = s'(k), k = 0..7 | 8..15
             if (!Q16 || a < 8u) ta += 1ull << (8 * a); else tb += 1ull << (8 * (a - 8u));
@@ -174,21 +176,31 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
             m.lut[i] = make_uint2((uint32_t)ta, (uint32_t)(ta >> 32));
             if (Q16) m.lutb[i] = make_uint2((uint32_t)tb, (uint32_t)(tb >> 32));
         }
-        m.bq[w] = bword;
-        m.sp0[w] = word;
-        reinterpret_cast<uint2*>(m.selb)[w] = make_uint2(s0, s1);
+        reinterpret_cast<uint16_t*>(m.bq)[hw] = (uint16_t)bhalf;   // low half of word w = sites 8w .. 8w+3
+        reinterpret_cast<uint32_t*>(m.selb)[hw] = s4;
+        if (h4 == 0) m.sp0[w] = word;
     }
 }
 
-// N_max of the configuration (Eq. 10), as count_nmax but on cta_sync.
+// N_max of the configuration (Eq. 10): per-thread colour counts in registers, one warp reduction and one shared-memory
+// atomic per colour and warp.  Called by all threads (cta_sync inside); every thread gets the result.
 __device__ __forceinline__ int direct_nmax(const uint32_t* sp, int W, int q, int* s_cnt) {
     if (threadIdx.x < 16) s_cnt[threadIdx.x] = 0;
     cta_sync();
+    int cnt[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) cnt[k] = 0;
     for (int w = threadIdx.x; w < W; w += blockDim.x) {
         const uint32_t word = sp[w];
-        for (int k = 0; k < q; ++k) {
-            const int c = __popc(match_nibbles(word, (uint32_t)k));
-            if (c) atomicAdd(&s_cnt[k], c);
+#pragma unroll
+        for (int k = 0; k < 16; ++k)
+            if (k < q) cnt[k] += __popc(match_nibbles(word, (uint32_t)k));
+    }
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        if (k < q) {
+            const int c = __reduce_add_sync(0xffffffffu, cnt[k]);
+            if ((threadIdx.x & 31) == 0 && c) atomicAdd(&s_cnt[k], c);
         }
     }
     cta_sync();
