@@ -33,8 +33,8 @@ UNIT = "attempts/s"
 IDP_LANES_PER_CLK_PER_SM = 64
 MACS_PER_IDP_LANE = 2
 # dram__bytes_read.sum + dram__bytes_write.sum per sweep of a persistent sweep_direct_kernel launch
-# (ncu --set full on a 40-sweep launch: 683 KB, profiles/r1_d_direct_v6.md)
-DRAM_BYTES_PER_SWEEP = 17.1e3
+# (ncu --set full on a 40-sweep launch: 407.6 KB read + 10.2 KB written, profiles/r1_f_direct_v8.md)
+DRAM_BYTES_PER_SWEEP = 10.45e3
 N_SM = 148
 
 

@@ -3,8 +3,8 @@
 // after", an O(L) sum per step, O(L^2) per sweep), organised for sm_100a.
 //
 // One CTA per replica, sites in blocks of 32 (site order 0..L-1, A5).  Warps are
-// specialised: NTB = L/8 threads of BULK warps and four CHAIN warps (one per SM
-// sub-partition), coupled only through two pairs of shared-memory mbarriers, so
+// specialised: NTB = 4*(L/64) threads of BULK warps (8 warps at L=4096) and four
+// CHAIN warps (one per SM sub-partition), coupled only through two pairs of shared-memory mbarriers, so
 // that the bulk sum of block k+1 runs while block k is being decided.
 //
 // DRAW (all threads, once per sweep).  Proposals b_i, integer thresholds
@@ -16,8 +16,11 @@
 //   S_i = sum_j Jq[(i-j) mod L] * s'_i(c_j),   s'_i(k) = 1 + [k==a_i] - [k==b_i],
 // so that dE_i = S_i - sum_r Jq[r]  (Jq is symmetric, so (i-j) mod L indexes the
 // same coupling as |i-j|; Jq[0] = 0 drops j == i).  The 32 x L pair terms of a
-// block are split as 8 site groups (4 sites of equal parity) x L/64 ranges of
-// 64 consecutive j, one (group, range) per thread.  The range is taken RELATIVE
+// block are split as 4 site groups (the 8 sites of equal parity of a 16-site
+// half) x L/64 ranges of 64 consecutive j, one (group, range) per thread: a fat
+// tile (up to 168 registers, one CTA per SM; the MINB=2 build of the same code
+// fits 80 registers for persistent launches that need more CTAs per SM), so
+// that every unpacked word of colours serves 8 sites.  The range is taken RELATIVE
 // to the block start, so the couplings a thread needs never change: they live
 // in registers for the whole launch as 16-bit halves packed in pairs
 // (pt_kernels.cuh: pack_pairs_kernel).  Per 4 sites j the colour -> s' map is
@@ -28,8 +31,9 @@
 // main loop sums the low halves only (0.5 IDP.2A per pair term) and each thread
 // adds the high halves of NEARQ of the 56 quads of sites within distance 95 of
 // the block (NEAR); NEARQ = 0 keeps both halves everywhere (small L or sigma).
-// Block sums are reduced with shuffles and shared-memory atomics; every bulk
-// warp then arrives on full[k&1].  Before block k a bulk warp waits on
+// Block sums: a transpose-shuffle reduction leaves one site's partial sum per
+// lane, then one shared-memory atomic per lane; every bulk warp then arrives on
+// full[k&1].  Before block k a bulk warp waits on
 // done[k&1] (block k-2 decided), so it reads: blocks < k-1 final, block k-1 as
 // it was at the START of the sweep (sp0; it may still be changing), blocks >= k
 // untouched.
@@ -45,12 +49,14 @@
 // which the site-by-site order of Eq. 8 solves by forward
 // substitution.  Here it is solved by fixed-point rounds a <- F(a) starting
 // from "no correction": after t rounds the first t bits are exact, so at most
-// 32 rounds give exactly the sequential result; measured: 2.5 rounds per block
+// 32 rounds give exactly the sequential result; measured: 2.8 rounds per block
 // for the hottest replica of configs[3], 0-1 for cold ones.  A round is a masked
 // sum of 8 rows per warp (LOP3 -> predicate, SEL, IADD3: ALU pipe only, the FMA
 // pipe is saturated by BULK), an exchange of the four partial sums through
 // shared memory (named barrier 1) and a ballot.  Chain warp 0 writes the new
-// spins and arrives on done[k&1].  Integer arithmetic makes all of this
+// spins; after the block's closing named barrier (all chain warps have read the
+// block sums by then, also when the block needed no round) it clears the sums
+// for block k+2 and arrives on done[k&1].  Integer arithmetic makes all of this
 // independent of the order of summation (parity tests: bit-identical).
 //
 // OBSERVABLES, SWAPS.  Lane 0 of chain warp 0 owns the configuration's running
