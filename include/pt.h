@@ -59,7 +59,7 @@ typedef enum {
  *                     (PAPER.md:118-124), for blocks of 32 consecutive sites at a
  *                     time, with exact integer corrections for the changes
  *                     accepted inside the block.  Needs L % 64 == 0,
- *                     64 <= L <= 4096 and sum_r Jq[r] < 2^30 - 1.
+ *                     64 <= L <= 10240 (q > 8: L <= 9664, shared memory) and sum_r Jq[r] < 2^30 - 1.
  *  PT_VARIANT_AUTO  : DIRECT where it applies, else FIELD.
  * Environment: PT_VARIANT=direct|field|auto sets the variant chosen by pt_create; PT_PERSISTENT=0|1|2 the launch
  * policy of the direct variant (0: one launch per swap interval; 1, default: persistent launches with the swap events

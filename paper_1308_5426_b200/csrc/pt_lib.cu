@@ -97,7 +97,7 @@ void free_ctx(pt_ctx* c) {
 }
 
 int recompute_energy(pt_ctx* c, long long* d_out) {
-    if (ptk::direct_applies(c->L, c->q)) {   // IDP.2A version (pt_sweep_direct.cuh), ~10x faster at L = 4096
+    if (ptk::energy_direct_applies(c->L, c->q)) {   // IDP.2A version (pt_sweep_direct.cuh), ~10x faster at L = 4096
         int rc = ptk::launch_energy_direct(c->dev(), d_out, c->stream);
         if (rc) return fail(PT_ECUDA, std::string("energy_direct launch: ") + cudaGetErrorString((cudaError_t)rc));
         return PT_OK;
@@ -128,9 +128,8 @@ int resolve_variant(int L, int q, long long rowsum, int variant, int* out) {
     if (variant == PT_VARIANT_AUTO) variant = direct_ok ? PT_VARIANT_DIRECT : PT_VARIANT_FIELD;
     if (variant == PT_VARIANT_DIRECT) {
         if (!direct_ok)
-            return fail(PT_EINVAL, "direct variant needs L % 64 == 0, 64 <= L <= 4096 and sum_r Jq[r] < 2^30 - 1");
-        if (ptk::direct_smem_bytes(L, q) + 256 > kSmemLimit)
-            return fail(PT_ECAPACITY, "direct variant does not fit in shared memory for this L");
+            return fail(PT_EINVAL, "direct variant needs L % 64 == 0, 64 <= L <= 10240 (L <= 9664 for q > 8: shared memory) "
+                                   "and sum_r Jq[r] < 2^30 - 1");
     } else if (variant == PT_VARIANT_FIELD) {
         if (!field_fits(L, q)) return fail(PT_ECAPACITY, "local-field table (L*q*4 bytes) does not fit in shared memory");
     } else {
@@ -460,7 +459,7 @@ int pt_create_shard(pt_ctx** out, int L, int q, double sigma, int n_rep, const d
     if (rc) return rc;
     if (c->variant != PT_VARIANT_DIRECT) {
         pt_destroy(c);
-        return fail(PT_EINVAL, "slot-sharded contexts need the direct variant (L % 64 == 0, 64 <= L <= 4096)");
+        return fail(PT_EINVAL, "slot-sharded contexts need the direct variant (L % 64 == 0, 64 <= L <= 10240)");
     }
     c->rep_base = rep_base;
     c->n_local = n_local;

@@ -77,14 +77,25 @@ constexpr int DIRECT_SITES = 8;     // sites of a block per bulk thread (4 threa
 constexpr int DIRECT_MAX_BULK = 256;
 constexpr int DIRECT_CHAIN_WARPS = 4;                       // one per SM sub-partition
 constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 32 * DIRECT_CHAIN_WARPS;
+// L > 4096 (the paper's benchmark range reaches L = 10240): more j-ranges, hence more bulk threads, with
+// the 80-register build of the same code (768 threads x 80 registers fill the register file of an SM).
+constexpr int DIRECT_BIG_BULK = 640;
+constexpr int DIRECT_BIG_THREADS = DIRECT_BIG_BULK + 32 * DIRECT_CHAIN_WARPS;
+constexpr int DIRECT_STATIC_SMEM = 13 * 1024;   // upper bound of the sweep kernel's static shared memory (12544 B)
 constexpr int DIRECT_NPAIR = 39;   // packed coupling pairs per thread and half: 64 + 2*7 couplings
 constexpr int ENERGY_MAX_THREADS = 512, ENERGY_NPAIR = 35;   // energy_direct_kernel: 4 sites x 64 j per thread
 constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: the 224 sites (56 quads) around a block
 constexpr int DIRECT_NEAR_QUADS = 56;
 constexpr int DIRECT_MAX_PERSIST_REP = 512;   // replicas per ensemble in a persistent launch (static shared arrays)
 
+__host__ __device__ inline size_t direct_smem_bytes(int L, int q);
 __host__ __device__ inline bool direct_applies(int L, int q) {
-    return (L % 64) == 0 && L >= 64 && L <= 64 * (DIRECT_MAX_BULK / 4) && q <= 16;
+    return (L % 64) == 0 && L >= 64 && L <= 64 * (DIRECT_BIG_BULK / 4) && q <= 16 &&
+           direct_smem_bytes(L, q) + DIRECT_STATIC_SMEM <= 227 * 1024;
+}
+// energy_direct_kernel keeps one j-range per thread of a single CTA: L <= 4096 (beyond: the plain energy_kernel)
+__host__ __device__ inline bool energy_direct_applies(int L, int q) {
+    return direct_applies(L, q) && L <= 64 * (ENERGY_MAX_THREADS / 8);
 }
 __host__ __device__ inline int direct_bulk_threads(int L) {
     const int t = 4 * (L / 64);
@@ -317,9 +328,10 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 // only, plus the high halves of NEARQ of the 56 quads of sites within distance 95 of the block (requires
 // r_hi <= 95 and NEARQ * L/64 >= 56).  NJR64: L == 4096 (64 j-ranges as a compile-time constant).
 // MINB: minimum CTAs per SM the register allocation must allow (1: up to 168 registers, for large L; 2: 80 registers,
-// so that several hundred small replicas can be co-resident for persistent launches).
+// so that several hundred small replicas can be co-resident for persistent launches); 3 stands for the L > 4096
+// build: one CTA of up to DIRECT_BIG_THREADS threads per SM, 80 registers.
 template <int NEARQ, bool NJR64, bool Q16, int MINB>
-__global__ void __launch_bounds__(DIRECT_MAX_THREADS, MINB)
+__global__ void __launch_bounds__(MINB == 3 ? DIRECT_BIG_THREADS : DIRECT_MAX_THREADS, MINB == 3 ? 1 : MINB)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi) {
     // swap_mode 0: no swap event; 1: one event at the end of the launch (last-arriving CTA, nobody waits);
     // 2: persistent launch, an event inside the kernel after every sweep whose index is a multiple of swap_every;
@@ -860,6 +872,10 @@ typedef void (*direct_kernel_t)(Dev, long long, int, int, int, int);
 inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb) {
     const bool l4096 = d.L == 4096;
     const int nq = direct_nearq(d.L, r_hi);
+    if (d.L > 64 * (DIRECT_MAX_BULK / 4)) {   // more than 64 j-ranges: every near quad has a thread of its own
+        if (d.q <= 8) return nq == 1 ? sweep_direct_kernel<1, false, false, 3> : sweep_direct_kernel<0, false, false, 3>;
+        return nq == 1 ? sweep_direct_kernel<1, false, true, 3> : sweep_direct_kernel<0, false, true, 3>;
+    }
     if (d.q <= 8) {
         if (minb == 1) {
             switch (nq) {

@@ -282,6 +282,27 @@ def test_direct_variant_with_more_than_8_colours(pt, oracle, L, q, sigma):
         g.close()
 
 
+@pytest.mark.parametrize("L,q,sigma,policy", [(4160, 3, 0.5, "1"), (8192, 8, 0.3, "1"), (8192, 8, 0.3, "0"),
+                                              (10240, 5, 0.75, "2"), (9216, 12, 0.4, "1"), (6144, 4, 0.1, "1")])
+def test_direct_variant_beyond_4096_sites(pt, oracle, L, q, sigma, policy, monkeypatch):
+    """SURVEY.md 8(f) NEXT-2, the paper's benchmark range L <= 10240: more than 64 j-ranges per block
+    (up to 640 bulk threads, 80-register build), every launch policy, more than 8 colours, a ragged last bulk warp
+    (L = 4160: 65 j-ranges) and a sigma whose high coupling halves reach beyond the NEAR window (0.1)."""
+    monkeypatch.setenv("PT_PERSISTENT", policy)
+    n_rep = 5
+    b = inputs.geometric_betas(0.6, 2.5, n_rep)
+    g = pt.PT(L, q, sigma, 1, n_rep, b, 77, variant="auto")
+    assert g.get_variant() == "direct"
+    o = oracle.Oracle(L, q, sigma, 1, n_rep, b, 77)
+    np.testing.assert_array_equal(g.get_couplings(), oracle.couplings(L, sigma))
+    assert_same_state(g, o, "L=%d initial state" % L)
+    for n in (1, 9):
+        g.sweeps(n, 1)
+        o.sweeps(n, 1, field=True, threads=THREADS)
+        assert_same_state(g, o, "L=%d q=%d sigma=%g policy %s after +%d" % (L, q, sigma, policy, n))
+    g.close()
+
+
 @pytest.mark.parametrize("policy", ["0", "2"])
 def test_persistent_and_per_interval_launches_agree_with_the_oracle(pt, oracle, policy, monkeypatch):
     """PT_PERSISTENT=2 forces persistent launches (swap events inside the kernel, slots moving between resident CTAs)
