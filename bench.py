@@ -38,6 +38,14 @@ DRAM_BYTES_PER_SWEEP = 10.45e3
 N_SM = 148
 
 
+_JSON_OUT = sys.stdout   # main() points this at the process's original stdout
+
+
+def emit(line):
+    _JSON_OUT.write(json.dumps(line) + "\n")
+    _JSON_OUT.flush()
+
+
 def workload_config(w, variant, n_gpus):
     return {"workload": "configs[3]: L=%d q=%d sigma=%.1f, 1 ensemble x %d replicas per GPU, T geometric in "
                         "[%.1f,%.1f], hot start, swap every sweep" % (w.L, w.q, w.sigma, w.n_rep, w.T_lo, w.T_hi),
@@ -153,7 +161,7 @@ def run_reference(args):
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": use_threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
-    print(json.dumps(line))
+    emit(line)
     return 0
 
 
@@ -170,7 +178,10 @@ def run_ours(args):
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: libpt has no CPU path")
     torch.cuda.set_device(local_rank)
-    if world > 1:
+    # under torch.distributed.run (RANK set) the process group is always used, also for one rank, so that a
+    # single-GPU launch exercises the same barrier / max-over-ranks code as N > 1
+    use_dist = world > 1 or "RANK" in os.environ
+    if use_dist:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     w = inputs.config(3)
@@ -183,7 +194,7 @@ def run_ours(args):
     g.use_torch_stream(stream)
 
     def barrier():
-        if world > 1:
+        if use_dist:
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -202,7 +213,7 @@ def run_ours(args):
         barrier()
         clocks = sampler.result()
     ms = ev0.elapsed_time(ev1)
-    if world > 1:
+    if use_dist:
         ms = shard.max_over_ranks(ms, dist, device="cuda")
     attempts_per_gpu = K * w.n_rep * w.L
     value = world * attempts_per_gpu / (ms * 1e-3)
@@ -220,7 +231,7 @@ def run_ours(args):
     ob = g.observables()                     # D2H: n_rep*144 bytes
     barrier()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
+    if use_dist:
         e2e_s = shard.max_over_ranks(e2e_s, dist, device="cuda")
     assert spins.shape == start.shape and E.size == w.n_rep and ob["n_samples"].min() > 0
     e2e = {"value": world * attempts_per_gpu / e2e_s, "unit": UNIT,
@@ -252,9 +263,9 @@ def run_ours(args):
                 "flip_acceptance": acc, "pair_evaluations_per_s": value * (w.L - 1)}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline_leg(w)
-        print(json.dumps(line))
+        emit(line)
     g.close()
-    if world > 1:
+    if use_dist:
         dist.destroy_process_group()
     return 0
 
@@ -270,6 +281,12 @@ def main():
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
+    # stdout carries exactly one JSON line: libraries that write to file descriptor 1 on their own (NCCL prints its
+    # version banner there at communicator creation, compilers their progress) are sent to stderr instead
+    global _JSON_OUT
+    sys.stdout.flush()
+    _JSON_OUT = os.fdopen(os.dup(1), "w")
+    os.dup2(2, 1)
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
 
