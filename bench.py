@@ -3,12 +3,16 @@
 L=4096, q=8, sigma=0.3, 128 replicas (configs[3]), swap event every sweep.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--variant auto|direct|field]
+                  [--workload cfg3|paper:L]
 
 One STEP = one sweep of every replica (L Metropolis steps each, Eq. 8) + the per-slot observables +
 one replica-exchange event (Eq. 9) = n_rep*L attempts, i.e. one pass of the whole hot path.  The
 default K = 2000 is the full configs[3] run.  Prints ONE JSON line (rank 0).  For N > 1 (torchrun)
 every rank runs its own ensemble of configs[3] (ens_base = rank: independent random streams, no
 data-path collective), so scaling is "weak" and `value` is the sum over ranks / max time.
+`--workload paper:L` (not the headline) times the same path on the shape of the paper's own
+benchmark runs instead: q=3, 400 replicas on a uniform ladder, L in 512..10240 (PAPER.md:136, :202;
+inputs.paper_benchmark), and says so in `metric` and `config.workload`.
 """
 import argparse
 import json
@@ -46,9 +50,26 @@ def emit(line):
     _JSON_OUT.flush()
 
 
+def pick_workload(args):
+    if args.workload in ("cfg3", "configs[3]"):
+        return inputs.config(3)
+    if args.workload.startswith("paper:"):
+        return inputs.paper_benchmark(int(args.workload.split(":", 1)[1]))
+    raise SystemExit("bench.py: --workload must be cfg3 or paper:L")
+
+
+def label(w):
+    return "configs[3]" if w.name == "cfg3" else "the paper's benchmark shape (PAPER.md:136,202; not BASELINE's config)"
+
+
+def metric_name(w):
+    return METRIC if w.name == "cfg3" else "Metropolis spin-flip attempts/s at L=%d q=%d %d replicas" % (w.L, w.q, w.n_rep)
+
+
 def workload_config(w, variant, n_gpus):
-    return {"workload": "configs[3]: L=%d q=%d sigma=%.1f, 1 ensemble x %d replicas per GPU, T geometric in "
-                        "[%.1f,%.1f], hot start, swap every sweep" % (w.L, w.q, w.sigma, w.n_rep, w.T_lo, w.T_hi),
+    return {"workload": "%s: L=%d q=%d sigma=%.1f, 1 ensemble x %d replicas per GPU, T %s in "
+                        "[%.1f,%.1f], hot start, swap every sweep"
+                        % (label(w), w.L, w.q, w.sigma, w.n_rep, w.ladder, w.T_lo, w.T_hi),
             "step": "1 sweep of all replicas + observables + 1 swap event = %d attempts per GPU" % (w.L * w.n_rep),
             "variant": variant, "parallelism": "ensembles sharded over %d GPU(s), no collective" % n_gpus,
             "l2": "not flushed: per-step state is %d KB of packed spins per GPU, resident in shared memory/L2 by "
@@ -117,8 +138,8 @@ def cpu_baseline_leg(w, budget_s=12.0):
         n += 1
     o.close()
     return {"value": n * w.n_rep * w.L / t, "unit": UNIT, "cores": min(threads, w.n_rep), "kind": "oracle",
-            "sample": "%d sweep(s) (+swap events) of the full configs[3] ensemble (128 replicas), direct-sum mode, "
-                      "%d std::threads, g++ -O2, %.1f s" % (n, min(threads, w.n_rep), t)}
+            "sample": "%d sweep(s) (+swap events) of the full %s ensemble (%d replicas), direct-sum mode, "
+                      "%d std::threads, g++ -O2, %.1f s" % (n, label(w), w.n_rep, min(threads, w.n_rep), t)}
 
 
 def run_reference(args):
@@ -129,7 +150,7 @@ def run_reference(args):
         return 0
     from oracle import pt_oracle
     pt_oracle.build()
-    w = inputs.config(3)
+    w = pick_workload(args)
     threads = oracle_threads()
     betas = inputs.betas(w)
     # calibrate on one replica, then size the sample so that (K+W) steps take <= ~150 s
@@ -152,9 +173,9 @@ def run_reference(args):
     dt = time.perf_counter() - t0
     o.close()
     value = args.steps * r * w.L / dt
-    sample = ("each step = 1 sweep + swap event of %d of the 128 slots of configs[3] (evenly spaced in the ladder), "
-              "direct-sum mode, %d std::threads" % (r, use_threads))
-    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+    sample = ("each step = 1 sweep + swap event of %d of the %d slots of %s (evenly spaced in the ladder), "
+              "direct-sum mode, %d std::threads" % (r, w.n_rep, label(w), use_threads))
+    line = {"impl": "reference", "metric": metric_name(w), "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32",
             "data": "synthetic", "config": workload_config(w, "oracle", args.gpus),
@@ -184,7 +205,7 @@ def run_ours(args):
     if use_dist:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    w = inputs.config(3)
+    w = pick_workload(args)
     betas = inputs.betas(w)
     K, W_ = args.steps, args.warmup
     ens_base, n_ens_local = shard.ensemble_shard(world, world, rank)   # one configs[3] ensemble per GPU
@@ -247,16 +268,17 @@ def run_ours(args):
         dram_per_launch = DRAM_BYTES_PER_SWEEP * K / max(1, launches)
         peak = N_SM * IDP_LANES_PER_CLK_PER_SM * MACS_PER_IDP_LANE * f_hz / 1e12
         roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tmac/s", "frac": achieved / peak,
-                    "traffic": dram_per_launch if variant == "direct" else None,
+                    "traffic": dram_per_launch if variant == "direct" and w.name == "cfg3" else None,
                     "kernel": "sweep_%s_kernel" % variant,
                     "note": "algorithmic work = sweeps*n_rep*L^2 = %.3e integer multiply-accumulates per launch (one per "
                             "pair term; %d sweeps per launch); peak = 148 SMs x 64 IDP.2A lanes/clk/SM (measured issue rate) x 2 MAC x "
                             "sampled SM clock %.0f MHz -- a derived ALU peak, not MEASURED_PEAKS.json (its HBM and "
-                            "tensor figures do not bound this path: %.0f KB of DRAM traffic per launch = %.2f GB/s "
-                            "of the measured %.0f GB/s); 128 of 148 SMs carry a replica"
-                            % (macs_per_launch, K // max(1, launches), f_hz / 1e6, dram_per_launch / 1e3,
-                               dram_per_launch / launch_s / 1e9, measured_hbm_gbs())}
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
+                            "tensor figures do not bound this path%s)"
+                            % (macs_per_launch, K // max(1, launches), f_hz / 1e6,
+                               ": %.0f KB of DRAM traffic per launch = %.2f GB/s of the measured %.0f GB/s; 128 of 148 "
+                               "SMs carry a replica" % (dram_per_launch / 1e3, dram_per_launch / launch_s / 1e9,
+                                                        measured_hbm_gbs()) if w.name == "cfg3" else "")}
+        line = {"metric": metric_name(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "int32", "data": "synthetic", "config": workload_config(w, variant, world),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
@@ -278,6 +300,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variant", default="auto", choices=["auto", "direct", "field"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workload", default="cfg3", help="cfg3 (BASELINE.json's headline config, default) or paper:L")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

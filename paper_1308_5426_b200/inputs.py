@@ -30,6 +30,7 @@ class Workload:
     burn_in: int = 0
     cold_half: bool = False      # cfg2: slots t < n_rep/2 (the colder half) start all-1
     seed: int = SEED_BASE
+    ladder: str = "geometric"    # "uniform": T_t equally spaced (the paper's ladder)
 
     @property
     def attempts(self) -> int:
@@ -43,6 +44,26 @@ def geometric_betas(T_lo: float, T_hi: float, n_rep: int) -> np.ndarray:
     t = np.arange(n_rep, dtype=np.float64) / float(n_rep - 1)
     T = T_lo * np.power(T_hi / T_lo, t)
     return np.ascontiguousarray(1.0 / T, dtype=np.float64)
+
+
+def uniform_betas(T_lo: float, T_hi: float, n_rep: int) -> np.ndarray:
+    """beta_t = 1/T_t, T_t equally spaced in [T_lo, T_hi], slot 0 = coldest ("a uniform distribution of the
+    temperatures", PAPER.md:136)."""
+    return np.ascontiguousarray(1.0 / np.linspace(T_lo, T_hi, n_rep, dtype=np.float64), dtype=np.float64)
+
+
+PAPER_BENCH_SIZES = (512, 1024, 2048, 3072, 4096, 6144, 8192, 10240)
+
+
+def paper_benchmark(L: int) -> Workload:
+    """The shape of the paper's own runs: q = 3, 400 replicas on a uniform temperature
+    ladder, lattice sizes 512..10240, swap event every sweep.  sigma = 0.5 (mid-range
+    of the paper's [0.2, 0.8]) and T in [0.5, 3.0] (brackets the Table 1 critical temperatures) are this build's
+    choices: the paper does not print the ladder's end points.  Synthetic parameters only; no dataset is involved."""
+    if L < 8 or L > 10240:
+        raise ValueError("paper_benchmark: L must be in 8..10240")
+    return Workload("paper[L=%d]" % L, L, 3, 0.5, 1, 400, 0.5, 3.0, 1000, ladder="uniform",
+                    seed=SEED_BASE + 0x500 + L)
 
 
 def config(k: int) -> Workload:
@@ -69,6 +90,8 @@ def config4() -> List[Workload]:
 
 
 def betas(w: Workload) -> np.ndarray:
+    if w.ladder == "uniform":
+        return uniform_betas(w.T_lo, w.T_hi, w.n_rep)
     return geometric_betas(w.T_lo, w.T_hi, w.n_rep)
 
 

@@ -74,3 +74,17 @@ def test_input_recipes():
     assert b.shape == (128,) and np.isclose(1 / b[0], 0.6) and np.isclose(1 / b[-1], 2.5)
     assert np.all(np.diff(b) < 0)
     assert len(inputs.config4()) == 40 and len({c.seed for c in inputs.config4()}) == 40
+
+
+def test_paper_benchmark_recipe():
+    """The paper's own run shape: q=3, 400 replicas, temperatures equally spaced."""
+    from paper_1308_5426_b200 import inputs
+    for L in inputs.PAPER_BENCH_SIZES:
+        w = inputs.paper_benchmark(L)
+        assert (w.L, w.q, w.n_rep, w.n_ens, w.swap_every, w.ladder) == (L, 3, 400, 1, 1, "uniform")
+        T = 1.0 / inputs.betas(w)
+        assert T.shape == (400,) and np.isclose(T[0], w.T_lo) and np.isclose(T[-1], w.T_hi)
+        assert np.allclose(np.diff(T), (w.T_hi - w.T_lo) / 399, rtol=1e-9)
+    assert len({inputs.paper_benchmark(L).seed for L in inputs.PAPER_BENCH_SIZES}) == len(inputs.PAPER_BENCH_SIZES)
+    with pytest.raises(ValueError):
+        inputs.paper_benchmark(20480)

@@ -428,3 +428,18 @@ def test_binder_crossing_reproduces_the_papers_critical_temperature(pt):
     assert crossings, "the cumulants of L=256 and L=512 do not cross"
     best = min(crossings, key=lambda x: abs(x - 2.085))
     assert abs(best - 2.085) < 0.01, crossings
+
+
+@pytest.mark.parametrize("L,sweeps", [(512, 12), (1024, 6), (2048, 3)])
+def test_paper_benchmark_shape(pt, oracle, L, sweeps):
+    """`bench.py --workload paper:L`: the paper's own run shape, q=3 and 400 replicas on a
+    uniform ladder, in the launch configuration the bench times (default policy: one persistent
+    launch while 400 CTAs are co-resident, i.e. L <= 1024, ordinary launches with several waves of CTAs beyond)."""
+    w = inputs.paper_benchmark(L)
+    g, o = make_pair(pt, oracle, w, "direct")
+    for n in (1, sweeps):
+        g.sweeps(n, w.swap_every)
+        o.sweeps(n, w.swap_every, field=True, threads=THREADS)
+        assert_same_state(g, o, "%s after %d more sweeps" % (w.name, n))
+    g.close()
+    o.close()
