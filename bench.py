@@ -3,7 +3,7 @@
 L=4096, q=8, sigma=0.3, 128 replicas (configs[3]), swap event every sweep.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--variant auto|direct|field]
-                  [--workload cfg3|paper:L]
+                  [--workload cfg3|paper:L[:R]]
 
 One STEP = one sweep of every replica (L Metropolis steps each, Eq. 8) + the per-slot observables +
 one replica-exchange event (Eq. 9) = n_rep*L attempts, i.e. one pass of the whole hot path.  The
@@ -12,7 +12,8 @@ every rank runs its own ensemble of configs[3] (ens_base = rank: independent ran
 data-path collective), so scaling is "weak" and `value` is the sum over ranks / max time.
 `--workload paper:L` (not the headline) times the same path on the shape of the paper's own
 benchmark runs instead: q=3, 400 replicas on a uniform ladder, L in 512..10240 (PAPER.md:136, :202;
-inputs.paper_benchmark), and says so in `metric` and `config.workload`.
+inputs.paper_benchmark; `paper:L:R` takes R replicas instead of 400, the replica-count scan of Fig. 5, :224), and says
+so in `metric` and `config.workload`.
 """
 import argparse
 import json
@@ -54,8 +55,9 @@ def pick_workload(args):
     if args.workload in ("cfg3", "configs[3]"):
         return inputs.config(3)
     if args.workload.startswith("paper:"):
-        return inputs.paper_benchmark(int(args.workload.split(":", 1)[1]))
-    raise SystemExit("bench.py: --workload must be cfg3 or paper:L")
+        parts = args.workload.split(":")
+        return inputs.paper_benchmark(int(parts[1]), int(parts[2]) if len(parts) > 2 else 400)
+    raise SystemExit("bench.py: --workload must be cfg3, paper:L or paper:L:R")
 
 
 def label(w):
@@ -300,7 +302,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variant", default="auto", choices=["auto", "direct", "field"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="cfg3", help="cfg3 (BASELINE.json's headline config, default) or paper:L")
+    ap.add_argument("--workload", default="cfg3", help="cfg3 (BASELINE.json's headline config, default), paper:L or paper:L:R")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3

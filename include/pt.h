@@ -63,7 +63,8 @@ typedef enum {
  *  PT_VARIANT_AUTO  : DIRECT where it applies, else FIELD.
  * Environment: PT_VARIANT=direct|field|auto sets the variant chosen by pt_create; PT_PERSISTENT=0|1|2 the launch
  * policy of the direct variant (0: one launch per swap interval; 1, default: persistent launches with the swap events
- * inside the kernel for contexts that take at least a third of the SMs; 2: whenever all replicas can be co-resident). */
+ * inside the kernel for contexts that take at least a third of the SMs; 2: whenever all replicas can be co-resident);
+ * PT_MINB=1|2 forces the 168- or the 80-register build of the direct sweep kernel (experiments; default: by size). */
 enum { PT_VARIANT_AUTO = 0, PT_VARIANT_FIELD = 1, PT_VARIANT_DIRECT = 2 };
 
 /* Cumulative per-slot accumulators since pt_create (the caller differences two

@@ -910,15 +910,23 @@ inline int direct_coresident(direct_kernel_t kern, const Dev& d, int device) {
 }
 
 // The kernel a context uses, and how many of its CTAs fit on the device at once (a persistent launch, swap_mode 2,
-// needs all n_ens * n_rep of them).  The 168-register variant unless only the 80-register one (L < 2048) makes all
-// replicas co-resident.
+// needs all n_ens * n_rep of them).  The 168-register build while all replicas fit in one wave of it; with more
+// replicas than that and L < 2048 the 80-register build, which puts more CTAs on an SM (co-resident or not: where they are
+// not, measured 5-13 % faster at L = 256..1536 with 600..1200 replicas, equal at L = 1024 with 740 and 2.5 % slower
+// with 1200, profiles/r1_g_paper_shapes.md).  From L = 2048
+// on the 80-register build is slower in every case measured (0.250 against 0.194 ms per sweep at L = 2048 with 400
+// replicas although it makes them co-resident; a factor 2 at L = 4096), so it is never picked there.
+// PT_MINB=1|2 (experiments) forces the 168- or, for L <= 4096, the 80-register build.
 inline direct_kernel_t select_direct_kernel(const Dev& d, int r_hi, int device, int* coresident) {
     direct_kernel_t k1 = direct_kernel_variant(d, r_hi, 1);
     int c1 = direct_coresident(k1, d, device);
-    if (d.n_ens * d.n_rep > c1 && d.L < 2048) {
+    const char* env = getenv("PT_MINB");
+    const bool force1 = env && env[0] == '1';
+    const bool force2 = env && env[0] == '2' && d.L <= 64 * (DIRECT_MAX_BULK / 4);
+    if (force2 || (d.n_ens * d.n_rep > c1 && d.L < 2048 && !force1)) {
         direct_kernel_t k2 = direct_kernel_variant(d, r_hi, 2);
         const int c2 = direct_coresident(k2, d, device);
-        if (d.n_ens * d.n_rep <= c2) { k1 = k2; c1 = c2; }
+        if (force2 || c2 > c1) { k1 = k2; c1 = c2; }
     }
     if (coresident) *coresident = c1;
     return k1;

@@ -55,14 +55,17 @@ def uniform_betas(T_lo: float, T_hi: float, n_rep: int) -> np.ndarray:
 PAPER_BENCH_SIZES = (512, 1024, 2048, 3072, 4096, 6144, 8192, 10240)
 
 
-def paper_benchmark(L: int) -> Workload:
+def paper_benchmark(L: int, n_rep: int = 400) -> Workload:
     """The shape of the paper's own runs: q = 3, 400 replicas on a uniform temperature
     ladder, lattice sizes 512..10240, swap event every sweep.  sigma = 0.5 (mid-range
     of the paper's [0.2, 0.8]) and T in [0.5, 3.0] (brackets the Table 1 critical temperatures) are this build's
-    choices: the paper does not print the ladder's end points.  Synthetic parameters only; no dataset is involved."""
+    choices: the paper does not print the ladder's end points.  Synthetic parameters only; no dataset is involved.
+    n_rep other than 400 gives the points of the replica-count scan (Fig. 5) on the same ladder range."""
     if L < 8 or L > 10240:
         raise ValueError("paper_benchmark: L must be in 8..10240")
-    return Workload("paper[L=%d]" % L, L, 3, 0.5, 1, 400, 0.5, 3.0, 1000, ladder="uniform",
+    if n_rep < 2 or n_rep > 4096:
+        raise ValueError("paper_benchmark: n_rep must be in 2..4096")
+    return Workload("paper[L=%d,R=%d]" % (L, n_rep), L, 3, 0.5, 1, n_rep, 0.5, 3.0, 1000, ladder="uniform",
                     seed=SEED_BASE + 0x500 + L)
 
 

@@ -443,3 +443,18 @@ def test_paper_benchmark_shape(pt, oracle, L, sweeps):
         assert_same_state(g, o, "%s after %d more sweeps" % (w.name, n))
     g.close()
     o.close()
+
+
+@pytest.mark.parametrize("L,n_rep", [(512, 740), (256, 1200)])
+def test_more_replicas_than_one_wave_of_the_small_build(pt, oracle, L, n_rep):
+    """Replica counts beyond what even the 80-register build holds at once (L=512: 3 CTAs per SM = 444) or beyond the
+    persistent-launch limit of 512 replicas: ordinary launches of the 80-register build in several waves, swap event
+    by the last CTA to arrive (select_direct_kernel; the Fig. 5 scan of profiles/r1_g_paper_shapes.md)."""
+    w = inputs.paper_benchmark(L, n_rep)
+    g, o = make_pair(pt, oracle, w, "direct")
+    for n in (1, 5):
+        g.sweeps(n, w.swap_every)
+        o.sweeps(n, w.swap_every, field=True, threads=THREADS)
+        assert_same_state(g, o, "%s after %d more sweeps" % (w.name, n))
+    g.close()
+    o.close()
