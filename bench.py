@@ -87,6 +87,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, index):
         super().__init__(daemon=True)
         self.index, self.stop_flag, self.sm, self.mask, self.max_mhz, self.err = index, False, [], 0, None, None
+        self.ready, self.first = threading.Event(), 0
 
     def run(self):
         try:
@@ -94,19 +95,31 @@ class ClockSampler(threading.Thread):
             pynvml.nvmlInit()
             h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
             self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM)
-            while not self.stop_flag:
+            self.ready.set()
+            while True:   # at least one sample, also for a timed region shorter than the sampling period
                 self.sm.append(pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM))
                 self.mask |= int(pynvml.nvmlDeviceGetCurrentClocksThrottleReasons(h))
-                time.sleep(0.02)
+                if self.stop_flag:
+                    break
+                time.sleep(0.01)
         except Exception as ex:  # NVML missing: report, do not fake
             self.err = repr(ex)
+        self.ready.set()
+
+    def start_sampling(self):
+        """Starts the thread and returns once NVML is initialised, so that the timed region is not over before the
+        first sample (nvmlInit takes tens of milliseconds)."""
+        self.start()
+        self.ready.wait(timeout=5.0)
+        self.first = len(self.sm)   # samples from here on lie in the timed region (or just after its end)
 
     def result(self):
         self.stop_flag = True
         self.join(timeout=2.0)
         if not self.sm:
             return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "error": self.err}
-        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.max_mhz, "samples": len(self.sm),
+        sm = self.sm[self.first:] or self.sm[-1:]
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": self.max_mhz, "samples": len(sm),
                 "reasons": [n for b, n in self.REASONS.items() if self.mask & b]}
 
 
@@ -227,7 +240,7 @@ def run_ours(args):
         g.sync()
         barrier()
         sampler = ClockSampler(local_rank)
-        sampler.start()
+        sampler.start_sampling()
         ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         ev0.record(stream)
         launches = g.sweeps_async(K, w.swap_every)
