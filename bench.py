@@ -3,7 +3,7 @@
 L=4096, q=8, sigma=0.3, 128 replicas (configs[3]), swap event every sweep.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--variant auto|direct|field]
-                  [--workload cfg3|paper:L[:R]]
+                  [--workload cfg3|cfg4|paper:L[:R]]
 
 One STEP = one sweep of every replica (L Metropolis steps each, Eq. 8) + the per-slot observables +
 one replica-exchange event (Eq. 9) = n_rep*L attempts, i.e. one pass of the whole hot path.  The
@@ -307,6 +307,95 @@ def run_ours(args):
     return 0
 
 
+def run_cfg4(args):
+    """--workload cfg4 (BASELINE.json configs[4], not the headline): the sigma-q scan, 40 independent handles of 32
+    replicas (L=2048, q in {3,5,7,9} x sigma in {0.1..1.0}), one CUDA stream per handle, swap event every sweep.
+    One step = one sweep + swap event of all 1280 replicas.  Single GPU only."""
+    import torch
+    from paper_1308_5426_b200 import build as ptbuild
+    ptbuild.build()
+    from paper_1308_5426_b200 import pt
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libpt has no CPU path")
+    if int(os.environ.get("WORLD_SIZE", "1")) != 1:
+        raise SystemExit("bench.py: --workload cfg4 is a single-GPU workload")
+    ws = inputs.config4()
+    K, W_ = args.steps, args.warmup
+    streams = [torch.cuda.Stream() for _ in ws]
+    gs = []
+    for w, st in zip(ws, streams):
+        g = pt.PT(w.L, w.q, w.sigma, 1, w.n_rep, inputs.betas(w), w.seed, variant=args.variant)
+        g.use_torch_stream(st)
+        gs.append(g)
+    main_s = torch.cuda.current_stream()
+
+    def steps(n):
+        launches = 0
+        for _ in range(n):           # interleaved, so that all 40 streams hold work from the start
+            for g in gs:
+                launches += g.sweeps_async(1, 1)
+        return launches
+
+    steps(W_)
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start_sampling()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(main_s)
+    for st in streams:
+        st.wait_event(ev0)
+    launches = steps(K)
+    for st in streams:
+        main_s.wait_stream(st)
+    ev1.record(main_s)
+    torch.cuda.synchronize()
+    clocks = sampler.result()
+    ms = ev0.elapsed_time(ev1)
+    attempts = K * sum(w.n_rep * w.L for w in ws)
+    value = attempts / (ms * 1e-3)
+
+    starts = [g.get_spins() for g in gs]
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for g, s0 in zip(gs, starts):
+        g.set_spins(s0)
+    steps(K)
+    d2h = 0
+    for g, w in zip(gs, ws):
+        sp, E, ob = g.get_spins(), g.energy(), g.observables()
+        d2h += sp.nbytes + E.nbytes + w.n_rep * 144
+        assert ob["n_samples"].min() > 0
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    f_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
+    macs = K * sum(w.n_rep * w.L * w.L for w in ws)
+    achieved = macs / (ms * 1e-3) / 1e12
+    peak = N_SM * IDP_LANES_PER_CLK_PER_SM * MACS_PER_IDP_LANE * f_hz / 1e12
+    line = {"metric": "Metropolis spin-flip attempts/s on the sigma-q scan (40 ensembles x 32 replicas, L=2048)",
+            "value": value, "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W_, "ms_per_step": ms / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": "configs[4] (not the headline config): L=2048, q in {3,5,7,9} x sigma in {0.1..1.0} = "
+                                   "40 handles x 32 replicas, T geometric in [0.4,3.0], hot start, swap every sweep, "
+                                   "40 CUDA streams", "variant": gs[0].get_variant(),
+                       "step": "1 sweep + swap event of all 1280 replicas = %d attempts" % (attempts // K),
+                       "l2": "not flushed: the per-step state (1.3 MB of packed spins) is resident by design"},
+            "clocks": clocks,
+            "e2e": {"value": attempts / e2e_s, "unit": UNIT, "h2d_bytes_per_step": sum(s0.nbytes for s0 in starts) / K,
+                    "d2h_bytes_per_step": d2h / K,
+                    "what": "per handle pt_set_spins(host) + K x pt_sweeps_async(1) + pt_get_spins + pt_energy + "
+                            "pt_observables (host buffers), wall clock"},
+            "gpu_launches": int(launches),
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tmac/s", "frac": achieved / peak,
+                         "traffic": None, "kernel": "sweep_%s_kernel" % gs[0].get_variant(),
+                         "note": "algorithmic work = sum over handles of sweeps*n_rep*L^2 multiply-accumulates over the "
+                                 "whole timed region (40 streams run concurrently, so per-launch durations overlap); "
+                                 "peak as for the headline config"}}
+    emit(line)
+    for g in gs:
+        g.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -315,7 +404,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variant", default="auto", choices=["auto", "direct", "field"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--workload", default="cfg3", help="cfg3 (BASELINE.json's headline config, default), paper:L or paper:L:R")
+    ap.add_argument("--workload", default="cfg3", help="cfg3 (BASELINE.json's headline config, default), cfg4, paper:L or paper:L:R")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -325,6 +414,10 @@ def main():
     sys.stdout.flush()
     _JSON_OUT = os.fdopen(os.dup(1), "w")
     os.dup2(2, 1)
+    if args.workload == "cfg4":
+        if args.impl == "reference":
+            raise SystemExit("bench.py: --impl reference times the headline config or a paper:L shape")
+        return run_cfg4(args)
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
 
