@@ -193,6 +193,17 @@ int pt_sweeps_async(pt_ctx* ctx, int64_t n, int swap_every, int64_t* n_launches)
 /* Blocks until the context's stream is idle; returns PT_ECUDA if a kernel failed. */
 int pt_sync(pt_ctx* ctx);
 
+/* Instruction-rate micro-benchmarks on the current device (the ALU roofline of the direct sweep kernel
+ * rests on the measured issue rate of IDP.2A, not on a datasheet).  rates[p*4 + (w-1)] = lane-operations per clock
+ * and SM of pattern p with w = 1..4 warps per SM sub-partition, timed with clock64() inside the kernel (median over
+ * the SMs).  Patterns: 0 IDP.2A, 1 IDP.4A, 2 IMAD, 3 PRMT, 4 LOP3, 5 the bulk loop's mix of 1 PRMT + 2 IDP.2A
+ * (counting the IDP.2A only), 6 1 LOP3 + 2 IDP.2A (ditto), 7 LDS.128 in bytes per clock and SM, 8 1 PRMT + 4 IDP.2A,
+ * 9 the mirror-paired mix 2 PRMT + 1 ADD + 2 IDP.2A (IDP.2A counted; 4 pair terms per IDP.2A lane-operation).
+ * One IDP.2A lane-operation is two multiply-accumulates (one per pair term of the energy sum).
+ * n = number of doubles `rates` holds, >= 4 * PT_PEAK_PATTERNS.  Errors: PT_EINVAL, PT_ENOMEM, PT_ECUDA. */
+#define PT_PEAK_PATTERNS 10
+int pt_measure_peaks(double* rates, int n);
+
 const char* pt_last_error(void);
 
 #ifdef __cplusplus

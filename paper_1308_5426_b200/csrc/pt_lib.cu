@@ -12,11 +12,13 @@
 #include <new>
 #include <string>
 #include <vector>
+#include <algorithm>
 
 #include "pt.h"
 #include "pt_kernels.cuh"
 #include "pt_sweep_direct.cuh"
 #include "pt_sweep_field.cuh"
+#include "pt_peaks.cuh"
 
 namespace {
 
@@ -328,8 +330,9 @@ int pt_sweeps_async(pt_ctx* c, int64_t n, int swap_every, int64_t* n_launches) {
         return fail(PT_EINVAL, "slot-sharded context: call pt_sweeps with swap_every = 0 and pt_swap_external");
     int64_t launches = 0;
     constexpr int64_t kMaxChunk = 1 << 16;  // sweeps per launch
-    // a persistent launch pays a counter reset and a cooperative launch: worth it from a handful of sweeps per call
-    const bool persistent = swap_every > 0 && (n >= 8 || c->persistent_policy == 2) && persistent_ok(c);
+    // a persistent launch pays a counter reset and a cooperative launch: taken for every call of two or more sweeps
+    // (single-sweep calls are what interleaved multi-handle drivers issue; they stay ordinary launches)
+    const bool persistent = swap_every > 0 && (n >= 2 || c->persistent_policy == 2) && persistent_ok(c);
     while (n > 0) {
         int64_t chunk = n < kMaxChunk ? n : kMaxChunk;
         int swap_mode = c->n_local ? 3 : 0;
@@ -502,6 +505,37 @@ int pt_debug_timing(pt_ctx* c, long long* out) {
     return PT_OK;
 }
 #endif
+
+int pt_measure_peaks(double* rates, int n) {
+    if (!rates || n < PT_PEAK_PATTERNS * 4) return fail(PT_EINVAL, "rates must hold PT_PEAK_PATTERNS * 4 doubles");
+    int dev = 0, n_sm = 0;
+    PT_CUDA(cudaGetDevice(&dev));
+    PT_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    long long* d_clk = nullptr;
+    uint32_t* d_sink = nullptr;
+    PT_CUDA(cudaMalloc(&d_clk, (size_t)n_sm * sizeof(long long)));
+    cudaError_t err = cudaMalloc(&d_sink, sizeof(uint32_t));
+    if (err != cudaSuccess) { cudaFree(d_clk); return fail(PT_ENOMEM, cudaGetErrorString(err)); }
+    std::vector<long long> clk(n_sm);
+    int rc = PT_OK;
+    for (int p = 0; p < PT_PEAK_PATTERNS && rc == PT_OK; ++p) {
+        ptk::peak_kernel_t k = ptk::peak_kernel_of(p);
+        for (int w = 1; w <= 4 && rc == PT_OK; ++w) {
+            const int threads = 128 * w;   // w warps on each of the 4 sub-partitions
+            for (int rep = 0; rep < 2; ++rep) k<<<n_sm, threads>>>(d_clk, d_sink, 12345u + rep);   // first run warms up
+            err = cudaMemcpy(clk.data(), d_clk, (size_t)n_sm * sizeof(long long), cudaMemcpyDeviceToHost);
+            if (err != cudaSuccess) { rc = fail(PT_ECUDA, cudaGetErrorString(err)); break; }
+            std::sort(clk.begin(), clk.end());
+            const double med = (double)clk[n_sm / 2];
+            // lane-operations (bytes for the LDS pattern) per clock and SM
+            const double per_thread = ptk::peak_counted_ops(p);
+            rates[p * 4 + (w - 1)] = p == ptk::PEAK_LDS128 ? per_thread * threads / med : per_thread * threads / med;
+        }
+    }
+    cudaFree(d_clk);
+    cudaFree(d_sink);
+    return rc;
+}
 
 int pt_set_variant(pt_ctx* c, int variant) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");

@@ -113,9 +113,9 @@ __host__ __device__ inline int direct_nearq(int L, int r_hi) {
     if (r_hi > DIRECT_NEAR_R || L < 256 || nq > 4) return 0;
     return nq == 3 ? 4 : nq;
 }
-// dynamic smem (32-bit words): theta[L] | lut[2L] | lutb[2L] (q > 8 only) | sp[W] | sp0[W] | bq[W] | selb[L/4] | part[64] | Jz[96]
+// dynamic smem (32-bit words): theta[L] | lut[2L] | lutb[2L] (q > 8 only) | sp[W] | sp0[W] | bq[W] | part[64] | Jz[96]
 __host__ __device__ inline size_t direct_smem_bytes(int L, int q) {
-    return (size_t)((q > 8 ? 5 : 3) * L + 3 * (L / 8) + L / 4 + 64 + 96) * 4;
+    return (size_t)((q > 8 ? 5 : 3) * L + 3 * (L / 8) + 64 + 96) * 4;
 }
 
 __device__ __forceinline__ int dp4a_s32_u32(int a, uint32_t b, int c) {
@@ -161,7 +161,6 @@ struct DirectSmem {
     uint32_t* sp;     // [W]  live packed spins
     uint32_t* sp0;    // [W]  spins at the start of the running sweep
     uint32_t* bq;     // [W]  proposed colours
-    uint8_t* selb;    // [L]  a0 | b << 4: colour at the start of the sweep and proposed colour
     uint32_t* part;   // [2][32] block sums S_i, double buffered
     int32_t* Jz;      // [96] Jz[n] = 0 for n < 32, Jq[n - 32] above
 };
@@ -176,7 +175,7 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
     for (int hw = threadIdx.x; hw < 2 * W; hw += blockDim.x) {
         const int w = hw >> 1, h4 = (hw & 1) << 2;
         const uint32_t word = m.sp[w];
-        uint32_t bhalf = 0, s4 = 0;
+        uint32_t bhalf = 0;
 #pragma unroll
         for (int n = 0; n < 4; ++n) {
             const int i = 8 * w + h4 + n;
@@ -185,7 +184,6 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
             const uint32_t k = __umulhi(p.w0, (uint32_t)(q - 1));
             const uint32_t b = k + (k >= a ? 1u : 0u);
             bhalf |= b << (4 * n);
-            s4 |= (a | (b << 4)) << (8 * n);
             m.theta[i] = min(accept_threshold(uniform53(p.w1, p.w2), scale), 1 << 30);  // |dE| < 2^30: same decisions
             unsigned long long ta = 0x0101010101010101ull, tb = ta;   // byte k = s'(k), k = 0..7 | 8..15
             if (!Q16 || a < 8u) ta += 1ull << (8 * a); else tb += 1ull << (8 * (a - 8u));
@@ -194,7 +192,6 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
             if (Q16) m.lutb[i] = make_uint2((uint32_t)tb, (uint32_t)(tb >> 32));
         }
         reinterpret_cast<uint16_t*>(m.bq)[hw] = (uint16_t)bhalf;   // low half of word w = sites 8w .. 8w+3
-        reinterpret_cast<uint32_t*>(m.selb)[hw] = s4;
         if (h4 == 0) m.sp0[w] = word;
     }
 }
@@ -303,6 +300,23 @@ __device__ __forceinline__ int masked_add4(int acc, unsigned m, int b, int4 c) {
     return acc;
 }
 
+// CHAIN: sum over the 8 sites f of one packed word of colours of  J[dist(l, f)] * s'_l(c_f)  for lane = site l:
+// two table look-ups (PRMT) and eight IDP.2A (both 16-bit halves of the couplings; Pl/Ph hold them in pairs).
+template <bool Q16>
+__device__ __forceinline__ uint32_t chain_dot8(const uint32_t (&Pl)[4], const uint32_t (&Ph)[4], const uint2& tab,
+                                               const uint2& tabb, uint32_t word) {
+    const uint32_t w1 = word >> 16;
+    const uint32_t S0 = tab_lookup<Q16>(tab, tabb, word, word ^ 0x8888u);
+    const uint32_t S1 = tab_lookup<Q16>(tab, tabb, w1, w1 ^ 0x8888u);
+    uint32_t lo0 = __dp2a_lo(Pl[0], S0, 0u), lo1 = __dp2a_lo(Pl[2], S1, 0u);
+    uint32_t hi0 = __dp2a_lo(Ph[0], S0, 0u), hi1 = __dp2a_lo(Ph[2], S1, 0u);
+    lo0 = __dp2a_hi(Pl[1], S0, lo0);
+    lo1 = __dp2a_hi(Pl[3], S1, lo1);
+    hi0 = __dp2a_hi(Ph[1], S0, hi0);
+    hi1 = __dp2a_hi(Ph[3], S1, hi1);
+    return (lo0 + lo1) + ((hi0 + hi1) << 16);
+}
+
 // ---- mbarrier (shared-memory transaction barrier) helpers: producer/consumer hand-off between the warps ----
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
@@ -350,8 +364,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     m.sp = (uint32_t*)(m.lut + (Q16 ? 2 * L : L));
     m.sp0 = m.sp + W;
     m.bq = m.sp0 + W;
-    m.selb = (uint8_t*)(m.bq + W);
-    m.part = (uint32_t*)(m.selb + L);
+    m.part = m.bq + W;
     m.Jz = (int32_t*)(m.part + 64);
     __shared__ int s_cnt[16];
     __shared__ long long s_E;   // running energy of this configuration (owner: lane 0 of chain warp 0)
@@ -452,18 +465,20 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             }
         }
         PT_LOAD_STATE();
+        if (tid == 0) {
+            mbar_init(&s_full[0], NTB >> 5); mbar_init(&s_full[1], NTB >> 5);
+            mbar_init(&s_done[0], 1); mbar_init(&s_done[1], 1);
+        }
         cta_sync();
         if (swap_mode == 3) { t = s_slot; scale = d.thr_scale[t]; }
 
         for (int s = 0; s < n_sweeps; ++s) {
             PT_T0(t_draw);
             direct_draw<Q16>(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
-            if (tid == 0) {
-                mbar_init(&s_full[0], NTB >> 5); mbar_init(&s_full[1], NTB >> 5);
-                mbar_init(&s_done[0], 1); mbar_init(&s_done[1], 1);
-            }
             cta_sync();
             PT_ACC(0, t_draw);
+            // the four barriers are initialised once per launch; every sweep completes NB/2 phases of each
+            const int phase0 = s * (NB >> 1);
             PT_T0(t_loop);
             // per-thread cursors, advanced by one block (32 sites = 4 words) per block
             const uint2* lutp = m.lut + gbase;   // (table of colours 8..15: L entries further)
@@ -479,10 +494,16 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             for (int kb = 0; kb < NB; ++kb) {
                 // block kb is summed against: blocks < kb-1 final (the chain warp is done with block kb-2, which
                 // also frees buffer kb&1), block kb-1 as at the start of the sweep, blocks >= kb untouched
-                if (kb >= 2) mbar_wait(&s_done[kb & 1], ((kb >> 1) - 1) & 1);
+#ifndef PT_EXP_NODONEWAIT
+                if (kb >= 2) mbar_wait(&s_done[kb & 1], (uint32_t)(phase0 + (kb >> 1) - 1) & 1u);
+#endif
                 PT_T0(t_b);
                 uint32_t val[DIRECT_SITES] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+#ifdef PT_EXP_NOBULK
+                if (false) {
+#else
                 if (active) {
+#endif
                     int wj2 = wj + 4;
                     wj2 -= wj2 >= W ? W : 0;
                     const uint4 wa = *reinterpret_cast<const uint4*>(m.sp + wj);
@@ -548,6 +569,14 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 // block sums: transpose-reduce over the 8 lanes of a warp that hold the same site group (lane bits
                 // 2..4 = j-range): 4 + 2 + 1 shuffles leave one site per lane, m = lane bits (2,3,4), then one
                 // shared-memory atomic per lane (32 different sites per warp)
+#ifdef PT_EXP_NOTAIL
+                {
+                    uint32_t v = 0;
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) v += val[i];
+                    if (v == 0x12345677u) atomicAdd(&m.part[(kb & 1) * 32 + lane], v);
+                }
+#else
                 {
                     uint32_t v4[4], v2[2];
                     const bool u4 = lane & 16, u3 = lane & 8, u2 = lane & 4;
@@ -561,6 +590,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                     const int msite = (u2 ? 1 : 0) + (u3 ? 2 : 0) + (u4 ? 4 : 0);
                     atomicAdd(&m.part[(kb & 1) * 32 + gbase + 2 * msite], v1);
                 }
+#endif
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&s_full[kb & 1]);
                 PT_ACC(1, t_b);
@@ -597,12 +627,20 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         // CORR: this warp's correction rows for lane = site l.  If site f of the previous block (rows f = 8cw+j)
         // or of the own block (rows 32 + 8cw + j) accepts a_f -> b_f, dE_l changes by
         //   Jq[dist] (s'_l(b_f) - s'_l(a_f)),   dist = l + 32 - f  resp.  l - f  (nothing for dist <= 0).
-        int Jp[8], Jo[8];
+        // The couplings are kept as 16-bit halves packed in pairs, like the bulk warps' (IDP.2A operands): pair p
+        // belongs to the sites f = 8cw + 2p, 8cw + 2p + 1.
+        uint32_t CPl[4], CPh[4], COl[4], COh[4];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const int dp = lane + 32 - (8 * cw + j), dn = lane - (8 * cw + j);
-            Jp[j] = __ldg(d.Jq + dp);               // 1 <= dp <= 63 < L
-            Jo[j] = dn > 0 ? __ldg(d.Jq + dn) : 0;
+        for (int p = 0; p < 4; ++p) {
+            const int f0 = 8 * cw + 2 * p, f1 = f0 + 1;
+            const uint32_t jp0 = (uint32_t)__ldg(d.Jq + (lane + 32 - f0));   // 1 <= distance <= 63 < L
+            const uint32_t jp1 = (uint32_t)__ldg(d.Jq + (lane + 32 - f1));
+            const uint32_t jo0 = lane - f0 > 0 ? (uint32_t)__ldg(d.Jq + (lane - f0)) : 0u;
+            const uint32_t jo1 = lane - f1 > 0 ? (uint32_t)__ldg(d.Jq + (lane - f1)) : 0u;
+            CPl[p] = (jp0 & 0xffffu) | (jp1 << 16);
+            CPh[p] = (jp0 >> 16) | ((jp1 >> 16) << 16);
+            COl[p] = (jo0 & 0xffffu) | (jo1 << 16);
+            COh[p] = (jo0 >> 16) | ((jo1 >> 16) << 16);
         }
         PT_LOAD_STATE();
         // Owner of the configuration's running energy and of the slot's accumulators (a8): lane 0 of chain warp 0.
@@ -612,50 +650,39 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         if (owner) { oa = ObsAcc(); s_E = d.E[x]; }
         cta_sync();
         if (swap_mode == 3) { t = s_slot; scale = d.thr_scale[t]; }
-        // A per-lane zero the compiler cannot see through: xor-ed into the accept masks it keeps the bit tests
-        // on the ALU pipe (LOP3 -> predicate, SEL) instead of shift pairs on the FMA or uniform pipes.
-        const unsigned lz = (unsigned)m.Jz[lane];
         int xb = 0;   // exchange buffer in use
 
         for (int s = 0; s < n_sweeps; ++s) {
             direct_draw<Q16>(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
             cta_sync();
+            const int phase0 = s * (NB >> 1);
             long long dE_acc = 0;
             int n_acc = 0;
             uint32_t mp = 0u;   // accept mask of the previous block
             for (int k = 0; k < NB; ++k) {
                 const int i0 = k << 5;
-                // independent of the bulk: threshold, the words of the block for the final update, and the
-                // correction rows (from the colours at the start of the sweep and the proposals: selb)
+                // independent of the bulk: threshold, the words of the block for the final update, and the part of the
+                // correction that does not depend on this block's decisions
                 const int th = m.theta[i0 + lane];
                 const int wsp = (i0 >> 3) + (lane & 3);
                 const uint32_t w_old = m.sp[wsp], w_new = m.bq[wsp];
                 const uint2 tab = m.lut[i0 + lane];
                 const uint2 tabb = Q16 ? m.lutb[i0 + lane] : make_uint2(0u, 0u);
-                int ipv = i0 - 32 + 8 * cw;
-                ipv += ipv < 0 ? L : 0;
-                const uint2 sfp = *reinterpret_cast<const uint2*>(m.selb + ipv);            // a | b << 4 of 8 sites
-                const uint2 sfo = *reinterpret_cast<const uint2*>(m.selb + i0 + 8 * cw);
-                int cp[8], co[8];
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const uint32_t wp = j < 4 ? sfp.x : sfp.y, wo = j < 4 ? sfo.x : sfo.y;
-                    // selector byte j: nibble 0 = a_f, nibble 1 = b_f (the two higher nibbles pick bytes that the
-                    // dot product weights with 0); byte 0 of the result = s'_l(a_f), byte 1 = s'_l(b_f)
-                    const uint32_t sp_ = wp >> (8 * (j & 3)), so_ = wo >> (8 * (j & 3));
-                    cp[j] = Jp[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, sp_, sp_ ^ 0x8888u), 0);
-                    co[j] = Jo[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, so_, so_ ^ 0x8888u), 0);
-                }
-                const int4 cp0 = make_int4(cp[0], cp[1], cp[2], cp[3]), cp1 = make_int4(cp[4], cp[5], cp[6], cp[7]);
-                const int4 co0 = make_int4(co[0], co[1], co[2], co[3]), co1 = make_int4(co[4], co[5], co[6], co[7]);
-                // changes accepted in block k-1, which the bulk sum saw as it was before: this warp's rows, known
-                // before the wait; they ride along with the first round below (one exchange less per block)
-                int pc = 0;
+                // this warp's 8 sites f = 8cw .. 8cw+7 of the block: colours now (= start of the sweep) and proposed
+                const uint32_t wf_old = m.sp[(i0 >> 3) + cw], wf_new = m.bq[(i0 >> 3) + cw];
+                // The bulk summed s'_l(a_f) for every site f of this block and of block k-1 (a_f = colour at the start
+                // of the sweep).  What site l must see instead is the colour c_f decided before its turn:
+                //   dS_l = sum_{f<l, own block} J[l-f] (s'_l(c_f) - s'_l(a_f)) + sum_{f in block k-1} J[l+32-f] (s'_l(c_f) - s'_l(a_f)).
+                // Each sum over this warp's 8 sites is one chain_dot8 (couplings 0 where f >= l).  base = everything
+                // that is known before the block sums arrive: -T_own(a) and, if block k-1 accepted anything, its part.
+                int base = -(int)chain_dot8<Q16>(COl, COh, tab, tabb, wf_old);
                 if (mp) {
-                    const unsigned mv = (mp >> (8 * cw)) ^ lz;
-                    pc = masked_add4(masked_add4(0, mv, 0, cp0), mv, 4, cp1);
+                    int wpv = ((i0 - 32) >> 3) + cw;
+                    wpv += wpv < 0 ? W : 0;
+                    base += (int)(chain_dot8<Q16>(CPl, CPh, tab, tabb, m.sp[wpv]) -
+                                  chain_dot8<Q16>(CPl, CPh, tab, tabb, m.sp0[wpv]));
                 }
-                mbar_wait(&s_full[k & 1], (k >> 1) & 1);
+                mbar_wait(&s_full[k & 1], (uint32_t)(phase0 + (k >> 1)) & 1u);
                 PT_T0(t_c);
                 const uint32_t S = m.part[(k & 1) * 32 + lane];
                 // slack y = theta - dE: the site accepts iff y >= 0 (theta <= 2^30 and |dE| < 2^30: no overflow)
@@ -663,17 +690,21 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 PT_ACC(1, t_c);
                 PT_T0(t_s);
                 // The accept mask a of the block is the unique solution of the triangular system
-                //   a_l = [ y_l - sum_{f<l} a_f cm[32+f][l] >= 0 ]      (cm[32+f][l] = 0 for f >= l),
+                //   a_l = [ y_l - dS_l(a_0 .. a_{l-1}) >= 0 ],
                 // which the site-by-site order solves by forward substitution.  Here: fixed-point iteration
                 // a <- F(a) from the guess "no correction"; after t rounds the first t bits are exact, so it ends
                 // after at most 33 rounds with exactly the sequential result, and in practice after two or three.
                 unsigned mask = __ballot_sync(0xffffffffu, y >= 0);   // first guess: no correction at all
                 int yy = y;
+#ifdef PT_EXP_NOCHAIN
+                mask = 0u;
+#endif
                 if (mask | mp) {   // nothing accepted here or in block k-1: nothing to correct
                     for (int it = 0; it < 33; ++it) {
-                        const unsigned mv = (mask >> (8 * cw)) ^ lz;
-                        const int part = masked_add4(masked_add4(pc, mv, 0, co0), mv, 4, co1);
-                        s_xch[xb][lane][cw] = part;
+                        // tentative colours of this warp's 8 sites under the current guess
+                        const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * cw));
+                        const uint32_t wt = (wf_old & ~nm) | (wf_new & nm);
+                        s_xch[xb][lane][cw] = base + (int)chain_dot8<Q16>(COl, COh, tab, tabb, wt);
                         asm volatile("bar.sync 1, 128;" ::: "memory");
                         const int4 pv = *reinterpret_cast<const int4*>(&s_xch[xb][lane][0]);
                         xb ^= 1;
@@ -870,6 +901,9 @@ typedef void (*direct_kernel_t)(Dev, long long, int, int, int, int);
 // r_hi = largest r <= L/2 with Jq[r] >= 2^16 (0 if none).
 // minb = 1: up to 168 registers per thread (fastest block sums); minb = 2: 80 registers, twice the CTAs per SM.
 inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb) {
+#ifdef PT_ONLY_HEADLINE   // development builds: only the configs[3] instantiation (fast to compile)
+    return sweep_direct_kernel<1, true, false, 1>;
+#else
     const bool l4096 = d.L == 4096;
     const int nq = direct_nearq(d.L, r_hi);
     if (d.L > 64 * (DIRECT_MAX_BULK / 4)) {   // more than 64 j-ranges: every near quad has a thread of its own
@@ -896,6 +930,7 @@ inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb) {
         }
     }
     return nq == 4 ? sweep_direct_kernel<4, false, true, 2> : sweep_direct_kernel<0, false, true, 2>;
+#endif
 }
 
 // CTAs of a sweep kernel variant that can be resident on the device at once (0 on error).

@@ -22,7 +22,7 @@ SYMBOLS = ["pt_create", "pt_create_ex", "pt_destroy", "pt_sweeps", "pt_energy", 
            "pt_observables", "pt_get_spins", "pt_get_spins_dev", "pt_set_spins", "pt_get_couplings",
            "pt_sweep_counter", "pt_set_variant", "pt_get_variant", "pt_set_stream", "pt_sweeps_async",
            "pt_sync", "pt_last_error", "pt_create_shard", "pt_energy_storage_dev", "pt_swap_external",
-           "pt_get_perm"]
+           "pt_get_perm", "pt_measure_peaks"]
 
 
 class PTError(RuntimeError):
@@ -74,6 +74,17 @@ _lib.pt_set_variant.argtypes = [_vp, _i32]
 _lib.pt_get_variant.argtypes = [_vp]
 _lib.pt_set_stream.argtypes = [_vp, _vp]
 _lib.pt_last_error.restype = ctypes.c_char_p
+_lib.pt_measure_peaks.argtypes = [_vp, _i32]
+
+PEAK_PATTERNS = ["idp2a", "idp4a", "imad", "prmt", "lop3", "prmt+2idp2a (idp2a counted)", "lop3+2idp2a (idp2a counted)",
+                 "lds128 (bytes)", "prmt+4idp2a (idp2a counted)", "2prmt+add+2idp2a (idp2a counted)"]
+
+
+def measure_peaks():
+    """pt_measure_peaks: {pattern: [rate with 1, 2, 3, 4 warps per sub-partition]} in lane-operations per clock and SM."""
+    r = np.zeros(len(PEAK_PATTERNS) * 4, dtype=np.float64)
+    _check(_lib.pt_measure_peaks(_p(r), int(r.size)))
+    return {name: [float(x) for x in r[4 * i:4 * i + 4]] for i, name in enumerate(PEAK_PATTERNS)}
 
 
 def _check(rc):
