@@ -29,7 +29,9 @@
  *    No C++ exception crosses this boundary.  Calls are synchronous: results
  *    are complete when the call returns (kernels run on the stream given to
  *    pt_set_stream, default stream otherwise).
- *  - A context must not be used from two threads at once.
+ *  - A context must not be used from two threads at once.  Every call runs on
+ *    the device the context was created on and restores the caller's current
+ *    device before it returns.
  */
 #ifndef PT_H_
 #define PT_H_
@@ -148,7 +150,8 @@ void pt_destroy(pt_ctx* ctx); /* NULL is allowed */
  * follows each sweep whose global index (counted from pt_create, first sweep
  * = 1) is a multiple of swap_every, so splitting n over several calls changes
  * nothing.  swap_every = 0: never swap.  Errors: PT_EINVAL (n < 0,
- * swap_every < 0), PT_ECUDA. */
+ * swap_every < 0), PT_EOVERFLOW (the sweep counter would pass 2^32 - 1: the
+ * sweep index is one 32-bit word of the Philox counter), PT_ECUDA. */
 int pt_sweeps(pt_ctx* ctx, int64_t n, int swap_every);
 
 /* Total energies E_out[n_ens*n_rep] (fixed point 2^-24).  recompute = 0 returns
@@ -170,6 +173,16 @@ int pt_get_spins_dev(pt_ctx* ctx, uint8_t* out_dev);
  * The sweep counter and the accumulators are kept. */
 int pt_set_spins(pt_ctx* ctx, const uint8_t* in);
 
+/* Checkpoint / resume.  The state of a context is: the configurations, their running energies,
+ * the accumulators and the sweep counter -- the generator is counter based and has no state, and the slot -> storage
+ * permutation is not observable.  pt_get_state writes them to host arrays (spins[n_ens*n_rep*L] colours 1..q,
+ * E[n_ens*n_rep], obs[n_ens*n_rep], all in slot order).  pt_set_state loads them into a context created with the same
+ * arguments: "destroy, create, pt_set_state, continue" is bit-identical to the uninterrupted run.  E may be NULL (the
+ * energies are recounted from the spins, O(L^2)); obs may be NULL (the accumulators are kept).  PT_EINVAL: a colour
+ * outside 1..q (state unchanged), sweep outside 0 .. 2^32 - 1, or a slot-sharded context. */
+int pt_get_state(pt_ctx* ctx, uint8_t* spins, int64_t* E, pt_obs* obs, int64_t* sweep);
+int pt_set_state(pt_ctx* ctx, const uint8_t* spins, const int64_t* E, const pt_obs* obs, int64_t sweep);
+
 /* Jq[L]: Jq[0] = 0, Jq[r] = Jq[L-r] = round(J*(r) 2^24). */
 int pt_get_couplings(pt_ctx* ctx, int32_t* Jq);
 
@@ -190,7 +203,9 @@ int pt_set_stream(pt_ctx* ctx, void* cuda_stream);
  * *n_launches (may be NULL) receives the number of kernels enqueued. */
 int pt_sweeps_async(pt_ctx* ctx, int64_t n, int swap_every, int64_t* n_launches);
 
-/* Blocks until the context's stream is idle; returns PT_ECUDA if a kernel failed. */
+/* Blocks until the context's stream is idle; returns PT_ECUDA if a kernel failed, or if a swap barrier inside a
+ * persistent launch timed out (30 s of wall-clock time without the arrival of a co-resident CTA: the state of the
+ * context is lost). */
 int pt_sync(pt_ctx* ctx);
 
 /* Instruction-rate micro-benchmarks on the current device (the ALU roofline of the direct sweep kernel

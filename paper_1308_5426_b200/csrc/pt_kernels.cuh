@@ -2,6 +2,9 @@
 // The sweep kernels are in pt_sweep_field.cuh and pt_sweep_direct.cuh.
 #pragma once
 #include <cstdint>
+#include <mutex>
+#include <set>
+#include <utility>
 
 #include "pt.h"
 #include "pt_device.cuh"
@@ -9,6 +12,22 @@
 namespace ptk {
 
 using namespace ptdev;
+
+// Opt a kernel in to the full dynamic shared memory of an SM once per process and device (not per launch: the
+// attribute belongs to the function, and contexts of different L share functions and may launch from different
+// host threads).  Returns a cudaError_t as int.
+inline int allow_max_dynamic_smem(const void* kernel, int static_bytes) {
+    static std::mutex mu;
+    static std::set<std::pair<const void*, int>> done;
+    int dev = 0;
+    cudaError_t err = cudaGetDevice(&dev);
+    if (err != cudaSuccess) return (int)err;
+    std::lock_guard<std::mutex> lock(mu);
+    if (done.count({kernel, dev})) return 0;
+    err = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - static_bytes);
+    if (err == cudaSuccess) done.insert({kernel, dev});
+    return (int)err;
+}
 
 // Everything a kernel needs to know about a context (passed by value).
 struct Dev {
@@ -30,6 +49,7 @@ struct Dev {
     unsigned* done;           // [n_ens] arrival counters of the swap event
     unsigned* gen;            // [n_ens] arrivals at the swap events of the running persistent launch
     long long* Epub;          // [2][n_ens][n_rep] energies published for those events, by storage index
+    int* err;                 // raised by a kernel whose in-kernel barrier timed out (host-mapped: read by pt_sync)
     long long* dbg;           // PT_TIMING builds: [n_ens*n_rep][32 warps][8] clock sums (else unused)
 };
 
@@ -365,6 +385,14 @@ __global__ void gather_slots_kernel(Dev d, const long long* __restrict__ in, lon
     if (gid >= d.n_ens * d.n_rep) return;
     const int e = gid / d.n_rep;
     out[gid] = in[(size_t)e * d.n_rep + d.perm[gid]];
+}
+
+// out[e][perm[e][slot]] = in[e][slot]
+__global__ void scatter_slots_kernel(Dev d, const long long* __restrict__ in, long long* __restrict__ out) {
+    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= d.n_ens * d.n_rep) return;
+    const int e = gid / d.n_rep;
+    out[(size_t)e * d.n_rep + d.perm[gid]] = in[gid];
 }
 
 }  // namespace ptk

@@ -39,6 +39,20 @@ int fail(int code, const std::string& msg) {
 
 constexpr size_t kSmemLimit = 227 * 1024;  // per CTA on sm_100
 
+// Every entry point runs on the context's device, whatever the caller's current device is, and restores it.
+struct DeviceGuard {
+    int prev = -1, want = -1;
+    explicit DeviceGuard(int dev) : want(dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != want) cudaSetDevice(want);
+    }
+    ~DeviceGuard() {
+        if (prev >= 0 && prev != want) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
 }  // namespace
 
 struct pt_ctx {
@@ -69,6 +83,10 @@ struct pt_ctx {
     long long* d_dbg = nullptr;
     unsigned* d_gen = nullptr;
     long long* d_Epub = nullptr;
+    uint8_t* d_stage = nullptr;   // [R*L] one byte per spin: staging for pt_get_spins / pt_set_spins / pt_set_state
+    uint8_t* h_stage = nullptr;   // pinned host bounce buffer of the same size
+    int* h_err = nullptr;    // pinned, device-mapped flag: an in-kernel barrier timed out
+    int* d_err = nullptr;    // its device address
     int coresident = -1;   // direct variant: CTAs that fit on the device at once (-1: not asked yet)
     ptk::direct_kernel_t direct_kern = nullptr;   // the sweep kernel instantiation this context uses
     int persistent_policy = 1;   // 0 never, 1 when the context fills the device and the call is long enough, 2 whenever possible
@@ -79,7 +97,7 @@ struct pt_ctx {
         d.L = L; d.W = L / 8; d.q = q; d.n_ens = n_ens; d.n_rep = n_rep; d.ens_base = ens_base;
         d.key0 = (uint32_t)seed; d.key1 = (uint32_t)(seed >> 32); d.rowsum = (uint32_t)rowsum;
         d.Jq = d_Jq; d.Jpair = d_Jpair; d.beta = d_beta; d.thr_scale = d_scale;
-        d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done; d.dbg = d_dbg; d.gen = d_gen; d.Epub = d_Epub;
+        d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done; d.dbg = d_dbg; d.gen = d_gen; d.Epub = d_Epub; d.err = d_err;
         d.rep_base = rep_base; d.n_local = n_local ? n_local : n_rep; d.count_swaps = rep_base == 0 ? 1 : 0;
         return d;
     }
@@ -95,6 +113,9 @@ void free_ctx(pt_ctx* c) {
     cudaFree(c->d_Jq); cudaFree(c->d_Jpair); cudaFree(c->d_beta); cudaFree(c->d_scale);
     cudaFree(c->d_spins); cudaFree(c->d_E); cudaFree(c->d_Etmp); cudaFree(c->d_Eout);
     cudaFree(c->d_perm); cudaFree(c->d_obs); cudaFree(c->d_h); cudaFree(c->d_done); cudaFree(c->d_flag); cudaFree(c->d_dbg); cudaFree(c->d_gen); cudaFree(c->d_Epub);
+    if (c->h_err) cudaFreeHost(c->h_err);
+    cudaFree(c->d_stage);
+    if (c->h_stage) cudaFreeHost(c->h_stage);
     delete c;
 }
 
@@ -105,8 +126,7 @@ int recompute_energy(pt_ctx* c, long long* d_out) {
         return PT_OK;
     }
     const size_t smem = (size_t)(c->L + c->L / 8) * 4;
-    if (smem > 48 * 1024)
-        PT_CUDA(cudaFuncSetAttribute(ptk::energy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (smem > 48 * 1024) PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::energy_kernel, 1024));
     ptk::energy_kernel<<<c->R(), 256, smem, c->stream>>>(c->dev(), d_out);
     PT_CUDA(cudaGetLastError());
     return PT_OK;
@@ -116,8 +136,7 @@ int ensure_fields(pt_ctx* c) {
     if (c->fields_valid) return PT_OK;
     if (!c->d_h) PT_CUDA(cudaMalloc(&c->d_h, (size_t)c->R() * c->q * c->L * sizeof(int32_t)));
     const size_t smem = (size_t)(c->L + c->L / 8) * 4;
-    if (smem > 48 * 1024)
-        PT_CUDA(cudaFuncSetAttribute(ptk::build_fields_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (smem > 48 * 1024) PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::build_fields_kernel, 1024));
     ptk::build_fields_kernel<<<c->R(), 256, smem, c->stream>>>(c->dev());
     PT_CUDA(cudaGetLastError());
     c->fields_valid = true;
@@ -151,7 +170,7 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
     const ptk::Dev d = c->dev();  // after ensure_fields: it may allocate d_h
     if (c->variant == PT_VARIANT_FIELD) {
         const size_t smem = ptk::field_smem_bytes(c->L, c->q);
-        PT_CUDA(cudaFuncSetAttribute(ptk::sweep_field_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::sweep_field_kernel, 1024));
         ptk::sweep_field_kernel<<<c->R(), ptk::FIELD_THREADS, smem, c->stream>>>(d, (long long)c->sweep, n_sweeps,
                                                                                  swap_mode == 1 ? 1 : 0);
     } else {
@@ -252,6 +271,11 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
     PT_CUDA_C(cudaMalloc(&c->d_gen, (size_t)n_ens * sizeof(unsigned)));
     PT_CUDA_C(cudaMemset(c->d_gen, 0, (size_t)n_ens * sizeof(unsigned)));
     PT_CUDA_C(cudaMalloc(&c->d_Epub, (size_t)2 * R * sizeof(long long)));
+    PT_CUDA_C(cudaMalloc(&c->d_stage, (size_t)R * L));
+    PT_CUDA_C(cudaHostAlloc(&c->h_stage, (size_t)R * L, cudaHostAllocDefault));
+    PT_CUDA_C(cudaHostAlloc(&c->h_err, sizeof(int), cudaHostAllocMapped));
+    *c->h_err = 0;
+    PT_CUDA_C(cudaHostGetDevicePointer(&c->d_err, c->h_err, 0));
     {
         // PT_PERSISTENT=0: one launch per swap interval; =2: persistent launches whenever all replicas can be
         // co-resident (tests); default: only for contexts that fill the device (see persistent_ok)
@@ -319,15 +343,20 @@ int pt_create(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep, co
 
 void pt_destroy(pt_ctx* ctx) {
     if (!ctx) return;
+    DeviceGuard guard(ctx->device);
     cudaStreamSynchronize(ctx->stream);
     free_ctx(ctx);
 }
 
 int pt_sweeps_async(pt_ctx* c, int64_t n, int swap_every, int64_t* n_launches) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");
+    DeviceGuard guard(c->device);
     if (n < 0 || swap_every < 0) return fail(PT_EINVAL, "n and swap_every must be >= 0");
     if (c->n_local && swap_every != 0)
         return fail(PT_EINVAL, "slot-sharded context: call pt_sweeps with swap_every = 0 and pt_swap_external");
+    // the sweep index is one 32-bit word of the Philox counter (site, sweep, slot, ensemble|tag): beyond 2^32 - 1 sweeps
+    // the random streams would repeat
+    if (c->sweep + n > 0xffffffffll) return fail(PT_EOVERFLOW, "sweep counter would exceed 2^32 - 1");
     int64_t launches = 0;
     constexpr int64_t kMaxChunk = 1 << 16;  // sweeps per launch
     // a persistent launch pays a counter reset and a cooperative launch: taken for every call of two or more sweeps
@@ -354,8 +383,12 @@ int pt_sweeps_async(pt_ctx* c, int64_t n, int swap_every, int64_t* n_launches) {
 
 int pt_sync(pt_ctx* c) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");
+    DeviceGuard guard(c->device);
     PT_CUDA(cudaStreamSynchronize(c->stream));
     PT_CUDA(cudaGetLastError());
+    if (c->h_err && *(volatile int*)c->h_err)
+        return fail(PT_ECUDA, "an in-kernel swap barrier timed out (a CTA of the ensemble did not arrive within 30 s): "
+                              "the state of this context is lost");
     return PT_OK;
 }
 
@@ -367,6 +400,7 @@ int pt_sweeps(pt_ctx* c, int64_t n, int swap_every) {
 
 int pt_energy_dev(pt_ctx* c, int64_t* E_out_dev, int recompute) {
     if (!c || !E_out_dev) return fail(PT_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     const long long* src = c->d_E;
     if (recompute) {
         int rc = recompute_energy(c, c->d_Etmp);
@@ -380,6 +414,7 @@ int pt_energy_dev(pt_ctx* c, int64_t* E_out_dev, int recompute) {
 
 int pt_energy(pt_ctx* c, int64_t* E_out, int recompute) {
     if (!c || !E_out) return fail(PT_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     int rc = pt_energy_dev(c, (int64_t*)c->d_Eout, recompute);
     if (rc) return rc;
     PT_CUDA(cudaMemcpy(E_out, c->d_Eout, (size_t)c->R() * sizeof(int64_t), cudaMemcpyDeviceToHost));
@@ -388,6 +423,7 @@ int pt_energy(pt_ctx* c, int64_t* E_out, int recompute) {
 
 int pt_observables(pt_ctx* c, pt_obs* out) {
     if (!c || !out) return fail(PT_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     int rc = pt_sync(c);
     if (rc) return rc;
     PT_CUDA(cudaMemcpy(out, c->d_obs, (size_t)c->R() * sizeof(pt_obs), cudaMemcpyDeviceToHost));
@@ -397,6 +433,7 @@ int pt_observables(pt_ctx* c, pt_obs* out) {
 
 int pt_get_spins_dev(pt_ctx* c, uint8_t* out_dev) {
     if (!c || !out_dev) return fail(PT_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     const long long nwords = (long long)c->R() * (c->L / 8);
     ptk::unpack_spins_kernel<<<(unsigned)((nwords + 255) / 256), 256, 0, c->stream>>>(c->dev(), out_dev);
     PT_CUDA(cudaGetLastError());
@@ -405,47 +442,86 @@ int pt_get_spins_dev(pt_ctx* c, uint8_t* out_dev) {
 
 int pt_get_spins(pt_ctx* c, uint8_t* out) {
     if (!c || !out) return fail(PT_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     const size_t n = (size_t)c->R() * c->L;
-    uint8_t* tmp = nullptr;
-    PT_CUDA(cudaMalloc(&tmp, n));
-    int rc = pt_get_spins_dev(c, tmp);
-    if (rc == PT_OK) {
-        cudaError_t err = cudaMemcpy(out, tmp, n, cudaMemcpyDeviceToHost);
-        if (err != cudaSuccess) rc = fail(PT_ECUDA, cudaGetErrorString(err));
-    }
-    cudaFree(tmp);
-    return rc;
+    int rc = pt_get_spins_dev(c, c->d_stage);
+    if (rc) return rc;
+    PT_CUDA(cudaMemcpyAsync(c->h_stage, c->d_stage, n, cudaMemcpyDeviceToHost, c->stream));   // pinned: one DMA
+    PT_CUDA(cudaStreamSynchronize(c->stream));
+    memcpy(out, c->h_stage, n);
+    return PT_OK;
 }
+
+namespace {
+// Uploads n_ens*n_rep*L colours 1..q (host, slot order), checks them and packs them into the spin words.  The state is
+// unchanged if a colour is out of range.  Leaves the stream busy (no synchronisation after the pack kernel).
+int upload_spins(pt_ctx* c, const uint8_t* in) {
+    const size_t n = (size_t)c->R() * c->L;
+    memcpy(c->h_stage, in, n);
+    PT_CUDA(cudaMemcpyAsync(c->d_stage, c->h_stage, n, cudaMemcpyHostToDevice, c->stream));
+    PT_CUDA(cudaMemsetAsync(c->d_flag, 0, sizeof(int), c->stream));
+    ptk::check_spins_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->dev(), c->d_stage, c->d_flag);
+    PT_CUDA(cudaGetLastError());
+    int flag = 0;
+    PT_CUDA(cudaMemcpyAsync(&flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    PT_CUDA(cudaStreamSynchronize(c->stream));
+    if (flag) return fail(PT_EINVAL, "colour outside 1..q");
+    const long long nwords = (long long)c->R() * (c->L / 8);
+    ptk::pack_spins_kernel<<<(unsigned)((nwords + 255) / 256), 256, 0, c->stream>>>(c->dev(), c->d_stage);
+    PT_CUDA(cudaGetLastError());
+    c->fields_valid = false;
+    return PT_OK;
+}
+}  // namespace
 
 int pt_set_spins(pt_ctx* c, const uint8_t* in) {
     if (!c || !in) return fail(PT_EINVAL, "NULL argument");
-    const size_t n = (size_t)c->R() * c->L;
-    uint8_t* tmp = nullptr;
-    PT_CUDA(cudaMalloc(&tmp, n));
-    int rc = PT_OK;
-    do {
-        cudaError_t err = cudaMemcpyAsync(tmp, in, n, cudaMemcpyHostToDevice, c->stream);
-        if (err == cudaSuccess) err = cudaMemsetAsync(c->d_flag, 0, sizeof(int), c->stream);
-        if (err != cudaSuccess) { rc = fail(PT_ECUDA, cudaGetErrorString(err)); break; }
-        ptk::check_spins_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->dev(), tmp, c->d_flag);
-        int flag = 0;
-        err = cudaMemcpyAsync(&flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
-        if (err == cudaSuccess) err = cudaStreamSynchronize(c->stream);
-        if (err != cudaSuccess) { rc = fail(PT_ECUDA, cudaGetErrorString(err)); break; }
-        if (flag) { rc = fail(PT_EINVAL, "colour outside 1..q"); break; }
-        const long long nwords = (long long)c->R() * (c->L / 8);
-        ptk::pack_spins_kernel<<<(unsigned)((nwords + 255) / 256), 256, 0, c->stream>>>(c->dev(), tmp);
-        c->fields_valid = false;
-        rc = recompute_energy(c, c->d_E);
-        if (rc) break;
-        rc = pt_sync(c);
-    } while (0);
-    cudaFree(tmp);
+    DeviceGuard guard(c->device);
+    int rc = upload_spins(c, in);
+    if (rc) return rc;
+    rc = recompute_energy(c, c->d_E);
+    if (rc) return rc;
+    return pt_sync(c);
+}
+
+int pt_get_state(pt_ctx* c, uint8_t* spins, int64_t* E, pt_obs* obs, int64_t* sweep) {
+    if (!c || !spins || !E || !obs || !sweep) return fail(PT_EINVAL, "NULL argument");
+    if (c->n_local) return fail(PT_EINVAL, "pt_get_state is not available for slot-sharded contexts");
+    int rc = pt_get_spins(c, spins);
+    if (rc == PT_OK) rc = pt_energy(c, E, 0);
+    if (rc == PT_OK) rc = pt_observables(c, obs);
+    if (rc == PT_OK) *sweep = c->sweep;
     return rc;
+}
+
+int pt_set_state(pt_ctx* c, const uint8_t* spins, const int64_t* E, const pt_obs* obs, int64_t sweep) {
+    if (!c || !spins) return fail(PT_EINVAL, "NULL argument");
+    if (c->n_local) return fail(PT_EINVAL, "pt_set_state is not available for slot-sharded contexts");
+    if (sweep < 0 || sweep > 0xffffffffll) return fail(PT_EINVAL, "sweep counter must be in 0 .. 2^32 - 1");
+    DeviceGuard guard(c->device);
+    int rc = upload_spins(c, spins);
+    if (rc) return rc;
+    if (E) {   // the caller's running energies (slot order) -> storage order, no O(L^2) recount
+        PT_CUDA(cudaMemcpyAsync(c->d_Eout, E, (size_t)c->R() * sizeof(int64_t), cudaMemcpyHostToDevice, c->stream));
+        ptk::scatter_slots_kernel<<<(c->R() + 255) / 256, 256, 0, c->stream>>>(c->dev(), c->d_Eout, c->d_E);
+        PT_CUDA(cudaGetLastError());
+    } else {
+        rc = recompute_energy(c, c->d_E);
+        if (rc) return rc;
+    }
+    if (obs) {
+        std::vector<pt_obs> tmp(obs, obs + c->R());
+        for (auto& o : tmp) o.near_ties = 0;
+        PT_CUDA(cudaMemcpyAsync(c->d_obs, tmp.data(), (size_t)c->R() * sizeof(pt_obs), cudaMemcpyHostToDevice, c->stream));
+        PT_CUDA(cudaStreamSynchronize(c->stream));   // tmp goes out of scope
+    }
+    c->sweep = sweep;
+    return pt_sync(c);
 }
 
 int pt_get_couplings(pt_ctx* c, int32_t* Jq) {
     if (!c || !Jq) return fail(PT_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     PT_CUDA(cudaMemcpy(Jq, c->d_Jq, (size_t)c->L * sizeof(int32_t), cudaMemcpyDeviceToHost));
     return PT_OK;
 }
@@ -472,6 +548,7 @@ int pt_create_shard(pt_ctx** out, int L, int q, double sigma, int n_rep, const d
 
 int pt_energy_storage_dev(pt_ctx* c, int64_t* E_out_dev) {
     if (!c || !E_out_dev) return fail(PT_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     const int n = c->n_local ? c->n_local : c->R();
     PT_CUDA(cudaMemcpyAsync(E_out_dev, c->d_E + c->rep_base, (size_t)n * sizeof(long long), cudaMemcpyDeviceToDevice,
                             c->stream));
@@ -480,6 +557,7 @@ int pt_energy_storage_dev(pt_ctx* c, int64_t* E_out_dev) {
 
 int pt_swap_external(pt_ctx* c, const int64_t* E_all_dev) {
     if (!c || !E_all_dev) return fail(PT_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     if (!c->n_local) return fail(PT_EINVAL, "pt_swap_external is for slot-sharded contexts (pt_create_shard)");
     PT_CUDA(cudaMemcpyAsync(c->d_E, E_all_dev, (size_t)c->n_rep * sizeof(long long), cudaMemcpyDeviceToDevice,
                             c->stream));
@@ -490,6 +568,7 @@ int pt_swap_external(pt_ctx* c, const int64_t* E_all_dev) {
 
 int pt_get_perm(pt_ctx* c, int32_t* perm) {
     if (!c || !perm) return fail(PT_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     int rc = pt_sync(c);
     if (rc) return rc;
     PT_CUDA(cudaMemcpy(perm, c->d_perm, (size_t)c->R() * sizeof(int), cudaMemcpyDeviceToHost));
@@ -551,6 +630,7 @@ int pt_get_variant(pt_ctx* c) { return c ? c->variant : PT_EINVAL; }
 
 int pt_set_stream(pt_ctx* c, void* cuda_stream) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");
+    DeviceGuard guard(c->device);
     PT_CUDA(cudaStreamSynchronize(c->stream));
     c->stream = (cudaStream_t)cuda_stream;
     return PT_OK;

@@ -82,10 +82,10 @@ constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 32 * DIRECT_CHAIN_WARPS;
 constexpr int DIRECT_BIG_BULK = 640;
 constexpr int DIRECT_BIG_THREADS = DIRECT_BIG_BULK + 32 * DIRECT_CHAIN_WARPS;
 constexpr int DIRECT_STATIC_SMEM = 13 * 1024;   // upper bound of the sweep kernel's static shared memory (12544 B)
-constexpr int DIRECT_NPAIR = 23;   // packed coupling pairs per thread and half: 32 + 2*7 distances
+constexpr int DIRECT_NPAIR = 39;   // packed coupling pairs per thread and half: 64 + 2*7 couplings
 constexpr int ENERGY_MAX_THREADS = 512, ENERGY_NPAIR = 35;   // energy_direct_kernel: 4 sites x 64 j per thread
-constexpr int DIRECT_NEAR_R = 95;  // NEAR covers the high halves of distances 32..95: the 24 quads of the left ranges 0..2
-constexpr int DIRECT_NEAR_QUADS = 24;
+constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: the 224 sites (56 quads) around a block
+constexpr int DIRECT_NEAR_QUADS = 56;
 constexpr int DIRECT_MAX_PERSIST_REP = 512;   // replicas per ensemble in a persistent launch (static shared arrays)
 
 __host__ __device__ inline size_t direct_smem_bytes(int L, int q);
@@ -113,9 +113,9 @@ __host__ __device__ inline int direct_nearq(int L, int r_hi) {
     if (r_hi > DIRECT_NEAR_R || L < 256 || nq > 4) return 0;
     return nq == 3 ? 4 : nq;
 }
-// dynamic smem (32-bit words): theta[L] | lut[2L] | lutb[2L] (q > 8 only) | sp[W] | sp0[W] | bq[W] | R0[4+W] | R2[4+W] | part[64]
+// dynamic smem (32-bit words): theta[L] | lut[2L] | lutb[2L] (q > 8 only) | sp[W] | sp0[W] | bq[W] | selb[L/4] | part[64] | Jz[96]
 __host__ __device__ inline size_t direct_smem_bytes(int L, int q) {
-    return (size_t)((q > 8 ? 5 : 3) * L + 5 * (L / 8) + 8 + 64) * 4;
+    return (size_t)((q > 8 ? 5 : 3) * L + 3 * (L / 8) + L / 4 + 64 + 96) * 4;
 }
 
 __device__ __forceinline__ int dp4a_s32_u32(int a, uint32_t b, int c) {
@@ -161,9 +161,9 @@ struct DirectSmem {
     uint32_t* sp;     // [W]  live packed spins
     uint32_t* sp0;    // [W]  spins at the start of the running sweep
     uint32_t* bq;     // [W]  proposed colours
-    uint32_t* R0;     // [4 + W] nibble-reversed copy of sp for even sites: word 4+w nibble n = colour of site (0 - 8w - n) mod L;
-    uint32_t* R2;     // [4 + W] ... for odd sites: site (2 - 8w - n) mod L.  Words 0..3 repeat words W..W+3 (wrap-around padding)
+    uint8_t* selb;    // [L]  a0 | b << 4: colour at the start of the sweep and proposed colour
     uint32_t* part;   // [2][32] block sums S_i, double buffered
+    int32_t* Jz;      // [96] Jz[n] = 0 for n < 32, Jq[n - 32] above
 };
 
 // Start of a sweep, all threads: proposals, thresholds and colour tables of all sites (A6, A7, A9) and the
@@ -176,7 +176,7 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
     for (int hw = threadIdx.x; hw < 2 * W; hw += blockDim.x) {
         const int w = hw >> 1, h4 = (hw & 1) << 2;
         const uint32_t word = m.sp[w];
-        uint32_t bhalf = 0;
+        uint32_t bhalf = 0, s4 = 0;
 #pragma unroll
         for (int n = 0; n < 4; ++n) {
             const int i = 8 * w + h4 + n;
@@ -185,6 +185,7 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
             const uint32_t k = __umulhi(p.w0, (uint32_t)(q - 1));
             const uint32_t b = k + (k >= a ? 1u : 0u);
             bhalf |= b << (4 * n);
+            s4 |= (a | (b << 4)) << (8 * n);
             m.theta[i] = min(accept_threshold(uniform53(p.w1, p.w2), scale), 1 << 30);  // |dE| < 2^30: same decisions
             unsigned long long ta = 0x0101010101010101ull, tb = ta;   // byte k = s'(k), k = 0..7 | 8..15
             if (!Q16 || a < 8u) ta += 1ull << (8 * a); else tb += 1ull << (8 * (a - 8u));
@@ -193,6 +194,7 @@ __device__ __forceinline__ void direct_draw(const Dev& d, const DirectSmem& m, u
             if (Q16) m.lutb[i] = make_uint2((uint32_t)tb, (uint32_t)(tb >> 32));
         }
         reinterpret_cast<uint16_t*>(m.bq)[hw] = (uint16_t)bhalf;   // low half of word w = sites 8w .. 8w+3
+        reinterpret_cast<uint32_t*>(m.selb)[hw] = s4;
         if (h4 == 0) m.sp0[w] = word;
     }
 }
@@ -232,6 +234,29 @@ __device__ __forceinline__ int direct_nmax(const uint32_t* sp, int W, int q, int
 // function of (energies, permutation, Philox(slot, sweep)), so all copies stay identical.  The CTA that holds storage 0
 // also counts the attempts/acceptances.  Returns the slot the configuration with storage index st now occupies.
 // Called by ALL threads of the CTA.
+// Waits (acquire) until the arrival counter *cnt reaches target.  The wait is bounded by wall-clock time (%globaltimer,
+// nanoseconds), not by a number of polls: a co-resident CTA may legitimately be late by a long time (time slicing with
+// another process, a profiler replaying the kernel).  After DIRECT_BARRIER_TIMEOUT_NS, or as soon as another CTA has
+// given up, *err is raised (pt_sync then returns PT_ECUDA; the state of the context is lost) and the wait returns.
+constexpr unsigned long long DIRECT_BARRIER_TIMEOUT_NS = 30ull * 1000ull * 1000ull * 1000ull;
+__device__ __forceinline__ void wait_arrivals(const unsigned* cnt, unsigned target, int* err) {
+    unsigned g = 0u, polls = 0u;
+    unsigned long long t0 = 0ull;
+    while (true) {
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(g) : "l"(cnt) : "memory");
+        if (g >= target) return;
+        if ((++polls & 1023u) == 0u) {
+            unsigned long long now;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+            if (t0 == 0ull) t0 = now;
+            if (now - t0 > DIRECT_BARRIER_TIMEOUT_NS || *(volatile int*)err != 0) {
+                *(volatile int*)err = 1;
+                return;
+            }
+        }
+    }
+}
+
 struct PersistSmem {
     int* perm;          // [n_rep] slot -> storage
     long long* Eall;    // [n_rep] energies by storage index
@@ -245,13 +270,7 @@ __device__ __forceinline__ int direct_swap_in_kernel(const Dev& d, const Persist
         __stcg(Epub + st, *s_E);
         // release: the energy is visible to whoever observes the arrival (cheaper than a full __threadfence)
         asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(d.gen + e) : "memory");
-        const unsigned target = (unsigned)n_rep * (unsigned)(event + 1);
-        unsigned g = 0u, spins = 0u;
-        while (true) {
-            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(g) : "l"(d.gen + e) : "memory");
-            if (g >= target) break;
-            if (++spins > (1u << 22)) __trap();   // seconds: a CTA of the ensemble is missing
-        }
+        wait_arrivals(d.gen + e, (unsigned)n_rep * (unsigned)(event + 1), d.err);
     }
     cta_sync();
     for (int t2 = threadIdx.x; t2 < n_rep; t2 += blockDim.x) ps.Eall[t2] = __ldcg(Epub + t2);
@@ -301,67 +320,6 @@ __device__ __forceinline__ int masked_add4(int acc, unsigned m, int b, int4 c) {
     return acc;
 }
 
-// the 8 nibbles of a word in reverse order
-__device__ __forceinline__ uint32_t nibble_reverse(uint32_t x) {
-    const uint32_t v = __byte_perm(x, 0u, 0x0123);
-    return ((v & 0x0f0f0f0fu) << 4) | ((v >> 4) & 0x0f0f0f0fu);
-}
-
-// Word ww of the nibble-reversed copy R_K (K = 0: Kp = 0, K = 2: Kp = 1) of the packed spins sp[W]: nibble n = colour
-// of site (K - 8 ww - n) mod L.  Those 8 sites are 8 consecutive nibbles of the word pair (sp[-ww-1], sp[-ww]).
-__device__ __forceinline__ uint32_t reversed_word(const uint32_t* sp, int W, int ww, int Kp) {
-    const uint32_t A = sp[W - ww - 1], B = sp[ww == 0 ? 0 : W - ww];
-    return nibble_reverse(__funnelshift_r(A, B, 4 + 8 * Kp));
-}
-__device__ __forceinline__ void store_reversed_word(uint32_t* Rp, int W, int ww, uint32_t v) {
-    Rp[4 + ww] = v;
-    if (ww >= W - 4) Rp[ww - (W - 4)] = v;   // wrap-around padding in front
-}
-
-// After block i0/32 has been decided: the 5 words of each reversed copy that hold sites of that block (lanes 0..9).
-__device__ __forceinline__ void update_reversed(const DirectSmem& m, int W, int i0, int lane) {
-    if (lane < 10) {
-        const int Kp = lane >= 5;
-        int ww = W - (i0 >> 3) - 4 + (lane - 5 * Kp);
-        ww -= ww >= W ? W : 0;
-        store_reversed_word(Kp ? m.R2 : m.R0, W, ww, reversed_word(m.sp, W, ww, Kp));
-    }
-}
-
-// CHAIN: sum over the 8 sites f of one packed word of colours of  J[dist(l, f)] * s'_l(c_f)  for lane = site l:
-// two table look-ups (PRMT) and eight IDP.2A (both 16-bit halves of the couplings; Pl/Ph hold them in pairs).
-template <bool Q16>
-__device__ __forceinline__ uint32_t chain_dot8(const uint32_t (&Pl)[4], const uint32_t (&Ph)[4], const uint2& tab,
-                                               const uint2& tabb, uint32_t word) {
-    const uint32_t w1 = word >> 16;
-    const uint32_t S0 = tab_lookup<Q16>(tab, tabb, word, word ^ 0x8888u);
-    const uint32_t S1 = tab_lookup<Q16>(tab, tabb, w1, w1 ^ 0x8888u);
-    uint32_t lo0 = __dp2a_lo(Pl[0], S0, 0u), lo1 = __dp2a_lo(Pl[2], S1, 0u);
-    uint32_t hi0 = __dp2a_lo(Ph[0], S0, 0u), hi1 = __dp2a_lo(Ph[2], S1, 0u);
-    lo0 = __dp2a_hi(Pl[1], S0, lo0);
-    lo1 = __dp2a_hi(Pl[3], S1, lo1);
-    hi0 = __dp2a_hi(Ph[1], S0, hi0);
-    hi1 = __dp2a_hi(Ph[3], S1, hi1);
-    return (lo0 + lo1) + ((hi0 + hi1) << 16);
-}
-
-// As chain_dot8, with the bytes M0, M1 (table values of eight more sites, here the mirror images of the word's sites
-// about lane = site l) added before the multiply: sum_f J[.] (s'_l(c_f) + s'_l(c_mirror(f))).
-template <bool Q16>
-__device__ __forceinline__ uint32_t chain_dot8m(const uint32_t (&Pl)[4], const uint32_t (&Ph)[4], const uint2& tab,
-                                                const uint2& tabb, uint32_t word, uint32_t M0, uint32_t M1) {
-    const uint32_t w1 = word >> 16;
-    const uint32_t S0 = tab_lookup<Q16>(tab, tabb, word, word ^ 0x8888u) + M0;
-    const uint32_t S1 = tab_lookup<Q16>(tab, tabb, w1, w1 ^ 0x8888u) + M1;
-    uint32_t lo0 = __dp2a_lo(Pl[0], S0, 0u), lo1 = __dp2a_lo(Pl[2], S1, 0u);
-    uint32_t hi0 = __dp2a_lo(Ph[0], S0, 0u), hi1 = __dp2a_lo(Ph[2], S1, 0u);
-    lo0 = __dp2a_hi(Pl[1], S0, lo0);
-    lo1 = __dp2a_hi(Pl[3], S1, lo1);
-    hi0 = __dp2a_hi(Ph[1], S0, hi0);
-    hi1 = __dp2a_hi(Ph[3], S1, hi1);
-    return (lo0 + lo1) + ((hi0 + hi1) << 16);
-}
-
 // ---- mbarrier (shared-memory transaction barrier) helpers: producer/consumer hand-off between the warps ----
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
@@ -409,9 +367,9 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     m.sp = (uint32_t*)(m.lut + (Q16 ? 2 * L : L));
     m.sp0 = m.sp + W;
     m.bq = m.sp0 + W;
-    m.R0 = m.bq + W;
-    m.R2 = m.R0 + 4 + W;
-    m.part = m.R2 + 4 + W;
+    m.selb = (uint8_t*)(m.bq + W);
+    m.part = (uint32_t*)(m.selb + L);
+    m.Jz = (int32_t*)(m.part + 64);
     __shared__ int s_cnt[16];
     __shared__ long long s_E;   // running energy of this configuration (owner: lane 0 of chain warp 0)
     __shared__ int s_slot;
@@ -456,71 +414,54 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(gt_start));
 #endif
 
+    for (int n = tid; n < 96; n += NT) m.Jz[n] = n < 32 ? 0 : d.Jq[n - 32];
     if (tid < 64) m.part[tid] = 0u;
     double scale = d.thr_scale[t];
     const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_SWEEP;
 
     if (tid < NTB) {
         // =========================== BULK warps ===========================
-        // thread -> (site group g, left range jr); group g = the 8 sites 16(g>>1) + (g&1) + {0,2,..,14}
+        // thread -> (site group g, j-range jr); group g = the 8 sites 16(g>>1) + (g&1) + {0,2,..,14}
         const int g = tid & 3, jr = tid >> 2;
-        const int par = g & 1, gh = g >> 1, gbase = 16 * gh + par;
+        const int par = g & 1, gbase = 16 * (g >> 1) + par;
         const int NJR = NJR64 ? 64 : L / 64;
         const bool active = jr < NJR;
-        const int H = L / 2;
-        // MIRROR PAIRING.  Jq[r] = Jq[L-r], so the two neighbours j = i-r and j' = i+r of a site i share one coupling:
-        //   sum_{j != i} Jq[|i-j|] s'_i(c_j) = sum_{r=1}^{L/2-1} Jq[r] (s'_i(c_{i-r}) + s'_i(c_{i+r})) + Jq[L/2] s'_i(c_{i+L/2}),
-        // i.e. ONE multiply-accumulate per pair of pair terms: per four distances r the bulk does two table
-        // look-ups (left and right neighbours), one byte-wise add (0..4 per byte) and two IDP.2A, instead of two
-        // look-ups and four IDP.2A.  Left range jr = the 32 sites of block kb-1-jr (8 quads u), jr = 0 .. L/64-1, so
-        // the left neighbours are the L/2 sites before the block and the pairs cover every distance 1 <= r < L/2 on
-        // the right and every left neighbour outside the own block: what is left for the chain warps are the left
-        // neighbours INSIDE the block (decided there), the changes of block kb-1 (read here as it was at the start of
-        // the sweep) and the one neighbour at distance L/2.  The right neighbours are read from a nibble-reversed copy
-        // of the spins (R0 for even, R2 for odd sites: R_K[p] = c[(K - p) mod L]), where they are 15 consecutive quads
-        // (quad u - mm + 8 of an 8-word window for site mm of the thread).
-        // Couplings of this thread: pair tt holds Jq[r], Jq[r-1] with r = R0 - 2 tt, 0 outside 1 <= r < L/2.
+        // couplings of this thread: pair tt holds Jq[r], Jq[r-1] with r = R0 - 2 tt  (mod L)
         uint32_t PL[DIRECT_NPAIR];
         uint32_t PH[FULL_HI ? DIRECT_NPAIR : 1];
         {
-            const int R0 = gbase + 14 + 32 * (jr + 1);
+            const int H = L / 2;
+            const int R0 = ((gbase + 14 - 64 * jr) % L + L) % L;
+            const uint32_t* lo = d.Jpair + (size_t)(2 * par) * H;
+            const uint32_t* hi = lo + H;
+            int r = R0;   // r = R0 - 2 tt (mod L) keeps the parity of `par`: no division or modulo per load
 #pragma unroll
             for (int tt = 0; tt < DIRECT_NPAIR; ++tt) {
-                const int r0 = R0 - 2 * tt, r1 = r0 - 1;
-                const uint32_t e0 = (active && r0 >= 1 && r0 < H) ? (uint32_t)__ldg(d.Jq + r0) : 0u;
-                const uint32_t e1 = (active && r1 >= 1 && r1 < H) ? (uint32_t)__ldg(d.Jq + r1) : 0u;
-                PL[tt] = (e0 & 0xffffu) | (e1 << 16);
-                if (FULL_HI) PH[tt] = (e0 >> 16) | ((e1 >> 16) << 16);
+                const int mm = (r - par) >> 1;
+                PL[tt] = active ? __ldg(lo + mm) : 0u;
+                if (FULL_HI) PH[tt] = active ? __ldg(hi + mm) : 0u;
+                r -= 2;
+                r += r < 0 ? L : 0;
             }
             if (!FULL_HI) PH[0] = 0u;
         }
-        // NEAR: the high halves Jq[r] >> 16 are non-zero for r <= r_hi <= 95 only, i.e. in the 24 quads of the left
-        // ranges 0..2.  Near quad n = 8 jrn + un (range jrn, quad un) is given to the thread slot x = jr + NJR iq with
-        // n = nearmap(x) (spread over all warps when there are 64 ranges).  NP[iq][mm][0] = hi(r) | hi(r-1) << 16,
-        // [1] = hi(r-2) | hi(r-3) << 16, r = gbase + 2mm + 32 (jrn+1) - 4 un; hi(x) = Jq[x] >> 16 for 1 <= x <= r_hi, x < L/2.
+        // NEAR: high halves of quad n = jr + NJR*iq (sites i0 - 96 + 4n + {0..3}) for this thread's 4 sites:
+        // NP[iq][mm][0] = hi(|r|) | hi(|r-1|) << 16, [1] = hi(|r-2|) | hi(|r-3|) << 16, r = gbase + 2mm + 96 - 4n,
+        // hi(x) = Jq[x] >> 16 for 1 <= x <= r_hi, else 0.
         uint32_t NP[NQ][DIRECT_SITES][2];
-        int njrn[NQ], nun[NQ];
+        if (NEARQ) {
 #pragma unroll
-        for (int iq = 0; iq < NQ; ++iq) {
-            const int x = jr + NJR * iq;
-            // with 64 or more ranges (8 or more bulk warps) the 24 near quads go to the first four warps, six each:
-            // one warp per SM sub-partition pays for the pass, the other warps skip it
-#ifdef PT_EXP_NEARALL
-            const int n = NJR64 ? (((x & 7) << 3) | (x >> 3)) : x;
-#else
-            const int n = NJR >= 64 ? (((jr >> 3) < 4 && (jr & 7) < 6) ? 6 * (jr >> 3) + (jr & 7) : 99) : x;
-#endif
-            njrn[iq] = n >> 3;
-            nun[iq] = n & 7;
-            if (NEARQ) {
+            for (int iq = 0; iq < NQ; ++iq) {
+                const int n = jr + NJR * iq;
 #pragma unroll
                 for (int mm = 0; mm < DIRECT_SITES; ++mm) {
                     uint32_t hv[4];
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
-                        const int r = gbase + 2 * mm + 32 * (njrn[iq] + 1) - 4 * nun[iq] - c;
-                        hv[c] = (active && n < DIRECT_NEAR_QUADS && r >= 1 && r <= r_hi && r < H)
-                                    ? ((uint32_t)__ldg(d.Jq + r) >> 16) : 0u;
+                        int r = gbase + 2 * mm + 96 - 4 * n - c;
+                        r = r < 0 ? -r : r;
+                        hv[c] = (active && n < DIRECT_NEAR_QUADS && r >= 1 && r <= r_hi) ? ((uint32_t)__ldg(d.Jq + r) >> 16)
+                                                                                        : 0u;
                     }
                     NP[iq][mm][0] = hv[0] | (hv[1] << 16);
                     NP[iq][mm][1] = hv[2] | (hv[3] << 16);
@@ -533,8 +474,6 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             mbar_init(&s_done[0], 1); mbar_init(&s_done[1], 1);
         }
         cta_sync();
-        for (int w = tid; w < 2 * W; w += NT)   // reversed copies of the spins (read after the sweep's first cta_sync)
-            store_reversed_word(w >= W ? m.R2 : m.R0, W, w >= W ? w - W : w, reversed_word(m.sp, W, w >= W ? w - W : w, w >= W));
         if (swap_mode == 3) { t = s_slot; scale = d.thr_scale[t]; }
 
         for (int s = 0; s < n_sweeps; ++s) {
@@ -547,157 +486,87 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             PT_T0(t_loop);
             // per-thread cursors, advanced by one block (32 sites = 4 words) per block
             const uint2* lutp = m.lut + gbase;   // (table of colours 8..15: L entries further)
-            // left range jr = block kb-1-jr: 4 words; range 0 is the block that is being decided: sweep-start copy
-            const uint32_t* spl = (jr == 0) ? m.sp0 : m.sp;
-            int wl = W - ((4 * (jr + 1)) % W);
-            wl -= wl >= W ? W : 0;
-            // right neighbours: 8 words of the reversed copy, starting at word (-4 kb - 4 (jr+1) - 4 gh - 4) mod W
-            const uint32_t* Rk = (par ? m.R2 : m.R0) + 4;   // (4 words of wrap-around padding in front)
-            int wr = W - ((4 * (jr + 1) + 4 * gh + 4) % W);
-            wr -= wr >= W ? W : 0;
-            // NEAR: halfword (quad) cursors of the left quad and of the right quad of site mm = 0
-            int hnl[NQ], hnr[NQ];
-            const uint16_t* nsrc[NQ];
+            int wj = 8 * jr;                                    // first word of this thread's j-range
+            // the second half of the last range is block kb-1, which is being decided: sweep-start copy
+            const uint32_t* sp2 = (jr == NJR - 1) ? m.sp0 : m.sp;
+            int wn[NQ];                                         // NEAR: word of quad n = jr + NJR*iq
 #pragma unroll
             for (int iq = 0; iq < NQ; ++iq) {
-                nsrc[iq] = reinterpret_cast<const uint16_t*>(njrn[iq] == 0 ? m.sp0 : m.sp);
-                hnl[iq] = ((2 * W - ((8 * (njrn[iq] + 1)) % (2 * W))) + nun[iq]) % (2 * W);
-                hnr[iq] = ((2 * W - ((8 * (njrn[iq] + 1) + 8 * gh) % (2 * W))) + nun[iq]) % (2 * W);
+                wn[iq] = ((jr + NJR * iq) >> 1) - 12;
+                wn[iq] += wn[iq] < 0 ? W : 0;
             }
             for (int kb = 0; kb < NB; ++kb) {
                 // block kb is summed against: blocks < kb-1 final (the chain warp is done with block kb-2, which
                 // also frees buffer kb&1), block kb-1 as at the start of the sweep, blocks >= kb untouched
-                // (two blocks only, L = 64: the right neighbours of block 1 are block 0 itself -- no overlap there)
-                if (NB == 2) {
-                    if (kb == 1) mbar_wait(&s_done[0], (uint32_t)phase0 & 1u);
-                } else if (kb >= 2) {
-                    mbar_wait(&s_done[kb & 1], (uint32_t)(phase0 + (kb >> 1) - 1) & 1u);
-                }
+                if (kb >= 2) mbar_wait(&s_done[kb & 1], (uint32_t)(phase0 + (kb >> 1) - 1) & 1u);
                 PT_T0(t_b);
                 uint32_t val[DIRECT_SITES] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
-#ifdef PT_EXP_NOBULK
-                if (false) {
-#else
                 if (active) {
-#endif
-                    int wr1 = wr + 4;
-                    wr1 -= wr1 >= W ? W : 0;
-                    const uint4 wa = *reinterpret_cast<const uint4*>(spl + wl);
-                    const uint4 ra = *reinterpret_cast<const uint4*>(Rk + wr);
-                    const uint4 rb = *reinterpret_cast<const uint4*>(Rk + wr1);
-                    const uint32_t words[4] = {wa.x, wa.y, wa.z, wa.w};
-                    const uint32_t rw[8] = {ra.x, ra.y, ra.z, ra.w, rb.x, rb.y, rb.z, rb.w};
+                    int wj2 = wj + 4;
+                    wj2 -= wj2 >= W ? W : 0;
+                    const uint4 wa = *reinterpret_cast<const uint4*>(m.sp + wj);
+                    const uint4 wb = *reinterpret_cast<const uint4*>(sp2 + wj2);
+                    const uint32_t words[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
                     uint2 lt[DIRECT_SITES], ltb[DIRECT_SITES];
 #pragma unroll
                     for (int mm = 0; mm < DIRECT_SITES; ++mm) {
                         lt[mm] = lutp[2 * mm];
                         ltb[mm] = Q16 ? lutp[L + 2 * mm] : make_uint2(0u, 0u);
                     }
-                    uint32_t rsel[16];   // right quads 1..15 of the window
+                    uint32_t nword[NQ];
 #pragma unroll
-                    for (int qd = 0; qd < 16; ++qd) rsel[qd] = (qd & 1) ? (rw[qd >> 1] >> 16) : rw[qd >> 1];
-                    // two accumulators per site (even / odd pair of distances) keep the IDP.2A chains short
+                    for (int iq = 0; iq < NQ; ++iq) {   // quads 16..23 are block kb-1: sweep-start copy
+                        const int n = jr + NJR * iq;
+                        nword[iq] = NEARQ ? ((n >= 16 && n < 24) ? m.sp0 : m.sp)[wn[iq]] : 0u;
+                    }
+                    // two accumulators per site (even / odd pair of j) keep the IDP.2A chains short
                     uint32_t alo[DIRECT_SITES], alo2[DIRECT_SITES], ahi[DIRECT_SITES];
 #pragma unroll
                     for (int mm = 0; mm < DIRECT_SITES; ++mm) { alo[mm] = 0u; alo2[mm] = 0u; ahi[mm] = 0u; }
-#ifdef PT_EXP_ACC4
-                    uint32_t alo3[DIRECT_SITES], alo4[DIRECT_SITES];
 #pragma unroll
-                    for (int mm = 0; mm < DIRECT_SITES; ++mm) { alo3[mm] = 0u; alo4[mm] = 0u; }
-#endif
-#pragma unroll
-                    for (int u = 0; u < 8; ++u) {
+                    for (int u = 0; u < 16; ++u) {
                         const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
                         const uint32_t selx = sel ^ 0x8888u;
 #pragma unroll
                         for (int mm = 0; mm < DIRECT_SITES; ++mm) {
-                            const uint32_t sr = rsel[u - mm + 8];
-                            // bytes: s'(left neighbour) + s'(right neighbour) in 0..4 for four distances
-                            const uint32_t S = tab_lookup<Q16>(lt[mm], ltb[mm], sel, selx) +
-                                               tab_lookup<Q16>(lt[mm], ltb[mm], sr, sr ^ 0x8888u);
+                            const uint32_t S = tab_lookup<Q16>(lt[mm], ltb[mm], sel, selx);
                             const int tt = 7 - mm + 2 * u;
-#ifdef PT_EXP_ACC4
-                            if (u & 1) {
-                                alo3[mm] = __dp2a_lo(PL[tt], S, alo3[mm]);
-                                alo4[mm] = __dp2a_hi(PL[tt + 1], S, alo4[mm]);
-                            } else
-#endif
-                            {
                             alo[mm] = __dp2a_lo(PL[tt], S, alo[mm]);
                             alo2[mm] = __dp2a_hi(PL[tt + 1], S, alo2[mm]);
-                            }
                             if (FULL_HI) {
                                 ahi[mm] = __dp2a_lo(PH[FULL_HI ? tt : 0], S, ahi[mm]);
                                 ahi[mm] = __dp2a_hi(PH[FULL_HI ? tt + 1 : 0], S, ahi[mm]);
                             }
                         }
                     }
-#ifdef PT_EXP_NONEAR
-                    if (false) {
-#else
-#ifdef PT_EXP_NEARALL
                     if (NEARQ) {
-#else
-                    if (NEARQ && (NJR < 64 || warp < 4)) {
-#endif
-#endif
-                        const uint16_t* Rh = reinterpret_cast<const uint16_t*>(Rk);   // halfword = quad; index >= -8 valid
 #pragma unroll
                         for (int iq = 0; iq < NQ; ++iq) {
-                            const uint32_t sel = nsrc[iq][hnl[iq]];
+                            const int n = jr + NJR * iq;
+                            const uint32_t sel = (n & 1) ? (nword[iq] >> 16) : nword[iq];
 #pragma unroll
                             for (int mm = 0; mm < DIRECT_SITES; ++mm) {
-                                const uint32_t sr = Rh[hnr[iq] - mm];
-                                const uint32_t S = tab_lookup<Q16>(lt[mm], ltb[mm], sel, sel ^ 0x8888u) +
-                                                   tab_lookup<Q16>(lt[mm], ltb[mm], sr, sr ^ 0x8888u);
+                                const uint32_t S = tab_lookup<Q16>(lt[mm], ltb[mm], sel, sel ^ 0x8888u);
                                 ahi[mm] = __dp2a_lo(NP[iq][mm][0], S, ahi[mm]);
                                 ahi[mm] = __dp2a_hi(NP[iq][mm][1], S, ahi[mm]);
                             }
                         }
                     }
 #pragma unroll
-#ifdef PT_EXP_ACC4
-#pragma unroll
-                    for (int mm = 0; mm < DIRECT_SITES; ++mm) alo[mm] += alo3[mm] + alo4[mm];
-#endif
-#pragma unroll
                     for (int mm = 0; mm < DIRECT_SITES; ++mm) val[mm] = alo[mm] + alo2[mm] + (ahi[mm] << 16);
                     // advance the cursors
                     lutp += 32;
-                    wl += 4;
-                    wl -= wl >= W ? W : 0;
-                    wr -= 4;
-                    wr += wr < 0 ? W : 0;
+                    wj += 4;
+                    wj -= wj >= W ? W : 0;
 #pragma unroll
                     for (int iq = 0; iq < NQ; ++iq) {
-                        hnl[iq] += 8;
-                        hnl[iq] -= hnl[iq] >= 2 * W ? 2 * W : 0;
-                        hnr[iq] -= 8;
-                        hnr[iq] += hnr[iq] < 0 ? 2 * W : 0;
+                        wn[iq] += 4;
+                        wn[iq] -= wn[iq] >= W ? W : 0;
                     }
                 }
                 // block sums: transpose-reduce over the 8 lanes of a warp that hold the same site group (lane bits
                 // 2..4 = j-range): 4 + 2 + 1 shuffles leave one site per lane, m = lane bits (2,3,4), then one
                 // shared-memory atomic per lane (32 different sites per warp)
-#ifdef PT_EXP_NOTAIL
-                {
-                    uint32_t v = 0;
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) v += val[i];
-                    if (v == 0x12345677u) atomicAdd(&m.part[(kb & 1) * 32 + lane], v);
-                }
-#elif defined(PT_EXP_REDUX)
-                {
-                    const unsigned gm = 0x11111111u << (lane & 3);
-                    uint32_t mine = 0u;
-#pragma unroll
-                    for (int i = 0; i < 8; ++i) {
-                        const uint32_t r = __reduce_add_sync(gm, val[i]);
-                        mine = (lane >> 2) == i ? r : mine;
-                    }
-                    atomicAdd(&m.part[(kb & 1) * 32 + gbase + 2 * (lane >> 2)], mine);
-                }
-#else
                 {
                     uint32_t v4[4], v2[2];
                     const bool u4 = lane & 16, u3 = lane & 8, u2 = lane & 4;
@@ -711,7 +580,6 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                     const int msite = (u2 ? 1 : 0) + (u3 ? 2 : 0) + (u4 ? 4 : 0);
                     atomicAdd(&m.part[(kb & 1) * 32 + gbase + 2 * msite], v1);
                 }
-#endif
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&s_full[kb & 1]);
                 PT_ACC(1, t_b);
@@ -748,27 +616,13 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         // CORR: this warp's correction rows for lane = site l.  If site f of the previous block (rows f = 8cw+j)
         // or of the own block (rows 32 + 8cw + j) accepts a_f -> b_f, dE_l changes by
         //   Jq[dist] (s'_l(b_f) - s'_l(a_f)),   dist = l + 32 - f  resp.  l - f  (nothing for dist <= 0).
-        // What the bulk sum of a block lacks (see BULK): the left neighbours inside the block, with the colours decided
-        // there; the changes accepted in block k-1, which the bulk read as it was at the start of the sweep; the one
-        // neighbour at distance L/2.  Couplings as 16-bit halves packed in pairs (IDP.2A operands): pair p belongs to
-        // the sites f = 8cw + 2p, 8cw + 2p + 1 of a block; lane = site l of block k.
-        //   JOl: own block, f < l (distance l - f)
-        //   JPa: block k-1, every f with distance l + 32 - f < L/2
-        uint32_t JOl[2][4], JPa[2][4];
+        int Jp[8], Jo[8];
 #pragma unroll
-        for (int p = 0; p < 4; ++p) {
-            uint32_t v[2][2];
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int f = 8 * cw + 2 * p + h;
-                const int dl = lane - f, dp = lane + 32 - f;
-                v[0][h] = dl > 0 ? (uint32_t)__ldg(d.Jq + dl) : 0u;
-                v[1][h] = dp < (L >> 1) ? (uint32_t)__ldg(d.Jq + dp) : 0u;   // dp >= 1
-            }
-            JOl[0][p] = (v[0][0] & 0xffffu) | (v[0][1] << 16); JOl[1][p] = (v[0][0] >> 16) | ((v[0][1] >> 16) << 16);
-            JPa[0][p] = (v[1][0] & 0xffffu) | (v[1][1] << 16); JPa[1][p] = (v[1][0] >> 16) | ((v[1][1] >> 16) << 16);
+        for (int j = 0; j < 8; ++j) {
+            const int dp = lane + 32 - (8 * cw + j), dn = lane - (8 * cw + j);
+            Jp[j] = __ldg(d.Jq + dp);               // 1 <= dp <= 63 < L
+            Jo[j] = dn > 0 ? __ldg(d.Jq + dn) : 0;
         }
-        const int JH = __ldg(d.Jq + (L >> 1));   // distance L/2: one neighbour only
         PT_LOAD_STATE();
         // Owner of the configuration's running energy and of the slot's accumulators (a8): lane 0 of chain warp 0.
         // They live in shared memory, so nothing of this costs registers in the bulk path.
@@ -776,9 +630,10 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         ObsAcc& oa = s_oa;
         if (owner) { oa = ObsAcc(); s_E = d.E[x]; }
         cta_sync();
-        for (int w = tid; w < 2 * W; w += NT)   // reversed copies of the spins (read after the sweep's first cta_sync)
-            store_reversed_word(w >= W ? m.R2 : m.R0, W, w >= W ? w - W : w, reversed_word(m.sp, W, w >= W ? w - W : w, w >= W));
         if (swap_mode == 3) { t = s_slot; scale = d.thr_scale[t]; }
+        // A per-lane zero the compiler cannot see through: xor-ed into the accept masks it keeps the bit tests
+        // on the ALU pipe (LOP3 -> predicate, SEL) instead of shift pairs on the FMA or uniform pipes.
+        const unsigned lz = (unsigned)m.Jz[lane];
         int xb = 0;   // exchange buffer in use
 
         for (int s = 0; s < n_sweeps; ++s) {
@@ -790,82 +645,55 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             uint32_t mp = 0u;   // accept mask of the previous block
             for (int k = 0; k < NB; ++k) {
                 const int i0 = k << 5;
-                // independent of the bulk: threshold, the words of the block for the final update, and the part of the
-                // correction that does not depend on this block's decisions
+                // independent of the bulk: threshold, the words of the block for the final update, and the
+                // correction rows (from the colours at the start of the sweep and the proposals: selb)
                 const int th = m.theta[i0 + lane];
                 const int wsp = (i0 >> 3) + (lane & 3);
                 const uint32_t w_old = m.sp[wsp], w_new = m.bq[wsp];
                 const uint2 tab = m.lut[i0 + lane];
                 const uint2 tabb = Q16 ? m.lutb[i0 + lane] : make_uint2(0u, 0u);
-                // this warp's 8 sites f = 8cw .. 8cw+7 of the block: colours now (= start of the sweep) and proposed
-                const uint32_t wf_old = m.sp[(i0 >> 3) + cw], wf_new = m.bq[(i0 >> 3) + cw];
-                // Known before the block sums arrive: the left neighbours inside the block under the guess "nobody
-                // before me changes" (own0), the changes accepted in block k-1 and the neighbour at distance L/2.
-                // Each sum over this warp's 8 sites is one chain_dot8; the four warps' parts are exchanged through
-                // shared memory before the wait.
-                int wpv = ((i0 - 32) >> 3) + cw;
-                wpv += wpv < 0 ? W : 0;
-#ifdef PT_EXP_NOPRE
-                const int own0 = 0;
-                int base = 0;
-#else
-                // The bulk pairs every left neighbour outside the block with the right neighbour at the same distance;
-                // the right neighbours at the distances of the left neighbours INSIDE the block (r = l - f, the sites
-                // i0 + 2l - f: not visited yet) are paired here: their table values M0, M1 are added to those of the
-                // sites f.  They are eight consecutive nibbles of the reversed copy R0, from position (8cw - i0 - 2l) mod L.
-                uint32_t M0, M1;
-                {
-                    int p0 = 8 * cw - i0 - 2 * lane;
-                    p0 += p0 < 0 ? L : 0;
-                    p0 += p0 < 0 ? L : 0;
-                    const int w0 = p0 >> 3, w1 = (w0 + 1 == W) ? 0 : w0 + 1;
-                    const uint32_t wm = __funnelshift_r(m.R0[4 + w0], m.R0[4 + w1], 4 * (p0 & 7));
-                    const uint32_t wmh = wm >> 16;
-                    M0 = tab_lookup<Q16>(tab, tabb, wm, wm ^ 0x8888u);
-                    M1 = tab_lookup<Q16>(tab, tabb, wmh, wmh ^ 0x8888u);
+                int ipv = i0 - 32 + 8 * cw;
+                ipv += ipv < 0 ? L : 0;
+                const uint2 sfp = *reinterpret_cast<const uint2*>(m.selb + ipv);            // a | b << 4 of 8 sites
+                const uint2 sfo = *reinterpret_cast<const uint2*>(m.selb + i0 + 8 * cw);
+                int cp[8], co[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const uint32_t wp = j < 4 ? sfp.x : sfp.y, wo = j < 4 ? sfo.x : sfo.y;
+                    // selector byte j: nibble 0 = a_f, nibble 1 = b_f (the two higher nibbles pick bytes that the
+                    // dot product weights with 0); byte 0 of the result = s'_l(a_f), byte 1 = s'_l(b_f)
+                    const uint32_t sp_ = wp >> (8 * (j & 3)), so_ = wo >> (8 * (j & 3));
+                    cp[j] = Jp[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, sp_, sp_ ^ 0x8888u), 0);
+                    co[j] = Jo[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, so_, so_ ^ 0x8888u), 0);
                 }
-                const int own0 = (int)chain_dot8m<Q16>(JOl[0], JOl[1], tab, tabb, wf_old, M0, M1);
-                int base = own0;
-                if (mp) base += (int)(chain_dot8<Q16>(JPa[0], JPa[1], tab, tabb, m.sp[wpv]) -
-                                      chain_dot8<Q16>(JPa[0], JPa[1], tab, tabb, m.sp0[wpv]));
-                if (cw == 3) {
-                    int ih = i0 + lane + (L >> 1);
-                    ih -= ih >= L ? L : 0;
-                    const uint32_t ch = (uint32_t)get_nibble(m.sp, ih);
-                    base += JH * (int)(tab_lookup<Q16>(tab, tabb, ch, ch ^ 0x8888u) & 0xffu);
+                const int4 cp0 = make_int4(cp[0], cp[1], cp[2], cp[3]), cp1 = make_int4(cp[4], cp[5], cp[6], cp[7]);
+                const int4 co0 = make_int4(co[0], co[1], co[2], co[3]), co1 = make_int4(co[4], co[5], co[6], co[7]);
+                // changes accepted in block k-1, which the bulk sum saw as it was before: this warp's rows, known
+                // before the wait; they ride along with the first round below (one exchange less per block)
+                int pc = 0;
+                if (mp) {
+                    const unsigned mv = (mp >> (8 * cw)) ^ lz;
+                    pc = masked_add4(masked_add4(0, mv, 0, cp0), mv, 4, cp1);
                 }
-                s_xch[xb][lane][cw] = base;
-                asm volatile("bar.sync 1, 128;" ::: "memory");
-                {
-                    const int4 pv = *reinterpret_cast<const int4*>(&s_xch[xb][lane][0]);
-                    xb ^= 1;
-                    base = (pv.x + pv.y) + (pv.z + pv.w);
-                }
-#endif
                 mbar_wait(&s_full[k & 1], (uint32_t)(phase0 + (k >> 1)) & 1u);
                 PT_T0(t_c);
                 const uint32_t S = m.part[(k & 1) * 32 + lane];
-                // slack y = theta - dE under the guess "nobody before me in this block changes": the site accepts iff
-                // y - (change of its own-block part) >= 0  (theta <= 2^30 and |dE| < 2^30: no overflow)
-                const int y = th - (int)(S + (uint32_t)base - rowsum);
+                // slack y = theta - dE: the site accepts iff y >= 0 (theta <= 2^30 and |dE| < 2^30: no overflow)
+                int y = th - (int)(S - rowsum);
                 PT_ACC(1, t_c);
                 PT_T0(t_s);
                 // The accept mask a of the block is the unique solution of the triangular system
-                //   a_l = [ y_l - sum_{f<l} Jq[l-f] (s'_l(c_f(a_f)) - s'_l(old colour of f)) >= 0 ],  c_f = b_f if a_f,
+                //   a_l = [ y_l - sum_{f<l} a_f cm[32+f][l] >= 0 ]      (cm[32+f][l] = 0 for f >= l),
                 // which the site-by-site order solves by forward substitution.  Here: fixed-point iteration
-                // a <- F(a) from that guess; after t rounds the first t bits are exact, so it ends after at most 33
-                // rounds with exactly the sequential result, and in practice after two or three.
-                unsigned mask = __ballot_sync(0xffffffffu, y >= 0);
+                // a <- F(a) from the guess "no correction"; after t rounds the first t bits are exact, so it ends
+                // after at most 33 rounds with exactly the sequential result, and in practice after two or three.
+                unsigned mask = __ballot_sync(0xffffffffu, y >= 0);   // first guess: no correction at all
                 int yy = y;
-#ifdef PT_EXP_NOCHAIN
-                mask = 0u;
-#endif
-                if (mask) {   // nothing accepted under the guess "no change before me": that guess is the answer
+                if (mask | mp) {   // nothing accepted here or in block k-1: nothing to correct
                     for (int it = 0; it < 33; ++it) {
-                        // tentative colours of this warp's 8 sites under the current guess
-                        const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * cw));
-                        const uint32_t wt = (wf_old & ~nm) | (wf_new & nm);
-                        s_xch[xb][lane][cw] = (int)chain_dot8m<Q16>(JOl[0], JOl[1], tab, tabb, wt, M0, M1) - own0;
+                        const unsigned mv = (mask >> (8 * cw)) ^ lz;
+                        const int part = masked_add4(masked_add4(pc, mv, 0, co0), mv, 4, co1);
+                        s_xch[xb][lane][cw] = part;
                         asm volatile("bar.sync 1, 128;" ::: "memory");
                         const int4 pv = *reinterpret_cast<const int4*>(&s_xch[xb][lane][0]);
                         xb ^= 1;
@@ -879,28 +707,17 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                     }
                 }
                 PT_ACC(2, t_s);
-                if (cw == 0) {
-                    if (lane < 4) {
-                        const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
-                        m.sp[wsp] = (w_old & ~nm) | (w_new & nm);
-                    }
-                    if (NB == 2) {   // L = 64: block k is the right neighbour of the next block: before the barrier
-                        __syncwarp();
-                        update_reversed(m, W, i0, lane);
-                    }
+                if (cw == 0 && lane < 4) {
+                    const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
+                    m.sp[wsp] = (w_old & ~nm) | (w_new & nm);
                 }
                 // every chain warp has read the block sums of buffer k&1 (without rounds there is no other barrier
                 // between a slow warp's read and this point) before they are cleared and the buffer is handed back
                 asm volatile("bar.sync 1, 128;" ::: "memory");
                 if (cw == 0) {
                     m.part[(k & 1) * 32 + lane] = 0u;
-                    // The bulk reads block k as a right neighbour from block k + NB/2 on, and has waited for the
-                    // release of block k + NB/2 - 2 by then: with 6 or more blocks the reversed copies can be
-                    // brought up to date after the release below (off the chain's critical path).
-                    if (NB == 4) update_reversed(m, W, i0, lane);
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&s_done[k & 1]);   // block k is final, buffer k&1 is free
-                    if (NB > 4) update_reversed(m, W, i0, lane);
                     if ((mask >> lane) & 1u) dE_acc += th - yy;   // yy: slack of every site at its own turn
                     n_acc += __popc(mask);
                 }
@@ -936,13 +753,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 // The observables of a slot are read-modify-written by one CTA at a time; a last counter barrier
                 // orders this final flush behind the flush of whoever left the slot at an earlier event.
                 asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(d.gen + e) : "memory");
-                const unsigned target = (unsigned)d.n_rep * (unsigned)(event + 1);
-                unsigned g = 0u, spins = 0u;
-                while (true) {
-                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(g) : "l"(d.gen + e) : "memory");
-                    if (g >= target) break;
-                    if (++spins > (1u << 22)) __trap();
-                }
+                wait_arrivals(d.gen + e, (unsigned)d.n_rep * (unsigned)(event + 1), d.err);
             }
             oa.flush(d.obs + (size_t)e * d.n_rep + t);
         }
@@ -1108,7 +919,7 @@ inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb) {
 // CTAs of a sweep kernel variant that can be resident on the device at once (0 on error).
 inline int direct_coresident(direct_kernel_t kern, const Dev& d, int device) {
     const size_t smem = direct_smem_bytes(d.L, d.q);
-    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return 0;
+    if (allow_max_dynamic_smem((const void*)kern, DIRECT_STATIC_SMEM) != 0) return 0;
     int per_sm = 0, n_sm = 0, coop = 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, direct_threads(d.L), smem) != cudaSuccess) return 0;
     if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return 0;
@@ -1148,8 +959,7 @@ inline direct_kernel_t select_direct_kernel(const Dev& d, int r_hi, int device, 
 inline int launch_sweep_direct(direct_kernel_t kern, const Dev& d, long long sweep0, int n_sweeps, int swap_mode,
                                int swap_every, int r_hi, cudaStream_t stream) {
     const size_t smem = direct_smem_bytes(d.L, d.q);
-    cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (err != cudaSuccess) return (int)err;
+    cudaError_t err = cudaSuccess;   // (the shared-memory attribute was set once, in direct_coresident)
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(swap_mode == 3 ? d.n_local : d.n_ens * d.n_rep));
     cfg.blockDim = dim3((unsigned)direct_threads(d.L));

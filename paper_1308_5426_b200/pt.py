@@ -22,7 +22,7 @@ SYMBOLS = ["pt_create", "pt_create_ex", "pt_destroy", "pt_sweeps", "pt_energy", 
            "pt_observables", "pt_get_spins", "pt_get_spins_dev", "pt_set_spins", "pt_get_couplings",
            "pt_sweep_counter", "pt_set_variant", "pt_get_variant", "pt_set_stream", "pt_sweeps_async",
            "pt_sync", "pt_last_error", "pt_create_shard", "pt_energy_storage_dev", "pt_swap_external",
-           "pt_get_perm", "pt_measure_peaks"]
+           "pt_get_perm", "pt_measure_peaks", "pt_get_state", "pt_set_state"]
 
 
 class PTError(RuntimeError):
@@ -75,6 +75,8 @@ _lib.pt_get_variant.argtypes = [_vp]
 _lib.pt_set_stream.argtypes = [_vp, _vp]
 _lib.pt_last_error.restype = ctypes.c_char_p
 _lib.pt_measure_peaks.argtypes = [_vp, _i32]
+_lib.pt_get_state.argtypes = [_vp, _vp, _vp, _vp, ctypes.POINTER(_i64)]
+_lib.pt_set_state.argtypes = [_vp, _vp, _vp, _vp, _i64]
 
 PEAK_PATTERNS = ["idp2a", "idp4a", "imad", "prmt", "lop3", "prmt+2idp2a (idp2a counted)", "lop3+2idp2a (idp2a counted)",
                  "lds128 (bytes)", "prmt+4idp2a (idp2a counted)", "2prmt+add+2idp2a (idp2a counted)"]
@@ -203,6 +205,24 @@ class PT:
             raise ValueError("spins must have n_ens*n_rep*L entries")
         _check(_lib.pt_set_spins(self._h, _p(s)))
 
+    def get_state(self):
+        """pt_get_state: (spins uint8 [n_ens, n_rep, L], E int64 [n_ens, n_rep], obs raw ctypes array, sweep)."""
+        s = np.zeros((self.n_ens, self.n_rep, self.L), dtype=np.uint8)
+        E = np.zeros((self.n_ens, self.n_rep), dtype=np.int64)
+        obs = (Obs * (self.n_ens * self.n_rep))()
+        sw = _i64(0)
+        _check(_lib.pt_get_state(self._h, _p(s), _p(E), ctypes.byref(obs), ctypes.byref(sw)))
+        return s, E, obs, sw.value
+
+    def set_state(self, spins, E=None, obs=None, sweep=0):
+        """pt_set_state: E None -> recount from the spins; obs None -> keep the accumulators."""
+        s = np.ascontiguousarray(spins, dtype=np.uint8)
+        if s.size != self.n_ens * self.n_rep * self.L:
+            raise ValueError("spins must have n_ens*n_rep*L entries")
+        Ea = None if E is None else np.ascontiguousarray(E, dtype=np.int64)
+        _check(_lib.pt_set_state(self._h, _p(s), None if Ea is None else _p(Ea),
+                                 None if obs is None else ctypes.byref(obs), int(sweep)))
+
     def get_couplings(self):
         J = np.zeros(self.L, dtype=np.int32)
         _check(_lib.pt_get_couplings(self._h, _p(J)))
@@ -228,5 +248,3 @@ class PT:
         self.set_stream(s.cuda_stream)
         return s
 
-
-from .pt_math import cumulants, derived, obs_diff  # noqa: E402,F401  (pure-Python reporting helpers)

