@@ -67,7 +67,14 @@ typedef enum {
  * policy of the direct variant (0: one launch per swap interval; 1, default: persistent launches with the swap events
  * inside the kernel for contexts that take at least a third of the SMs; 2: whenever all replicas can be co-resident);
  * PT_MINB=1|2 forces the 168- or the 80-register build of the direct sweep kernel (experiments; default: by size). */
-enum { PT_VARIANT_AUTO = 0, PT_VARIANT_FIELD = 1, PT_VARIANT_DIRECT = 2 };
+enum { PT_VARIANT_AUTO = 0, PT_VARIANT_FIELD = 1, PT_VARIANT_DIRECT = 2, PT_VARIANT_FP32 = 3, PT_VARIANT_FP64 = 4 };
+/* PT_VARIANT_FP32 / PT_VARIANT_FP64: the paper's own arithmetic as a COMPARISON variant ("single
+ * precision ... rounding errors"; :110-124: one thread block per replica, each of its 128 threads sums a subset of the
+ * pair terms of dE, then a tree reduction; :216 "double precision ... about half the speed").  Same quantised model
+ * (couplings (T)(Jq[r] 2^-24)), same random streams; dE and the running energy in T = float / double, Eqs. 8-9 in
+ * fp64 on those values.  fp64 reproduces the integer trajectory exactly; fp32 measures what single precision costs.
+ * pt_energy(recompute = 0) returns the running value rounded to fixed point; leaving the variant recounts the
+ * energies exactly.  Never chosen by AUTO; swap events by one launch per swap interval. */
 
 /* Cumulative per-slot accumulators since pt_create (the caller differences two
  * snapshots to discard burn-in).  Sampled after every sweep, before the swap

@@ -20,8 +20,12 @@
 //       states) within 3 sigma, with and without swaps; beta=0 <delta>=1/q;
 //       field mode == direct mode bit for bit; call-splitting invariance;
 //       threaded == single-threaded
+//   orc_sweeps_arith (the paper's floating-point arithmetic as a comparison mode):
+//       fp64 mode reproduces the integer trajectory bit for bit (the couplings Jq 2^-24 have 25 significant
+//       bits, so every fp64 sum is exact); fp32 mode: dE within the summation error bound of the exact
+//       integer value, <E> of the L=8 enumeration within 3 sigma
 //   the paper's fp32 error figures and its speedups:
-//       PARITY UNPINNED (context only; nothing here computes them)
+//       PARITY UNPINNED (context only; the fp32 mode MEASURES the rounding error of this build's model)
 //
 // Arithmetic: couplings evaluated in long double, quantised to int32 at scale
 // 2^24 (A16); every dE and E is an exact integer; acceptance in fp64.
@@ -128,6 +132,7 @@ struct Obs {              // same field order as include/pt.h's pt_obs (declared
 struct Replica {
     std::vector<uint8_t> c;     // colours 0..q-1 (A4)
     int64_t E = 0;              // total energy, fixed point 2^24 (A13)
+    double Ef = 0.0;            // floating-point modes: running energy in units of 1 (fp32 mode: a float value)
     std::vector<int64_t> h;     // field mode only: h[i*q+k] = sum_{j!=i} Jq[|i-j|] [c_j==k]
 };
 
@@ -142,6 +147,7 @@ struct Ctx {
     std::vector<Replica> rep;   // [ens*n_rep + slot]
     std::vector<Obs> obs;       // [ens*n_rep + slot]
     int64_t sweep = 0;          // global sweep counter (A10)
+    int float_mode = 0;         // 0: exact integers; 1 / 2: the fp32 / fp64 comparison mode has been entered
 };
 
 inline int iabs(int x) { return x < 0 ? -x : x; }
@@ -207,6 +213,86 @@ void metropolis_cycle(Ctx& C, int e, int t, bool field) {
                     R.h[(size_t)j * q + a] -= J;
                     R.h[(size_t)j * q + b] += J;
                 }
+            }
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------
+// The paper's own arithmetic as a comparison mode ("single precision ... rounding errors";
+// :118-124 and the caption of Listing 2: "each thread sums a subset of pair terms", then a parallel reduction).
+// Reading: couplings Jf[r] = (T)(Jq[r] 2^-24), i.e. the SAME quantised model in type T = float or
+// double; dE = sum of the 128 thread-partial sums, thread t adding its terms j = t, t+128, ... in increasing j,
+// combined by a binary tree (stride 64, 32, .., 1); the terms are +-Jf or 0, so no product is rounded.  The running
+// energy is kept in T; Eq. 8 and Eq. 9 are evaluated in fp64 on the T values (libm's expf is not involved).
+// ---------------------------------------------------------------------------
+template <typename T>
+T delta_e_float(const Ctx& C, const std::vector<T>& Jf, const std::vector<uint8_t>& c, int i, int a, int b) {
+    T part[128];
+    for (int t = 0; t < 128; ++t) {
+        T acc = (T)0;
+        for (int j = t; j < C.L; j += 128) {
+            if (j == i) continue;
+            const T J = Jf[iabs(i - j)];
+            if (c[j] == a) acc = acc + J;
+            else if (c[j] == b) acc = acc - J;
+        }
+        part[t] = acc;
+    }
+    for (int s = 64; s >= 1; s >>= 1)
+        for (int t = 0; t < s; ++t) part[t] = part[t] + part[t + s];
+    return part[0];
+}
+
+template <typename T>
+void metropolis_cycle_float(Ctx& C, const std::vector<T>& Jf, int e, int t) {
+    Replica& R = C.rep[(size_t)e * C.n_rep + t];
+    Obs& O = C.obs[(size_t)e * C.n_rep + t];
+    const double beta = C.beta[t];
+    const int q = C.q, L = C.L;
+    T E = (T)R.Ef;
+    for (int i = 0; i < L; ++i) {
+        const uint32_t ctr[4] = {(uint32_t)i, (uint32_t)C.sweep, (uint32_t)t,
+                                 ((uint32_t)(C.ens_base + e) << 4) | TAG_SWEEP};
+        uint32_t w[4];
+        philox4x32_10(ctr, C.key, w);
+        const int a = R.c[i];
+        const int k = (int)mulhi32(w[0], (uint32_t)(q - 1));
+        const int b = k + (k >= a);
+        const T dE = delta_e_float<T>(C, Jf, R.c, i, a, b);
+        const double x = -(beta * (double)dE);
+        const double p = (dE <= (T)0) ? 1.0 : exp(x);
+        const double u = uniform53(w[1], w[2]);
+        if (dE > (T)0 && fabs(u - p) < 1e-12) O.near_ties++;
+        O.flip_attempts++;
+        if (dE <= (T)0 || u < p) {
+            R.c[i] = (uint8_t)b;
+            E = E + dE;
+            O.flip_accepts++;
+        }
+    }
+    R.Ef = (double)E;
+    R.E = llrint(ldexp(R.Ef, 24));   // what the accumulators see: the running value in fixed point
+}
+
+void swap_event_float(Ctx& C, int e) {
+    for (int stage = 0; stage < 2; ++stage) {
+        for (int t = stage; t + 1 < C.n_rep; t += 2) {
+            Replica& Ra = C.rep[(size_t)e * C.n_rep + t];
+            Replica& Rb = C.rep[(size_t)e * C.n_rep + t + 1];
+            Obs& O = C.obs[(size_t)e * C.n_rep + t];
+            const double d = (C.beta[t] - C.beta[t + 1]) * (Ra.Ef - Rb.Ef);
+            const uint32_t ctr[4] = {(uint32_t)t, (uint32_t)C.sweep, 0u, ((uint32_t)(C.ens_base + e) << 4) | TAG_SWAP};
+            uint32_t w[4];
+            philox4x32_10(ctr, C.key, w);
+            const double u = uniform53(w[1], w[2]);
+            O.swap_attempts++;
+            if (d < 0 && fabs(u - exp(d)) < 1e-12) O.near_ties++;
+            if (d >= 0 || u < exp(d)) {
+                std::swap(Ra.c, Rb.c);
+                std::swap(Ra.E, Rb.E);
+                std::swap(Ra.Ef, Rb.Ef);
+                O.swap_accepts++;
             }
         }
     }
@@ -278,6 +364,37 @@ void swap_event(Ctx& C, int e) {
             }
         }
     }
+}
+
+// Floating-point comparison modes: arith = 1 (fp32) or 2 (fp64).  A context is used in ONE mode from creation (or
+// from a point where its running energies are exact: the first call converts E to the floating type).
+template <typename T>
+int sweeps_float(Ctx& C, int64_t n, int swap_every, int n_threads, bool first) {
+    const int R = C.n_ens * C.n_rep;
+    std::vector<T> Jf(C.L);
+    for (int r = 0; r < C.L; ++r) Jf[r] = (T)ldexp((double)C.Jq[r], -24);
+    if (first)
+        for (int x = 0; x < R; ++x) C.rep[x].Ef = (double)(T)ldexp((double)C.rep[x].E, -24);
+    if (n_threads < 1) n_threads = 1;
+    if (n_threads > R) n_threads = R;
+    for (int64_t s = 0; s < n; ++s) {
+        C.sweep += 1;
+        auto work = [&](int tid) {
+            for (int x = tid; x < R; x += n_threads) {
+                metropolis_cycle_float<T>(C, Jf, x / C.n_rep, x % C.n_rep);
+                measure(C, x / C.n_rep, x % C.n_rep);
+            }
+        };
+        if (n_threads == 1) work(0);
+        else {
+            std::vector<std::thread> th;
+            for (int t = 0; t < n_threads; ++t) th.emplace_back(work, t);
+            for (auto& t : th) t.join();
+        }
+        if (swap_every > 0 && C.sweep % swap_every == 0)
+            for (int e = 0; e < C.n_ens; ++e) swap_event_float(C, e);
+    }
+    return 0;
 }
 
 }  // namespace
@@ -383,6 +500,30 @@ int orc_sweeps(void* hh, int64_t n, int swap_every, int field, int n_threads) {
     if (field)
         for (int x = 0; x < R; ++x) { C.rep[x].h.clear(); C.rep[x].h.shrink_to_fit(); }
     return 0;
+}
+
+int orc_sweeps_arith(void* hh, int64_t n, int swap_every, int arith, int n_threads) {
+    Ctx& C = *(Ctx*)hh;
+    if (n < 0 || swap_every < 0 || (arith != 1 && arith != 2)) return -1;
+    const bool first = C.float_mode == 0;
+    if (!first && C.float_mode != arith) return -1;
+    C.float_mode = arith;
+    return arith == 1 ? sweeps_float<float>(C, n, swap_every, n_threads, first)
+                      : sweeps_float<double>(C, n, swap_every, n_threads, first);
+}
+
+// dE of changing site i of (ens, slot) to colour b_api in the floating-point mode arith (1 fp32, 2 fp64), as a double.
+double orc_delta_e_arith(void* hh, int ens, int slot, int i, int b_api, int arith) {
+    Ctx& C = *(Ctx*)hh;
+    const Replica& R = C.rep[(size_t)ens * C.n_rep + slot];
+    if (arith == 1) {
+        std::vector<float> Jf(C.L);
+        for (int r = 0; r < C.L; ++r) Jf[r] = (float)ldexp((double)C.Jq[r], -24);
+        return (double)delta_e_float<float>(C, Jf, R.c, i, R.c[i], b_api - 1);
+    }
+    std::vector<double> Jf(C.L);
+    for (int r = 0; r < C.L; ++r) Jf[r] = ldexp((double)C.Jq[r], -24);
+    return delta_e_float<double>(C, Jf, R.c, i, R.c[i], b_api - 1);
 }
 
 int orc_energy(void* hh, int64_t* E_out, int recompute) {

@@ -60,6 +60,9 @@ def lib():
         L.orc_destroy.argtypes = [vp]
         L.orc_destroy.restype = None
         L.orc_sweeps.argtypes = [vp, i64, i32, i32, i32]
+        L.orc_sweeps_arith.argtypes = [vp, i64, i32, i32, i32]
+        L.orc_delta_e_arith.argtypes = [vp, i32, i32, i32, i32, i32]
+        L.orc_delta_e_arith.restype = dbl
         L.orc_energy.argtypes = [vp, vp, i32]
         L.orc_observables.argtypes = [vp, vp]
         L.orc_get_spins.argtypes = [vp, vp]
@@ -126,6 +129,15 @@ class Oracle:
         rc = lib().orc_sweeps(self._h, int(n), int(swap_every), int(bool(field)), int(threads))
         if rc:
             raise ValueError("orc_sweeps: invalid arguments")
+
+    def sweeps_arith(self, n, swap_every=1, arith="fp32", threads=1):
+        """The paper's floating-point arithmetic as a comparison mode (fp32 or fp64 sums of dE)."""
+        rc = lib().orc_sweeps_arith(self._h, int(n), int(swap_every), {"fp32": 1, "fp64": 2}[arith], int(threads))
+        if rc:
+            raise ValueError("orc_sweeps_arith: invalid arguments (or the context is in the other mode)")
+
+    def delta_e_arith(self, ens, slot, i, b, arith):
+        return lib().orc_delta_e_arith(self._h, ens, slot, i, b, {"fp32": 1, "fp64": 2}[arith])
 
     def energy(self, recompute=False):
         E = np.zeros((self.n_ens, self.n_rep), dtype=np.int64)

@@ -19,6 +19,7 @@
 #include "pt_sweep_direct.cuh"
 #include "pt_sweep_field.cuh"
 #include "pt_peaks.cuh"
+#include "pt_sweep_float.cuh"
 
 namespace {
 
@@ -85,6 +86,8 @@ struct pt_ctx {
     long long* d_Epub = nullptr;
     uint8_t* d_stage = nullptr;   // [R*L] one byte per spin: staging for pt_get_spins / pt_set_spins / pt_set_state
     uint8_t* h_stage = nullptr;   // pinned host bounce buffer of the same size
+    double* d_Ef = nullptr;  // floating-point comparison variants: running energies in units of 1, storage order
+    bool ef_valid = false;   // d_Ef continues the running energies (else it is set from d_E at the next float launch)
     int* h_err = nullptr;    // pinned, device-mapped flag: an in-kernel barrier timed out
     int* d_err = nullptr;    // its device address
     int coresident = -1;   // direct variant: CTAs that fit on the device at once (-1: not asked yet)
@@ -115,6 +118,7 @@ void free_ctx(pt_ctx* c) {
     cudaFree(c->d_perm); cudaFree(c->d_obs); cudaFree(c->d_h); cudaFree(c->d_done); cudaFree(c->d_flag); cudaFree(c->d_dbg); cudaFree(c->d_gen); cudaFree(c->d_Epub);
     if (c->h_err) cudaFreeHost(c->h_err);
     cudaFree(c->d_stage);
+    cudaFree(c->d_Ef);
     if (c->h_stage) cudaFreeHost(c->h_stage);
     delete c;
 }
@@ -153,6 +157,9 @@ int resolve_variant(int L, int q, long long rowsum, int variant, int* out) {
                                    "and sum_r Jq[r] < 2^30 - 1");
     } else if (variant == PT_VARIANT_FIELD) {
         if (!field_fits(L, q)) return fail(PT_ECAPACITY, "local-field table (L*q*4 bytes) does not fit in shared memory");
+    } else if (variant == PT_VARIANT_FP32 || variant == PT_VARIANT_FP64) {
+        const size_t smem = variant == PT_VARIANT_FP32 ? ptk::float_smem_bytes<float>(L) : ptk::float_smem_bytes<double>(L);
+        if (smem + 2048 > kSmemLimit) return fail(PT_ECAPACITY, "couplings and uniforms (L*14 or L*18 bytes) do not fit in shared memory");
     } else {
         return fail(PT_EINVAL, "unknown variant");
     }
@@ -168,7 +175,26 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
         if (rc) return rc;
     }
     const ptk::Dev d = c->dev();  // after ensure_fields: it may allocate d_h
-    if (c->variant == PT_VARIANT_FIELD) {
+    if (c->variant == PT_VARIANT_FP32 || c->variant == PT_VARIANT_FP64) {
+        const bool f32 = c->variant == PT_VARIANT_FP32;
+        if (!c->d_Ef) PT_CUDA(cudaMalloc(&c->d_Ef, (size_t)c->R() * sizeof(double)));
+        if (!c->ef_valid) {   // entering the variant: the running energies are exact integers
+            if (f32) ptk::energy_to_float_kernel<float><<<(c->R() + 255) / 256, 256, 0, c->stream>>>(d, c->d_Ef);
+            else ptk::energy_to_float_kernel<double><<<(c->R() + 255) / 256, 256, 0, c->stream>>>(d, c->d_Ef);
+            PT_CUDA(cudaGetLastError());
+            c->ef_valid = true;
+        }
+        c->fields_valid = false;
+        if (f32) {
+            PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::sweep_float_kernel<float>, 2048));
+            ptk::sweep_float_kernel<float><<<c->R(), ptk::FLOAT_THREADS, ptk::float_smem_bytes<float>(c->L), c->stream>>>(
+                d, c->d_Ef, (long long)c->sweep, n_sweeps, swap_mode == 1 ? 1 : 0);
+        } else {
+            PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::sweep_float_kernel<double>, 2048));
+            ptk::sweep_float_kernel<double><<<c->R(), ptk::FLOAT_THREADS, ptk::float_smem_bytes<double>(c->L), c->stream>>>(
+                d, c->d_Ef, (long long)c->sweep, n_sweeps, swap_mode == 1 ? 1 : 0);
+        }
+    } else if (c->variant == PT_VARIANT_FIELD) {
         const size_t smem = ptk::field_smem_bytes(c->L, c->q);
         PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::sweep_field_kernel, 1024));
         ptk::sweep_field_kernel<<<c->R(), ptk::FIELD_THREADS, smem, c->stream>>>(d, (long long)c->sweep, n_sweeps,
@@ -470,6 +496,7 @@ int upload_spins(pt_ctx* c, const uint8_t* in) {
     ptk::pack_spins_kernel<<<(unsigned)((nwords + 255) / 256), 256, 0, c->stream>>>(c->dev(), c->d_stage);
     PT_CUDA(cudaGetLastError());
     c->fields_valid = false;
+    c->ef_valid = false;
     return PT_OK;
 }
 }  // namespace
@@ -619,9 +646,20 @@ int pt_measure_peaks(double* rates, int n) {
 int pt_set_variant(pt_ctx* c, int variant) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");
     if (c->n_local && variant == PT_VARIANT_FIELD) return fail(PT_EINVAL, "slot-sharded contexts need the direct variant");
+    const bool to_float = variant == PT_VARIANT_FP32 || variant == PT_VARIANT_FP64;
+    if (c->n_local && to_float) return fail(PT_EINVAL, "slot-sharded contexts need the direct variant");
+    DeviceGuard guard(c->device);
     int v = 0;
     int rc = resolve_variant(c->L, c->q, c->rowsum, variant, &v);
     if (rc) return rc;
+    const bool from_float = c->variant == PT_VARIANT_FP32 || c->variant == PT_VARIANT_FP64;
+    if (from_float && v != c->variant) {
+        // the floating-point running energies carry rounding errors: the exact variants restart from the recount
+        // (a change between fp32 and fp64 re-enters from the exact energies as well)
+        c->ef_valid = false;
+        rc = recompute_energy(c, c->d_E);
+        if (rc) return rc;
+    }
     c->variant = v;
     return PT_OK;
 }

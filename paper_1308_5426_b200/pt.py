@@ -13,8 +13,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpt.so")
 
-VARIANT_AUTO, VARIANT_FIELD, VARIANT_DIRECT = 0, 1, 2
-_VARIANTS = {"auto": VARIANT_AUTO, "field": VARIANT_FIELD, "direct": VARIANT_DIRECT}
+VARIANT_AUTO, VARIANT_FIELD, VARIANT_DIRECT, VARIANT_FP32, VARIANT_FP64 = 0, 1, 2, 3, 4
+_VARIANTS = {"auto": VARIANT_AUTO, "field": VARIANT_FIELD, "direct": VARIANT_DIRECT, "fp32": VARIANT_FP32,
+             "fp64": VARIANT_FP64}
 STATUS = {0: "PT_OK", -1: "PT_EINVAL", -2: "PT_EOVERFLOW", -3: "PT_ENOMEM", -4: "PT_ECUDA", -5: "PT_ECAPACITY"}
 
 # every symbol include/pt.h declares
@@ -236,7 +237,7 @@ class PT:
 
     def get_variant(self):
         v = _lib.pt_get_variant(self._h)
-        return {VARIANT_FIELD: "field", VARIANT_DIRECT: "direct"}.get(v, str(v))
+        return {VARIANT_FIELD: "field", VARIANT_DIRECT: "direct", VARIANT_FP32: "fp32", VARIANT_FP64: "fp64"}.get(v, str(v))
 
     def set_stream(self, cuda_stream_ptr):
         _check(_lib.pt_set_stream(self._h, ctypes.c_void_p(int(cuda_stream_ptr) if cuda_stream_ptr else None)))
