@@ -202,6 +202,15 @@ int64_t pt_sweep_counter(pt_ctx* ctx);
 int pt_set_variant(pt_ctx* ctx, int variant);
 int pt_get_variant(pt_ctx* ctx); /* the variant that pt_sweeps runs (FIELD or DIRECT) */
 
+/* Site order of a sweep (reading A5 of DESIGN.md).  PT_ORDER_SEQUENTIAL (default, BASELINE configs): sites 0..L-1
+ * in order.  PT_ORDER_RANDOM ("L Metropolis steps ... an average of one Monte Carlo step per
+ * spin"): step n = 0..L-1 of a sweep visits site mulhi32(w3, L) of the Philox draw keyed by (n, sweep, slot), which
+ * also gives the proposal and the uniform of the step.  Random order runs in the field variant (it is selected by
+ * this call; PT_ECAPACITY if the local-field table and the step lists do not fit in shared memory; pt_set_variant
+ * to another variant is refused while it is on).  Errors: PT_EINVAL, PT_ECAPACITY. */
+enum { PT_ORDER_SEQUENTIAL = 0, PT_ORDER_RANDOM = 1 };
+int pt_set_site_order(pt_ctx* ctx, int order);
+
 /* Kernels are launched on `cuda_stream` (a cudaStream_t; NULL = default stream). */
 int pt_set_stream(pt_ctx* ctx, void* cuda_stream);
 

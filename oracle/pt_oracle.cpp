@@ -147,6 +147,7 @@ struct Ctx {
     std::vector<Replica> rep;   // [ens*n_rep + slot]
     std::vector<Obs> obs;       // [ens*n_rep + slot]
     int64_t sweep = 0;          // global sweep counter (A10)
+    int site_order = 0;         // 0: sites 0..L-1 in order (A5); 1: step n visits site mulhi32(w3, L) (A5')
     int float_mode = 0;         // 0: exact integers; 1 / 2: the fp32 / fp64 comparison mode has been entered
 };
 
@@ -186,11 +187,14 @@ void metropolis_cycle(Ctx& C, int e, int t, bool field) {
     Obs& O = C.obs[(size_t)e * C.n_rep + t];
     const double beta = C.beta[t];
     const int q = C.q, L = C.L;
-    for (int i = 0; i < L; ++i) {
-        const uint32_t ctr[4] = {(uint32_t)i, (uint32_t)C.sweep, (uint32_t)t,
+    for (int n = 0; n < L; ++n) {                         // step n of the cycle
+        const uint32_t ctr[4] = {(uint32_t)n, (uint32_t)C.sweep, (uint32_t)t,
                                  ((uint32_t)(C.ens_base + e) << 4) | TAG_SWEEP};
         uint32_t w[4];
         philox4x32_10(ctr, C.key, w);
+        // A5: sequential order visits site n; A5' ("an average of one Monte Carlo step per spin"):
+        // a site drawn uniformly from the same Philox word group
+        const int i = C.site_order ? (int)mulhi32(w[3], (uint32_t)L) : n;
         const int a = R.c[i];
         const int k = (int)mulhi32(w[0], (uint32_t)(q - 1));
         const int b = k + (k >= a);                       // A6: uniform over the other q-1
@@ -567,6 +571,13 @@ int orc_get_couplings(void* hh, int32_t* Jq) {
 }
 
 int64_t orc_sweep_counter(void* hh) { return ((Ctx*)hh)->sweep; }
+
+// 0: sequential site order (default), 1: random sites.  The floating-point comparison modes are sequential only.
+int orc_set_site_order(void* hh, int order) {
+    if (order != 0 && order != 1) return -1;
+    ((Ctx*)hh)->site_order = order;
+    return 0;
+}
 
 // dE of changing site i of (ens, slot) to colour b_api (1..q), by the direct sum.
 int64_t orc_delta_e(void* hh, int ens, int slot, int i, int b_api) {

@@ -69,6 +69,7 @@ def lib():
         L.orc_set_spins.argtypes = [vp, vp]
         L.orc_get_couplings.argtypes = [vp, vp]
         L.orc_sweep_counter.argtypes = [vp]
+        L.orc_set_site_order.argtypes = [vp, i32]
         L.orc_sweep_counter.restype = i64
         L.orc_delta_e.argtypes = [vp, i32, i32, i32, i32]
         L.orc_delta_e.restype = i64
@@ -129,6 +130,10 @@ class Oracle:
         rc = lib().orc_sweeps(self._h, int(n), int(swap_every), int(bool(field)), int(threads))
         if rc:
             raise ValueError("orc_sweeps: invalid arguments")
+
+    def set_site_order(self, order):
+        if lib().orc_set_site_order(self._h, {"sequential": 0, "random": 1}[order]):
+            raise ValueError("orc_set_site_order: invalid order")
 
     def sweeps_arith(self, n, swap_every=1, arith="fp32", threads=1):
         """The paper's floating-point arithmetic as a comparison mode (fp32 or fp64 sums of dE)."""

@@ -86,6 +86,7 @@ struct pt_ctx {
     long long* d_Epub = nullptr;
     uint8_t* d_stage = nullptr;   // [R*L] one byte per spin: staging for pt_get_spins / pt_set_spins / pt_set_state
     uint8_t* h_stage = nullptr;   // pinned host bounce buffer of the same size
+    int site_order = 0;      // PT_ORDER_SEQUENTIAL | PT_ORDER_RANDOM (field variant only)
     double* d_Ef = nullptr;  // floating-point comparison variants: running energies in units of 1, storage order
     bool ef_valid = false;   // d_Ef continues the running energies (else it is set from d_E at the next float launch)
     int* h_err = nullptr;    // pinned, device-mapped flag: an in-kernel barrier timed out
@@ -195,10 +196,16 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
                 d, c->d_Ef, (long long)c->sweep, n_sweeps, swap_mode == 1 ? 1 : 0);
         }
     } else if (c->variant == PT_VARIANT_FIELD) {
-        const size_t smem = ptk::field_smem_bytes(c->L, c->q);
-        PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::sweep_field_kernel, 1024));
-        ptk::sweep_field_kernel<<<c->R(), ptk::FIELD_THREADS, smem, c->stream>>>(d, (long long)c->sweep, n_sweeps,
-                                                                                 swap_mode == 1 ? 1 : 0);
+        const size_t smem = ptk::field_smem_bytes(c->L, c->q, c->site_order == PT_ORDER_RANDOM);
+        if (c->site_order == PT_ORDER_RANDOM) {
+            PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::sweep_field_kernel<true>, 1024));
+            ptk::sweep_field_kernel<true><<<c->R(), ptk::FIELD_THREADS, smem, c->stream>>>(d, (long long)c->sweep, n_sweeps,
+                                                                                           swap_mode == 1 ? 1 : 0);
+        } else {
+            PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::sweep_field_kernel<false>, 1024));
+            ptk::sweep_field_kernel<false><<<c->R(), ptk::FIELD_THREADS, smem, c->stream>>>(d, (long long)c->sweep, n_sweeps,
+                                                                                            swap_mode == 1 ? 1 : 0);
+        }
     } else {
         c->fields_valid = false;
         if (!c->direct_kern) c->direct_kern = ptk::select_direct_kernel(d, c->r_hi, c->device, &c->coresident);
@@ -646,6 +653,8 @@ int pt_measure_peaks(double* rates, int n) {
 int pt_set_variant(pt_ctx* c, int variant) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");
     if (c->n_local && variant == PT_VARIANT_FIELD) return fail(PT_EINVAL, "slot-sharded contexts need the direct variant");
+    if (c->site_order == PT_ORDER_RANDOM && variant != PT_VARIANT_FIELD)
+        return fail(PT_EINVAL, "random site order runs in the field variant only");
     const bool to_float = variant == PT_VARIANT_FP32 || variant == PT_VARIANT_FP64;
     if (c->n_local && to_float) return fail(PT_EINVAL, "slot-sharded contexts need the direct variant");
     DeviceGuard guard(c->device);
@@ -665,6 +674,20 @@ int pt_set_variant(pt_ctx* c, int variant) {
 }
 
 int pt_get_variant(pt_ctx* c) { return c ? c->variant : PT_EINVAL; }
+
+int pt_set_site_order(pt_ctx* c, int order) {
+    if (!c) return fail(PT_EINVAL, "ctx is NULL");
+    if (order != PT_ORDER_SEQUENTIAL && order != PT_ORDER_RANDOM) return fail(PT_EINVAL, "unknown site order");
+    if (order == PT_ORDER_RANDOM) {
+        if (c->n_local) return fail(PT_EINVAL, "slot-sharded contexts sweep in sequential order");
+        if (ptk::field_smem_bytes(c->L, c->q, true) + 256 > kSmemLimit)
+            return fail(PT_ECAPACITY, "local-field table and step lists do not fit in shared memory");
+        int rc = pt_set_variant(c, PT_VARIANT_FIELD);   // (leaving a floating-point variant recounts the energies)
+        if (rc) return rc;
+    }
+    c->site_order = order;
+    return PT_OK;
+}
 
 int pt_set_stream(pt_ctx* c, void* cuda_stream) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");

@@ -23,11 +23,19 @@ namespace ptk {
 
 constexpr int FIELD_THREADS = 512;
 
+// RANDOM (site order of reading A5': "L Metropolis steps ... an average of one Monte Carlo step per spin",
+// PAPER.md:112-114): step n of a sweep visits site mulhi32(w3, L) of the Philox draw keyed by (n, sweep, slot); the
+// same draw gives the proposal (w0) and the uniform (w1, w2).  A site can be visited twice in a sweep, so the old
+// colour a -- and with it the proposed colour k + (k >= a) -- is read at the step's turn, not at the start of the
+// sweep; the scan over 32 consecutive STEPS is otherwise the same: the first accepting step is the next change.
+//
 // dynamic smem layout (32-bit words): J[L] | theta[L] | sp[W] | bq[W] | h[q*L]
-__host__ __device__ inline size_t field_smem_bytes(int L, int q) {
-    return (size_t)(2 * L + 2 * (L / 8) + q * L) * 4;
+//                            RANDOM: J[L] | theta[L] | sp[W] | site[L] | kk[L/4] | h[q*L]
+__host__ __device__ inline size_t field_smem_bytes(int L, int q, bool random_order = false) {
+    return (size_t)(2 * L + (L / 8) + (random_order ? L + L / 4 : L / 8) + q * L) * 4;
 }
 
+template <bool RANDOM>
 __global__ void __launch_bounds__(FIELD_THREADS, 1)
 sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
     extern __shared__ uint32_t smem_f[];
@@ -35,9 +43,11 @@ sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
     int32_t* J = (int32_t*)smem_f;
     int32_t* theta = J + L;
     uint32_t* sp = (uint32_t*)(theta + L);
-    uint32_t* bq = sp + W;
-    int32_t* h = (int32_t*)(bq + W);
-    __shared__ int s_flip[4];
+    uint32_t* bq = sp + W;                                  // sequential order: proposed colours, packed
+    int32_t* site = (int32_t*)(sp + W);                     // RANDOM: site of step n ...
+    uint8_t* kk = (uint8_t*)(site + L);                     // ... and its draw k in 0..q-2
+    int32_t* h = RANDOM ? (int32_t*)(kk + L) : (int32_t*)(bq + W);
+    __shared__ int s_flip[5];
     __shared__ int s_cnt[16];
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -58,8 +68,16 @@ sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
 
     for (int s = 0; s < n_sweeps; ++s) {
         const uint32_t sweep = (uint32_t)(sweep0 + s + 1);
+        if (RANDOM) {
+            for (int n = tid; n < L; n += FIELD_THREADS) {
+                const Philox4 p = philox4x32_10((uint32_t)n, sweep, (uint32_t)t, c3, d.key0, d.key1);
+                site[n] = (int32_t)__umulhi(p.w3, (uint32_t)L);
+                kk[n] = (uint8_t)__umulhi(p.w0, (uint32_t)(q - 1));
+                theta[n] = accept_threshold(uniform53(p.w1, p.w2), scale);
+            }
+        }
         // proposals and thresholds of all sites (A6, A7, A9), one word of 8 sites per thread
-        for (int w = tid; w < W; w += FIELD_THREADS) {
+        for (int w = tid; !RANDOM && w < W; w += FIELD_THREADS) {
             const uint32_t word = sp[w];
             uint32_t bword = 0;
 #pragma unroll
@@ -79,44 +97,47 @@ sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
         int pos = 0;
         while (true) {
             if (warp == 0) {
-                int f = L, fa = 0, fb = 0, fdE = 0;
+                int f = L, fi = 0, fa = 0, fb = 0, fdE = 0;
                 for (int base = pos; base < L; base += 32) {
-                    const int i = base + lane;
-                    int a = 0, b = 0, dE = 0;
+                    const int n = base + lane;     // step; sequential order: step n visits site n
+                    int i = n, a = 0, b = 0, dE = 0;
                     bool acc = false;
-                    if (i < L) {
+                    if (n < L) {
+                        if (RANDOM) i = site[n];
                         a = get_nibble(sp, i);
-                        b = get_nibble(bq, i);
+                        if (RANDOM) { const int k = kk[n]; b = k + (k >= a ? 1 : 0); }
+                        else b = get_nibble(bq, i);
                         dE = h[a * L + i] - h[b * L + i];
-                        acc = dE <= theta[i];
+                        acc = dE <= theta[n];
                     }
                     const unsigned m = __ballot_sync(0xffffffffu, acc);
                     if (m) {
                         const int src = __ffs(m) - 1;
                         f = base + src;
+                        fi = __shfl_sync(0xffffffffu, i, src);
                         fa = __shfl_sync(0xffffffffu, a, src);
                         fb = __shfl_sync(0xffffffffu, b, src);
                         fdE = __shfl_sync(0xffffffffu, dE, src);
                         break;
                     }
                 }
-                if (lane == 0) { s_flip[0] = f; s_flip[1] = fa; s_flip[2] = fb; s_flip[3] = fdE; }
+                if (lane == 0) { s_flip[0] = f; s_flip[1] = fa; s_flip[2] = fb; s_flip[3] = fdE; s_flip[4] = fi; }
             }
             __syncthreads();
             const int f = s_flip[0];
             if (f >= L) break;
-            const int a = s_flip[1], b = s_flip[2];
+            const int a = s_flip[1], b = s_flip[2], fs = s_flip[4];   // fs: the site of step f
             int32_t* ha = h + a * L;
             int32_t* hb = h + b * L;
             for (int j = tid; j < L; j += FIELD_THREADS) {
-                const int dist = j > f ? j - f : f - j;
+                const int dist = j > fs ? j - fs : fs - j;
                 const int32_t Jv = J[dist];  // J[0] = 0: the site's own field is unchanged
                 ha[j] -= Jv;
                 hb[j] += Jv;
             }
             if (tid == 0) {
-                const int sh = (f & 7) << 2;
-                sp[f >> 3] = (sp[f >> 3] & ~(15u << sh)) | ((uint32_t)b << sh);
+                const int sh = (fs & 7) << 2;
+                sp[fs >> 3] = (sp[fs >> 3] & ~(15u << sh)) | ((uint32_t)b << sh);
                 E += s_flip[3];
                 oa.acc += 1;
             }

@@ -23,7 +23,7 @@ SYMBOLS = ["pt_create", "pt_create_ex", "pt_destroy", "pt_sweeps", "pt_energy", 
            "pt_observables", "pt_get_spins", "pt_get_spins_dev", "pt_set_spins", "pt_get_couplings",
            "pt_sweep_counter", "pt_set_variant", "pt_get_variant", "pt_set_stream", "pt_sweeps_async",
            "pt_sync", "pt_last_error", "pt_create_shard", "pt_energy_storage_dev", "pt_swap_external",
-           "pt_get_perm", "pt_measure_peaks", "pt_get_state", "pt_set_state"]
+           "pt_get_perm", "pt_measure_peaks", "pt_get_state", "pt_set_state", "pt_set_site_order"]
 
 
 class PTError(RuntimeError):
@@ -78,6 +78,7 @@ _lib.pt_last_error.restype = ctypes.c_char_p
 _lib.pt_measure_peaks.argtypes = [_vp, _i32]
 _lib.pt_get_state.argtypes = [_vp, _vp, _vp, _vp, ctypes.POINTER(_i64)]
 _lib.pt_set_state.argtypes = [_vp, _vp, _vp, _vp, _i64]
+_lib.pt_set_site_order.argtypes = [_vp, _i32]
 
 PEAK_PATTERNS = ["idp2a", "idp4a", "imad", "prmt", "lop3", "prmt+2idp2a (idp2a counted)", "lop3+2idp2a (idp2a counted)",
                  "lds128 (bytes)", "prmt+4idp2a (idp2a counted)", "2prmt+add+2idp2a (idp2a counted)"]
@@ -234,6 +235,10 @@ class PT:
 
     def set_variant(self, variant):
         _check(_lib.pt_set_variant(self._h, _VARIANTS[variant] if isinstance(variant, str) else int(variant)))
+
+    def set_site_order(self, order):
+        """'sequential' (default) or 'random' (pt_set_site_order; random order selects the field variant)."""
+        _check(_lib.pt_set_site_order(self._h, {"sequential": 0, "random": 1}[order]))
 
     def get_variant(self):
         v = _lib.pt_get_variant(self._h)

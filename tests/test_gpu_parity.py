@@ -654,3 +654,31 @@ def test_floating_point_comparison_variants(pt, oracle, arith):
             np.testing.assert_array_equal(g.energy(), g.energy(recompute=True))
         g.close()
         o.close()
+
+
+def test_random_site_order(pt, oracle):
+    """Reading A5' ("an average of one Monte Carlo step per spin"): step n visits the site drawn from
+    the step's Philox word group; field variant, bit-identical to the oracle; the direct variant refuses."""
+    for (L, q, sigma, n_ens, n_rep, n) in [(64, 3, 0.5, 1, 8, 200), (256, 8, 0.3, 2, 5, 60), (1024, 5, 0.8, 1, 6, 12),
+                                           (200, 12, 0.45, 1, 3, 40)]:
+        b = inputs.geometric_betas(0.6, 2.4, n_rep)
+        g = pt.PT(L, q, sigma, n_ens, n_rep, b, 606)
+        o = oracle.Oracle(L, q, sigma, n_ens, n_rep, b, 606)
+        g.set_site_order("random")
+        o.set_site_order("random")
+        assert g.get_variant() == "field"
+        for k in (1, n):
+            g.sweeps(k, 1)
+            o.sweeps(k, 1, field=True, threads=THREADS)
+            assert_same_state(g, o, "random order L=%d q=%d after +%d" % (L, q, k))
+        if L % 64 == 0:
+            with pytest.raises(pt.PTError):
+                g.set_variant("direct")
+            g.set_site_order("sequential")
+            g.set_variant("direct")
+            o.set_site_order("sequential")
+            g.sweeps(5, 1)
+            o.sweeps(5, 1)
+            assert_same_state(g, o, "back to sequential order, direct variant")
+        g.close()
+        o.close()
