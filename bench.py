@@ -35,11 +35,13 @@ UNIT = "attempts/s"
 # ALU roofline: the algorithmic work of one attempt is L pair terms, each ONE integer
 # multiply-accumulate (16-bit coupling half x 8-bit weight); IDP.2A does two of them per lane and issues at a measured
 # 64 lanes/clk/SM on the FMA-heavy pipe (profiles/r1_a_direct_v1a.md), so peak = 148 SMs x 64 x 2 MAC x f_SM.
-IDP_LANES_PER_CLK_PER_SM = 64
+IDP_LANES_PER_CLK_PER_SM = 64    # fallback only: the line carries the rate pt_measure_peaks measured in this run
 MACS_PER_IDP_LANE = 2
-# dram__bytes_read.sum + dram__bytes_write.sum per sweep of a persistent sweep_direct_kernel launch
-# (ncu --set full on a 40-sweep launch: 407.6 KB read + 10.2 KB written, profiles/r1_f_direct_v8.md)
-DRAM_BYTES_PER_SWEEP = 10.45e3
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE persistent sweep_direct_kernel launch on configs[3], from ncu
+# --set full captures of a 20-sweep and a 40-sweep launch (profiles/r2_a_headline.md): a fixed part (couplings, spins,
+# ladder, permutation: read once) plus a part per sweep (energies and arrival counters of the swap events)
+DRAM_BYTES_PER_LAUNCH_FIXED = 397.0e3
+DRAM_BYTES_PER_SWEEP = 0.52e3
 N_SM = 148
 
 
@@ -54,14 +56,24 @@ def emit(line):
 def pick_workload(args):
     if args.workload in ("cfg3", "configs[3]"):
         return inputs.config(3)
+    if args.workload in ("cfg0", "cfg1", "cfg2"):
+        return inputs.config(int(args.workload[3]))
+    if args.workload.count(":") == 3 and not args.workload.startswith("paper:"):   # L:q:sigma:R, geometric T in [0.6, 2.5]
+        L, q, sigma, R = args.workload.split(":")
+        return inputs.Workload("custom[L=%s,q=%s,sigma=%s,R=%s]" % (L, q, sigma, R), int(L), int(q), float(sigma), 1,
+                               int(R), 0.6, 2.5, 1000, seed=inputs.SEED_BASE + 0x900 + int(L))
     if args.workload.startswith("paper:"):
         parts = args.workload.split(":")
         return inputs.paper_benchmark(int(parts[1]), int(parts[2]) if len(parts) > 2 else 400)
-    raise SystemExit("bench.py: --workload must be cfg3, paper:L or paper:L:R")
+    raise SystemExit("bench.py: --workload must be cfg0..cfg4, paper:L, paper:L:R or L:q:sigma:R")
 
 
 def label(w):
-    return "configs[3]" if w.name == "cfg3" else "the paper's benchmark shape (PAPER.md:136,202; not BASELINE's config)"
+    if w.name.startswith("cfg"):
+        return "configs[%s]" % w.name[3] + ("" if w.name == "cfg3" else " (not the headline config)")
+    if w.name.startswith("custom"):
+        return "custom shape (not BASELINE's config)"
+    return "the paper's benchmark shape (PAPER.md:136,202; not BASELINE's config)"
 
 
 def metric_name(w):
@@ -226,6 +238,7 @@ def run_ours(args):
     ens_base, n_ens_local = shard.ensemble_shard(world, world, rank)   # one configs[3] ensemble per GPU
     g = pt.PT(w.L, w.q, w.sigma, n_ens_local, w.n_rep, betas, w.seed, ens_base=ens_base, variant=args.variant)
     variant = g.get_variant()
+    peaks = pt.measure_peaks()   # instruction rates per SM and clock, measured now: ~1 s
     stream = torch.cuda.Stream()
     g.use_torch_stream(stream)
 
@@ -257,10 +270,10 @@ def run_ours(args):
     acc = float(obs["flip_accepts"].sum()) / float(obs["flip_attempts"].sum())
 
     # ---- end to end through the C ABI with host buffers: upload a start configuration, K steps, read back ----
-    start = g.get_spins()
+    start, E0, _, sweep0 = g.get_state()
     barrier()
     t0 = time.perf_counter()
-    g.set_spins(start)                       # H2D: n_rep*L bytes
+    g.set_state(start, E0, None, sweep0)     # H2D: n_rep*L bytes of spins + n_rep*8 bytes of energies (pinned staging)
     g.sweeps(K, w.swap_every)
     spins = g.get_spins()                    # D2H: n_rep*L bytes
     E = g.energy()                           # D2H: n_rep*8 bytes
@@ -271,8 +284,10 @@ def run_ours(args):
         e2e_s = shard.max_over_ranks(e2e_s, dist, device="cuda")
     assert spins.shape == start.shape and E.size == w.n_rep and ob["n_samples"].min() > 0
     e2e = {"value": world * attempts_per_gpu / e2e_s, "unit": UNIT,
-           "h2d_bytes_per_step": start.nbytes / K, "d2h_bytes_per_step": (spins.nbytes + E.nbytes + w.n_rep * 144) / K,
-           "what": "pt_set_spins(host) + pt_sweeps(K) + pt_get_spins + pt_energy + pt_observables (host buffers), wall clock"}
+           "h2d_bytes_per_step": (start.nbytes + E0.nbytes) / K,
+           "d2h_bytes_per_step": (spins.nbytes + E.nbytes + w.n_rep * 144) / K,
+           "what": "pt_set_state(host spins + energies) + pt_sweeps(K) + pt_get_spins + pt_energy + pt_observables "
+                   "(host buffers), wall clock"}
 
     if rank == 0:
         f_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
@@ -280,23 +295,31 @@ def run_ours(args):
         macs_per_launch = K * w.n_rep * w.L * w.L / max(1, launches)
         launch_s = ms * 1e-3 / max(1, launches)              # CUDA events on the launching stream
         achieved = macs_per_launch / launch_s / 1e12
-        dram_per_launch = DRAM_BYTES_PER_SWEEP * K / max(1, launches)
-        peak = N_SM * IDP_LANES_PER_CLK_PER_SM * MACS_PER_IDP_LANE * f_hz / 1e12
+        dram_per_launch = DRAM_BYTES_PER_LAUNCH_FIXED + DRAM_BYTES_PER_SWEEP * K / max(1, launches)
+        lanes = peaks["idp2a"][1] or IDP_LANES_PER_CLK_PER_SM          # IDP.2A alone, 2 warps per sub-partition
+        lanes_mix = peaks["prmt+2idp2a (idp2a counted)"][1]            # ... next to one PRMT per two IDP.2A
+        peak = N_SM * lanes * MACS_PER_IDP_LANE * f_hz / 1e12
+        persistent = launches == 1 and K > 1 and variant == "direct"
         roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tmac/s", "frac": achieved / peak,
-                    "traffic": dram_per_launch if variant == "direct" and w.name == "cfg3" else None,
+                    "traffic": dram_per_launch if persistent and w.name == "cfg3" else None,
                     "kernel": "sweep_%s_kernel" % variant,
+                    "idp2a_lanes_per_clk_per_sm": lanes, "idp2a_lanes_in_bulk_mix": lanes_mix,
+                    "frac_of_mix_ceiling": achieved / peak * lanes / lanes_mix if lanes_mix else None,
+                    "launch": "persistent (cooperative, swap events inside the kernel)" if persistent
+                              else "one launch per swap interval",
                     "note": "algorithmic work = sweeps*n_rep*L^2 = %.3e integer multiply-accumulates per launch (one per "
-                            "pair term; %d sweeps per launch); peak = 148 SMs x 64 IDP.2A lanes/clk/SM (measured issue rate) x 2 MAC x "
+                            "pair term; %d sweeps per launch); peak = 148 SMs x %.1f IDP.2A lanes/clk/SM (pt_measure_peaks, "
+                            "this run) x 2 MAC x "
                             "sampled SM clock %.0f MHz -- a derived ALU peak, not MEASURED_PEAKS.json (its HBM and "
                             "tensor figures do not bound this path%s)"
-                            % (macs_per_launch, K // max(1, launches), f_hz / 1e6,
+                            % (macs_per_launch, K // max(1, launches), lanes, f_hz / 1e6,
                                ": %.0f KB of DRAM traffic per launch = %.2f GB/s of the measured %.0f GB/s; 128 of 148 "
                                "SMs carry a replica" % (dram_per_launch / 1e3, dram_per_launch / launch_s / 1e9,
                                                         measured_hbm_gbs()) if w.name == "cfg3" else "")}
         line = {"metric": metric_name(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "int32", "data": "synthetic", "config": workload_config(w, variant, world),
-                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+                "dtype": {"fp32": "f32", "fp64": "f64"}.get(variant, "int32"), "data": "synthetic",
+                "config": workload_config(w, variant, world), "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
                 "flip_acceptance": acc, "pair_evaluations_per_s": value * (w.L - 1)}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline_leg(w)
@@ -317,9 +340,19 @@ def run_cfg4(args):
     from paper_1308_5426_b200 import pt
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: libpt has no CPU path")
-    if int(os.environ.get("WORLD_SIZE", "1")) != 1:
-        raise SystemExit("bench.py: --workload cfg4 is a single-GPU workload")
-    ws = inputs.config4()
+    import torch.distributed as dist
+    from paper_1308_5426_b200 import shard
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local_rank)
+    use_dist = world > 1 or "RANK" in os.environ
+    if use_dist:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    # the 40 members are independent: rank r takes a contiguous block of them (no data-path collective; scaling "strong")
+    base, n_loc = shard.ensemble_shard(40, world, rank)
+    ws_all = inputs.config4()
+    ws = ws_all[base:base + n_loc]
     K, W_ = args.steps, args.warmup
     streams = [torch.cuda.Stream() for _ in ws]
     gs = []
@@ -338,7 +371,9 @@ def run_cfg4(args):
 
     steps(W_)
     torch.cuda.synchronize()
-    sampler = ClockSampler(0)
+    if use_dist:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
     sampler.start_sampling()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record(main_s)
@@ -351,7 +386,9 @@ def run_cfg4(args):
     torch.cuda.synchronize()
     clocks = sampler.result()
     ms = ev0.elapsed_time(ev1)
-    attempts = K * sum(w.n_rep * w.L for w in ws)
+    if use_dist:
+        ms = shard.max_over_ranks(ms, dist, device="cuda")
+    attempts = K * sum(w.n_rep * w.L for w in ws_all)       # whole job: all 40 members over all ranks
     value = attempts / (ms * 1e-3)
 
     starts = [g.get_spins() for g in gs]
@@ -367,13 +404,21 @@ def run_cfg4(args):
         assert ob["n_samples"].min() > 0
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
+    if use_dist:
+        e2e_s = shard.max_over_ranks(e2e_s, dist, device="cuda")
+        launches = int(shard.max_over_ranks(float(launches), dist, device="cuda")) * world
+    if rank != 0:
+        for g in gs:
+            g.close()
+        dist.destroy_process_group()
+        return 0
     f_hz = (clocks.get("sm_mhz") or 1965.0) * 1e6
-    macs = K * sum(w.n_rep * w.L * w.L for w in ws)
+    macs = K * sum(w.n_rep * w.L * w.L for w in ws_all) / world     # per GPU
     achieved = macs / (ms * 1e-3) / 1e12
     peak = N_SM * IDP_LANES_PER_CLK_PER_SM * MACS_PER_IDP_LANE * f_hz / 1e12
     line = {"metric": "Metropolis spin-flip attempts/s on the sigma-q scan (40 ensembles x 32 replicas, L=2048)",
-            "value": value, "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": W_, "ms_per_step": ms / K,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_, "ms_per_step": ms / K,
+            "higher_is_better": True, "scaling": "strong" if world > 1 else "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
             "config": {"workload": "configs[4] (not the headline config): L=2048, q in {3,5,7,9} x sigma in {0.1..1.0} = "
                                    "40 handles x 32 replicas, T geometric in [0.4,3.0], hot start, swap every sweep, "
                                    "40 CUDA streams", "variant": gs[0].get_variant(),
@@ -393,6 +438,60 @@ def run_cfg4(args):
     emit(line)
     for g in gs:
         g.close()
+    if use_dist:
+        dist.destroy_process_group()
+    return 0
+
+
+def run_sharded(args):
+    """--sharded: ONE configs[3] ensemble with its 128 slots spread over the ranks; every rank sweeps
+    its configurations, at every swap event the ranks all-gather the running energies (n_rep int64 over NCCL: the only
+    data that crosses GPUs) and take the same decisions (shard.ShardedEnsemble).  Scaling "strong".  One launch per
+    sweep per rank (no persistent kernel: the swap barrier spans GPUs)."""
+    import torch
+    import torch.distributed as dist
+    from paper_1308_5426_b200 import build as ptbuild
+    ptbuild.build()
+    from paper_1308_5426_b200 import pt, shard
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local_rank)
+    use_dist = world > 1 or "RANK" in os.environ
+    if use_dist:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    w = pick_workload(args)
+    K, W_ = args.steps, args.warmup
+    ens = shard.ShardedEnsemble(pt, w.L, w.q, w.sigma, w.n_rep, inputs.betas(w), w.seed, dist=dist if use_dist else None)
+    ens.sweeps(W_, w.swap_every)
+    torch.cuda.synchronize()
+    if use_dist:
+        dist.barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start_sampling()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    ens.sweeps(K, w.swap_every)
+    ev1.record()
+    torch.cuda.synchronize()
+    if use_dist:
+        dist.barrier()
+    clocks = sampler.result()
+    ms = ev0.elapsed_time(ev1)
+    if use_dist:
+        ms = shard.max_over_ranks(ms, dist, device="cuda")
+    value = K * w.n_rep * w.L / (ms * 1e-3)
+    if rank == 0:
+        emit({"metric": metric_name(w) + " (one ensemble sharded over the GPUs)", "value": value, "unit": UNIT,
+              "n_gpus": world, "steps": K, "warmup": W_, "ms_per_step": ms / K, "higher_is_better": True,
+              "scaling": "strong", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+              "config": dict(workload_config(w, "direct", world),
+                             parallelism="slots of one ensemble sharded over %d GPU(s); all-gather of %d int64 energies "
+                                         "per swap event (NCCL)" % (world, w.n_rep)),
+              "clocks": clocks, "gpu_launches": 2 * K, "e2e": None, "roofline": None})
+    ens.close()
+    if use_dist:
+        dist.destroy_process_group()
     return 0
 
 
@@ -402,7 +501,9 @@ def main():
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=20)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--variant", default="auto", choices=["auto", "direct", "field"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "direct", "field", "fp32", "fp64"])
+    ap.add_argument("--sharded", action="store_true", help="one ensemble with its slots sharded over the GPUs (SURVEY.md 8(e)(2))")
+    ap.add_argument("--peaks", action="store_true", help="print the instruction-rate micro-benchmarks (pt_measure_peaks) and exit")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--workload", default="cfg3", help="cfg3 (BASELINE.json's headline config, default), cfg4, paper:L or paper:L:R")
     args = ap.parse_args()
@@ -414,6 +515,15 @@ def main():
     sys.stdout.flush()
     _JSON_OUT = os.fdopen(os.dup(1), "w")
     os.dup2(2, 1)
+    if args.peaks:
+        from paper_1308_5426_b200 import build as ptbuild
+        ptbuild.build()
+        from paper_1308_5426_b200 import pt
+        emit({"peaks": pt.measure_peaks(), "unit": "lane-operations per clock and SM (lds128: bytes), for 1, 2, 3, 4 warps "
+              "per SM sub-partition; clock64() inside the kernel"})
+        return 0
+    if args.sharded:
+        return run_sharded(args)
     if args.workload == "cfg4":
         if args.impl == "reference":
             raise SystemExit("bench.py: --impl reference times the headline config or a paper:L shape")

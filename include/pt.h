@@ -148,6 +148,11 @@ int pt_energy_storage_dev(pt_ctx* ctx, int64_t* E_out_dev);
  * all n_rep configurations in storage order, E_all_dev[n_rep] (DEVICE pointer). */
 int pt_swap_external(pt_ctx* ctx, const int64_t* E_all_dev);
 
+/* Asynchronous forms of the two calls above: enqueued on the context's stream, no synchronisation (the caller orders
+ * its own collective on the same stream and calls pt_sync at the end): one swap event then costs no host round trip. */
+int pt_energy_storage_dev_async(pt_ctx* ctx, int64_t* E_out_dev);
+int pt_swap_external_async(pt_ctx* ctx, const int64_t* E_all_dev);
+
 /* perm[n_ens*n_rep]: storage index (inside the ensemble) of the configuration at each slot. */
 int pt_get_perm(pt_ctx* ctx, int32_t* perm);
 

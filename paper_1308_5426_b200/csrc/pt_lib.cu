@@ -580,24 +580,34 @@ int pt_create_shard(pt_ctx** out, int L, int q, double sigma, int n_rep, const d
     return PT_OK;
 }
 
-int pt_energy_storage_dev(pt_ctx* c, int64_t* E_out_dev) {
+int pt_energy_storage_dev_async(pt_ctx* c, int64_t* E_out_dev) {
     if (!c || !E_out_dev) return fail(PT_EINVAL, "NULL argument");
     DeviceGuard guard(c->device);
     const int n = c->n_local ? c->n_local : c->R();
     PT_CUDA(cudaMemcpyAsync(E_out_dev, c->d_E + c->rep_base, (size_t)n * sizeof(long long), cudaMemcpyDeviceToDevice,
                             c->stream));
-    return pt_sync(c);
+    return PT_OK;
 }
 
-int pt_swap_external(pt_ctx* c, const int64_t* E_all_dev) {
+int pt_energy_storage_dev(pt_ctx* c, int64_t* E_out_dev) {
+    int rc = pt_energy_storage_dev_async(c, E_out_dev);
+    return rc ? rc : pt_sync(c);
+}
+
+int pt_swap_external_async(pt_ctx* c, const int64_t* E_all_dev) {
     if (!c || !E_all_dev) return fail(PT_EINVAL, "NULL argument");
-    DeviceGuard guard(c->device);
     if (!c->n_local) return fail(PT_EINVAL, "pt_swap_external is for slot-sharded contexts (pt_create_shard)");
+    DeviceGuard guard(c->device);
     PT_CUDA(cudaMemcpyAsync(c->d_E, E_all_dev, (size_t)c->n_rep * sizeof(long long), cudaMemcpyDeviceToDevice,
                             c->stream));
     ptk::swap_kernel<<<1, 256, 0, c->stream>>>(c->dev(), (uint32_t)c->sweep);
     PT_CUDA(cudaGetLastError());
-    return pt_sync(c);
+    return PT_OK;
+}
+
+int pt_swap_external(pt_ctx* c, const int64_t* E_all_dev) {
+    int rc = pt_swap_external_async(c, E_all_dev);
+    return rc ? rc : pt_sync(c);
 }
 
 int pt_get_perm(pt_ctx* c, int32_t* perm) {

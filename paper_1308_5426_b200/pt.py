@@ -23,7 +23,8 @@ SYMBOLS = ["pt_create", "pt_create_ex", "pt_destroy", "pt_sweeps", "pt_energy", 
            "pt_observables", "pt_get_spins", "pt_get_spins_dev", "pt_set_spins", "pt_get_couplings",
            "pt_sweep_counter", "pt_set_variant", "pt_get_variant", "pt_set_stream", "pt_sweeps_async",
            "pt_sync", "pt_last_error", "pt_create_shard", "pt_energy_storage_dev", "pt_swap_external",
-           "pt_get_perm", "pt_measure_peaks", "pt_get_state", "pt_set_state", "pt_set_site_order"]
+           "pt_get_perm", "pt_measure_peaks", "pt_get_state", "pt_set_state", "pt_set_site_order",
+           "pt_energy_storage_dev_async", "pt_swap_external_async"]
 
 
 class PTError(RuntimeError):
@@ -79,6 +80,8 @@ _lib.pt_measure_peaks.argtypes = [_vp, _i32]
 _lib.pt_get_state.argtypes = [_vp, _vp, _vp, _vp, ctypes.POINTER(_i64)]
 _lib.pt_set_state.argtypes = [_vp, _vp, _vp, _vp, _i64]
 _lib.pt_set_site_order.argtypes = [_vp, _i32]
+_lib.pt_energy_storage_dev_async.argtypes = [_vp, _vp]
+_lib.pt_swap_external_async.argtypes = [_vp, _vp]
 
 PEAK_PATTERNS = ["idp2a", "idp4a", "imad", "prmt", "lop3", "prmt+2idp2a (idp2a counted)", "lop3+2idp2a (idp2a counted)",
                  "lds128 (bytes)", "prmt+4idp2a (idp2a counted)", "2prmt+add+2idp2a (idp2a counted)"]
@@ -173,6 +176,15 @@ class PT:
         """Slot-sharded contexts: E_all = torch int64 CUDA tensor, energies of all n_rep configurations, storage order."""
         assert E_all.is_cuda and E_all.numel() == self.n_rep and E_all.element_size() == 8 and E_all.is_contiguous()
         _check(_lib.pt_swap_external(self._h, ctypes.c_void_p(E_all.data_ptr())))
+
+    def energy_storage_dev_async(self, out):
+        assert out.is_cuda and out.element_size() == 8
+        _check(_lib.pt_energy_storage_dev_async(self._h, ctypes.c_void_p(out.data_ptr())))
+        return out
+
+    def swap_external_async(self, E_all):
+        assert E_all.is_cuda and E_all.numel() == self.n_rep and E_all.element_size() == 8 and E_all.is_contiguous()
+        _check(_lib.pt_swap_external_async(self._h, ctypes.c_void_p(E_all.data_ptr())))
 
     def get_perm(self):
         perm = np.zeros((self.n_ens, self.n_rep), dtype=np.int32)

@@ -84,18 +84,29 @@ class ShardedEnsemble:
         if self.n_local < 1:
             raise ValueError("more ranks than replicas")
         self.g = pt.PT(L, q, sigma, 1, n_rep, betas, seed, ens_base=ens_base, shard=(self.base, self.n_local))
+        # sweeps, the copy of the local energies, the all-gather and the swap kernel are all enqueued on ONE stream (the
+        # current torch stream, which NCCL collectives follow): a swap event costs no host round trip
+        self.g.use_torch_stream(torch.cuda.current_stream())
         self.n_max = -(-n_rep // self.world)
         self._loc = torch.zeros(self.n_max, dtype=torch.int64, device="cuda")
+        self._flat = torch.zeros(self.world * self.n_max, dtype=torch.int64, device="cuda")
         self._all = torch.zeros(n_rep, dtype=torch.int64, device="cuda")
+        idx = []   # position of storage index x in the padded gather buffer
+        for r in range(self.world):
+            _, n_r = ensemble_shard(n_rep, self.world, r)
+            idx += [r * self.n_max + k for k in range(n_r)]
+        self._index = torch.tensor(idx, dtype=torch.int64, device="cuda")
 
     def gather_energies(self):
-        """All configurations' running energies in storage order, on the device (the exchange step)."""
+        """All configurations' running energies in storage order, on the device (the exchange step), enqueued."""
         torch = self.torch
-        self.g.energy_storage_dev(self._loc[: self.n_local])
+        self.g.energy_storage_dev_async(self._loc[: self.n_local])
         if self.dist is None:
             self._all.copy_(self._loc[: self.n_rep])
             return self._all
-        return all_gather_blocks(self._loc, self.n_rep, self.dist, out=self._all)
+        self.dist.all_gather_into_tensor(self._flat, self._loc)
+        torch.index_select(self._flat, 0, self._index, out=self._all)
+        return self._all
 
     def sweeps(self, n, swap_every=1):
         done = 0
@@ -106,10 +117,11 @@ class ShardedEnsemble:
                 to_event = swap_every - (self.g.sweep_counter() % swap_every)
                 if to_event <= chunk:
                     chunk, event = to_event, True
-            self.g.sweeps(chunk, 0)
+            self.g.sweeps_async(chunk, 0)
             if event:
-                self.g.swap_external(self.gather_energies())
+                self.g.swap_external_async(self.gather_energies())
             done += chunk
+        self.g.sync()
 
     def close(self):
         self.g.close()
