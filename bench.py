@@ -40,8 +40,8 @@ MACS_PER_IDP_LANE = 2
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE persistent sweep_direct_kernel launch on configs[3], from ncu
 # --set full captures of a 20-sweep and a 40-sweep launch (profiles/r2_a_headline.md): a fixed part (couplings, spins,
 # ladder, permutation: read once) plus a part per sweep (energies and arrival counters of the swap events)
-DRAM_BYTES_PER_LAUNCH_FIXED = 397.0e3
-DRAM_BYTES_PER_SWEEP = 0.52e3
+DRAM_BYTES_PER_LAUNCH_FIXED = 412.7e3
+DRAM_BYTES_PER_SWEEP = 0.165e3
 N_SM = 148
 
 
