@@ -32,6 +32,15 @@ def _deps():
     return out
 
 
+def build_variant(out_path, defines, verbose=False):
+    """A development build of the same sources with extra -D flags (e.g. ["PT_PARANOID", "PT_ONLY_HEADLINE"]) at
+    out_path; load it with PT_LIBPT=out_path."""
+    cmd = [_nvcc()] + NVCC_FLAGS + ["-D" + d for d in defines] + (["-Xptxas", "-v"] if verbose else []) + \
+          ["-o", out_path] + SOURCES
+    subprocess.check_call(cmd)
+    return out_path
+
+
 def build(force=False, verbose=False):
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(p) for p in _deps()):
         return LIB

@@ -419,6 +419,8 @@ int pt_sync(pt_ctx* c) {
     DeviceGuard guard(c->device);
     PT_CUDA(cudaStreamSynchronize(c->stream));
     PT_CUDA(cudaGetLastError());
+    if (c->h_err && *(volatile int*)c->h_err == 2)
+        return fail(PT_ECUDA, "PT_PARANOID: the accept mask of a block differs from its site-by-site forward substitution");
     if (c->h_err && *(volatile int*)c->h_err)
         return fail(PT_ECUDA, "an in-kernel swap barrier timed out (a CTA of the ensemble did not arrive within 30 s): "
                               "the state of this context is lost");

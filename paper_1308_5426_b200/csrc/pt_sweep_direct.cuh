@@ -707,6 +707,24 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                     }
                 }
                 PT_ACC(2, t_s);
+#ifdef PT_PARANOID
+                // Development builds (-DPT_PARANOID): the accept mask once more, by the forward substitution the
+                // site-by-site order of Eq. 8 prescribes -- one site per step, 32 exchanges -- and compared with the
+                // fixed point found above.  A mismatch raises the context's error flag (value 2): pt_sync fails.
+                {
+                    unsigned seq = 0u;
+                    for (int l = 0; l < 32; ++l) {
+                        const unsigned mv = (seq >> (8 * cw)) ^ lz;
+                        s_xch[xb][lane][cw] = masked_add4(masked_add4(pc, mv, 0, co0), mv, 4, co1);
+                        asm volatile("bar.sync 1, 128;" ::: "memory");
+                        const int4 pv = *reinterpret_cast<const int4*>(&s_xch[xb][lane][0]);
+                        xb ^= 1;
+                        const int ys = y - ((pv.x + pv.y) + (pv.z + pv.w));
+                        seq |= (unsigned)__shfl_sync(0xffffffffu, ys >= 0 ? 1 : 0, l) << l;   // site l, all before it decided
+                    }
+                    if (seq != mask && lane == 0) *(volatile int*)d.err = 2;
+                }
+#endif
                 if (cw == 0 && lane < 4) {
                     const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
                     m.sp[wsp] = (w_old & ~nm) | (w_new & nm);

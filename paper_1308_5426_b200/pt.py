@@ -11,7 +11,8 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libpt.so")
+# PT_LIBPT=<path> loads another build of the same library (development builds: -DPT_PARANOID, -DPT_TIMING)
+LIB_PATH = os.environ.get("PT_LIBPT") or os.path.join(_HERE, "libpt.so")
 
 VARIANT_AUTO, VARIANT_FIELD, VARIANT_DIRECT, VARIANT_FP32, VARIANT_FP64 = 0, 1, 2, 3, 4
 _VARIANTS = {"auto": VARIANT_AUTO, "field": VARIANT_FIELD, "direct": VARIANT_DIRECT, "fp32": VARIANT_FP32,

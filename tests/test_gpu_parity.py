@@ -682,3 +682,36 @@ def test_random_site_order(pt, oracle):
             assert_same_state(g, o, "back to sequential order, direct variant")
         g.close()
         o.close()
+
+
+def test_paranoid_build_confirms_the_fixed_point_solution(tmp_path):
+    """a -DPT_PARANOID build of the sweep kernel re-derives every block's accept mask by the
+    32-step forward substitution of the site-by-site order and raises an error on any mismatch with the fixed-point
+    rounds.  configs[3], 50 sweeps, persistent launch; in a subprocess, because the binding loads one library."""
+    import subprocess
+    import sys
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("gpu-marked test on a box without CUDA")
+    from paper_1308_5426_b200 import build
+    lib = build.build_variant(str(tmp_path / "libpt_paranoid.so"), ["PT_PARANOID", "PT_ONLY_HEADLINE"])
+    code = ("import numpy as np\n"
+            "from paper_1308_5426_b200 import inputs, pt\n"
+            "w = inputs.config(3)\n"
+            "g = pt.PT(w.L, w.q, w.sigma, 1, w.n_rep, inputs.betas(w), w.seed, variant='direct')\n"
+            "g.sweeps(50, 1)\n"
+            "acc = g.observables()['flip_accepts'].sum()\n"
+            "assert np.array_equal(g.energy(), g.energy(recompute=True))\n"
+            "print('PARANOID_OK', int(acc))\n")
+    import os
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    run = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=600, cwd=root,
+                         env=dict(os.environ, PT_LIBPT=lib))
+    assert run.returncode == 0 and "PARANOID_OK" in run.stdout, run.stdout[-500:] + run.stderr[-2000:]
+    # the same 50 sweeps with the product build accept the same number of changes (the check changes nothing)
+    from paper_1308_5426_b200 import inputs, pt
+    w = inputs.config(3)
+    g = pt.PT(w.L, w.q, w.sigma, 1, w.n_rep, inputs.betas(w), w.seed, variant="direct")
+    g.sweeps(50, 1)
+    assert int(g.observables()["flip_accepts"].sum()) == int(run.stdout.split("PARANOID_OK")[1].split()[0])
+    g.close()
