@@ -108,7 +108,10 @@ typedef struct {
  * device in fp64 and quantises it, draws the hot start (spins uniform in
  * {1..q} from the Philox stream) and computes every replica's total energy.
  *  L      : ring length, L >= 8 and L % 8 == 0 (8 spins per 32-bit word)
- *  q      : number of colours, 2 <= q <= 16 (4 bits per spin)
+ *  q      : number of colours, 2 <= q <= 64.  q <= 16: 4 bits per spin, every variant.  16 < q <= 64: 8 bits per
+ *           spin (4 spins per word); the field and the floating-point variants only (the direct kernels are built
+ *           on nibble tables), so PT_VARIANT_AUTO resolves to PT_VARIANT_FIELD and needs L*q*4 bytes + tables of
+ *           shared memory (PT_ECAPACITY beyond that)
  *  sigma  : decay exponent of Eq. 4, finite and > 0
  *  n_ens  : independent ensembles (same model, different random streams) >= 1
  *  n_rep  : replicas per ensemble >= 1

@@ -433,7 +433,7 @@ double orc_uniform53(uint32_t w1, uint32_t w2) { return uniform53(w1, w2); }
 void* orc_create_ex(int L, int q, double sigma, int n_ens, int n_rep, const double* betas, uint64_t seed,
                     int ens_base) {
     if (ens_base < 0) return nullptr;
-    if (L < 2 || (L % 8) != 0 || q < 2 || q > 16 || !(sigma > 0.0) || !std::isfinite(sigma) ||
+    if (L < 2 || (L % 8) != 0 || q < 2 || q > 64 || !(sigma > 0.0) || !std::isfinite(sigma) ||
         n_ens < 1 || n_rep < 1 || !betas)
         return nullptr;
     for (int t = 0; t < n_rep; ++t)

@@ -38,7 +38,7 @@ int main() {
         check += (long long)(orc_uniform53(w[1], w[2]) * 1000.0);
     }
     struct Shape { int L, q, n_ens, n_rep; double sigma; };
-    const Shape shapes[] = {{8, 2, 1, 1, 0.5}, {64, 3, 2, 5, 0.4}, {40, 16, 1, 3, 0.9}, {128, 8, 1, 4, 0.3}};
+    const Shape shapes[] = {{8, 2, 1, 1, 0.5}, {64, 3, 2, 5, 0.4}, {40, 16, 1, 3, 0.9}, {128, 8, 1, 4, 0.3}, {48, 37, 1, 2, 0.6}};
     for (const Shape& s : shapes) {
         std::vector<double> betas(s.n_rep);
         for (int t = 0; t < s.n_rep; ++t) betas[t] = 0.3 + 0.4 * t;
@@ -75,7 +75,7 @@ int main() {
     // invalid arguments must be refused, not crash
     const double b1[1] = {1.0};
     if (orc_create_ex(12, 3, 0.5, 1, 1, b1, 1, 0)) return 8;
-    if (orc_create_ex(64, 17, 0.5, 1, 1, b1, 1, 0)) return 8;
+    if (orc_create_ex(64, 65, 0.5, 1, 1, b1, 1, 0)) return 8;
     if (orc_create_ex(64, 3, 0.5, 1, 1, nullptr, 1, 0)) return 8;
     std::printf("sanitize_main OK %lld\n", check);
     return 0;

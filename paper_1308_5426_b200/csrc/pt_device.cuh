@@ -58,6 +58,21 @@ __device__ __forceinline__ uint32_t match_nibbles(uint32_t w, uint32_t k) {
     return ~nz & 0x88888888u;
 }
 
+// Wide packing (q > 16): 4 spins per 32-bit word, colour c in 0..255 of site i in byte i%4 of word i/4.  The
+// generic kernels take the width (4 or 8 bits per spin) at run time; the direct kernels are 4-bit only.
+__device__ __forceinline__ int get_colour(const uint32_t* words, int i, int bits) {
+    return bits == 4 ? get_nibble(words, i) : (int)((words[i >> 2] >> ((i & 3) << 3)) & 255u);
+}
+
+// Top bit of every field of w (nibble or byte) that equals colour k; the n-th site of the word answers at bit
+// bits*(n+1)-1, so site = bit / bits.
+__device__ __forceinline__ uint32_t match_colours(uint32_t w, uint32_t k, int bits) {
+    if (bits == 4) return match_nibbles(w, k);
+    const uint32_t z = w ^ (k * 0x01010101u);
+    const uint32_t nz = ((z & 0x7f7f7f7fu) + 0x7f7f7f7fu) | z;
+    return ~nz & 0x80808080u;
+}
+
 // Adds x*x to the 128-bit accumulator (lo, hi).
 __device__ __forceinline__ void add_square_128(unsigned long long& lo, long long& hi, long long x) {
     const unsigned long long ax = (unsigned long long)(x < 0 ? -x : x);

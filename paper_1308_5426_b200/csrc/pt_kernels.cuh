@@ -32,6 +32,7 @@ inline int allow_max_dynamic_smem(const void* kernel, int static_bytes) {
 // Everything a kernel needs to know about a context (passed by value).
 struct Dev {
     int L, W, q, n_ens, n_rep, ens_base;
+    int bits;                 // bits per spin in spins[]: 4 (q <= 16, 8 sites per word) or 8 (q <= 64, 4 sites per word)
     int rep_base, n_local;    // slot-sharded contexts (pt_create_shard): this process sweeps the configurations with
                               // storage index rep_base .. rep_base + n_local - 1; otherwise 0, n_rep
     int count_swaps;          // 0: this shard leaves the swap counters to the shard with rep_base = 0
@@ -126,10 +127,10 @@ __global__ void init_spins_kernel(Dev d) {
     const int e = x / d.n_rep, t = x % d.n_rep;
     const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_INIT;
     uint32_t word = 0;
-#pragma unroll
-    for (int n = 0; n < 8; ++n) {
-        const Philox4 p = philox4x32_10((uint32_t)(8 * w + n), 0u, (uint32_t)t, c3, d.key0, d.key1);
-        word |= __umulhi(p.w0, (uint32_t)d.q) << (4 * n);
+    const int per = 32 / d.bits;
+    for (int n = 0; n < per; ++n) {
+        const Philox4 p = philox4x32_10((uint32_t)(per * w + n), 0u, (uint32_t)t, c3, d.key0, d.key1);
+        word |= __umulhi(p.w0, (uint32_t)d.q) << (d.bits * n);
     }
     d.spins[gid] = word;  // storage index == slot at creation (perm = identity)
 }
@@ -143,7 +144,7 @@ __global__ void init_perm_kernel(Dev d) {
 // a6. Total energy (Eq. 2 in reading A1):
 //   E = -sum_{i<j} Jq[j-i] [c_i==c_j] = -(1/2) sum_i sum_{j!=i} Jq[|i-j|] [c_j==c_i].
 // One CTA per replica (storage order), one site per thread and pass; spins and
-// couplings staged in shared memory; SWAR match of 8 sites per word.
+// couplings staged in shared memory; SWAR match of the 8 (or 4) sites of a word.
 // dynamic smem: (L + W) * 4 bytes.
 // ---------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) energy_kernel(Dev d, long long* __restrict__ E_out) {
@@ -156,15 +157,16 @@ __global__ void __launch_bounds__(256) energy_kernel(Dev d, long long* __restric
     for (int w = threadIdx.x; w < d.W; w += blockDim.x) sp[w] = d.spins[(size_t)x * d.W + w];
     __syncthreads();
     long long acc = 0;
+    const int per = 32 / d.bits, lg = d.bits == 4 ? 2 : 3;
     for (int i = threadIdx.x; i < d.L; i += blockDim.x) {
-        const uint32_t a = (uint32_t)get_nibble(sp, i);
+        const uint32_t a = (uint32_t)get_colour(sp, i, d.bits);
         long long row = 0;
         for (int w = 0; w < d.W; ++w) {
-            uint32_t m = match_nibbles(sp[w], a);
+            uint32_t m = match_colours(sp[w], a, d.bits);
             while (m) {
                 const int bit = __ffs(m) - 1;
                 m &= m - 1;
-                const int j = 8 * w + (bit >> 2);
+                const int j = per * w + (bit >> lg);
                 const int dist = j > i ? j - i : i - j;
                 row += J[dist];  // J[0] = 0 removes j == i
             }
@@ -195,15 +197,16 @@ __global__ void __launch_bounds__(256) build_fields_kernel(Dev d) {
     for (int w = threadIdx.x; w < d.W; w += blockDim.x) sp[w] = d.spins[(size_t)x * d.W + w];
     __syncthreads();
     int32_t* hx = d.h + (size_t)x * d.q * d.L;
+    const int per = 32 / d.bits, lg = d.bits == 4 ? 2 : 3;
     for (int i = threadIdx.x; i < d.L; i += blockDim.x) {
         for (int k = 0; k < d.q; ++k) {
             int32_t acc = 0;
             for (int w = 0; w < d.W; ++w) {
-                uint32_t m = match_nibbles(sp[w], (uint32_t)k);
+                uint32_t m = match_colours(sp[w], (uint32_t)k, d.bits);
                 while (m) {
                     const int bit = __ffs(m) - 1;
                     m &= m - 1;
-                    const int j = 8 * w + (bit >> 2);
+                    const int j = per * w + (bit >> lg);
                     const int dist = j > i ? j - i : i - j;
                     acc += J[dist];
                 }
@@ -273,15 +276,16 @@ __global__ void swap_kernel(Dev d, uint32_t sweep) { swap_event(d, blockIdx.x, s
 // ---------------------------------------------------------------------------
 // a8 helper.  N_max = max_k N_k of the configuration in packed words sp[W]
 // (Eq. 10).  All threads call; result valid in thread 0.
-// s_cnt: 16 ints of shared memory.
+// s_cnt: PT_QMAX ints of shared memory.
 // ---------------------------------------------------------------------------
-__device__ inline int count_nmax(const uint32_t* sp, int W, int q, int* s_cnt) {
-    if (threadIdx.x < 16) s_cnt[threadIdx.x] = 0;
+constexpr int PT_QMAX = 64;
+__device__ inline int count_nmax(const uint32_t* sp, int W, int q, int bits, int* s_cnt) {
+    if (threadIdx.x < PT_QMAX) s_cnt[threadIdx.x] = 0;
     __syncthreads();
     for (int w = threadIdx.x; w < W; w += blockDim.x) {
         const uint32_t word = sp[w];
         for (int k = 0; k < q; ++k) {
-            const int c = __popc(match_nibbles(word, (uint32_t)k));
+            const int c = __popc(match_colours(word, (uint32_t)k, bits));
             if (c) atomicAdd(&s_cnt[k], c);
         }
     }
@@ -351,9 +355,10 @@ __global__ void unpack_spins_kernel(Dev d, uint8_t* __restrict__ out) {
     const int e = x / d.n_rep;
     const int st = d.perm[x];
     const uint32_t word = d.spins[((size_t)e * d.n_rep + st) * d.W + w];
-    uint8_t* o = out + (size_t)x * d.L + 8 * w;
-#pragma unroll
-    for (int n = 0; n < 8; ++n) o[n] = (uint8_t)(((word >> (4 * n)) & 15u) + 1u);  // A4: API colours 1..q
+    const int per = 32 / d.bits;
+    const uint32_t mask = (1u << d.bits) - 1u;
+    uint8_t* o = out + (size_t)x * d.L + per * w;
+    for (int n = 0; n < per; ++n) o[n] = (uint8_t)(((word >> (d.bits * n)) & mask) + 1u);  // A4: API colours 1..q
 }
 
 __global__ void check_spins_kernel(Dev d, const uint8_t* __restrict__ in, int* __restrict__ bad) {
@@ -372,10 +377,10 @@ __global__ void pack_spins_kernel(Dev d, const uint8_t* __restrict__ in) {
     const int x = (int)(gid / d.W);
     const int e = x / d.n_rep;
     const int st = d.perm[x];
-    const uint8_t* s = in + (size_t)x * d.L + 8 * w;
+    const int per = 32 / d.bits;
+    const uint8_t* s = in + (size_t)x * d.L + per * w;
     uint32_t word = 0;
-#pragma unroll
-    for (int n = 0; n < 8; ++n) word |= (uint32_t)(s[n] - 1) << (4 * n);
+    for (int n = 0; n < per; ++n) word |= (uint32_t)(s[n] - 1) << (d.bits * n);
     d.spins[((size_t)e * d.n_rep + st) * d.W + w] = word;
 }
 

@@ -96,9 +96,11 @@ struct pt_ctx {
     int persistent_policy = 1;   // 0 never, 1 when the context fills the device and the call is long enough, 2 whenever possible
 
     int R() const { return n_ens * n_rep; }
+    int bits() const { return q <= 16 ? 4 : 8; }     // bits per spin in d_spins
+    int words() const { return L * bits() / 32; }    // 32-bit words per configuration
     ptk::Dev dev() const {
         ptk::Dev d;
-        d.L = L; d.W = L / 8; d.q = q; d.n_ens = n_ens; d.n_rep = n_rep; d.ens_base = ens_base;
+        d.bits = bits(); d.L = L; d.W = words(); d.q = q; d.n_ens = n_ens; d.n_rep = n_rep; d.ens_base = ens_base;
         d.key0 = (uint32_t)seed; d.key1 = (uint32_t)(seed >> 32); d.rowsum = (uint32_t)rowsum;
         d.Jq = d_Jq; d.Jpair = d_Jpair; d.beta = d_beta; d.thr_scale = d_scale;
         d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done; d.dbg = d_dbg; d.gen = d_gen; d.Epub = d_Epub; d.err = d_err;
@@ -109,7 +111,7 @@ struct pt_ctx {
 
 namespace {
 
-bool field_fits(int L, int q) { return ptk::field_smem_bytes(L, q) + 256 <= kSmemLimit; }
+bool field_fits(int L, int q) { return ptk::field_smem_bytes(L, q) + 512 <= kSmemLimit; }
 bool direct_applies(int L, int q) { return ptk::direct_applies(L, q); }
 
 void free_ctx(pt_ctx* c) {
@@ -130,7 +132,7 @@ int recompute_energy(pt_ctx* c, long long* d_out) {
         if (rc) return fail(PT_ECUDA, std::string("energy_direct launch: ") + cudaGetErrorString((cudaError_t)rc));
         return PT_OK;
     }
-    const size_t smem = (size_t)(c->L + c->L / 8) * 4;
+    const size_t smem = (size_t)(c->L + c->words()) * 4;
     if (smem > 48 * 1024) PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::energy_kernel, 1024));
     ptk::energy_kernel<<<c->R(), 256, smem, c->stream>>>(c->dev(), d_out);
     PT_CUDA(cudaGetLastError());
@@ -140,7 +142,7 @@ int recompute_energy(pt_ctx* c, long long* d_out) {
 int ensure_fields(pt_ctx* c) {
     if (c->fields_valid) return PT_OK;
     if (!c->d_h) PT_CUDA(cudaMalloc(&c->d_h, (size_t)c->R() * c->q * c->L * sizeof(int32_t)));
-    const size_t smem = (size_t)(c->L + c->L / 8) * 4;
+    const size_t smem = (size_t)(c->L + c->words()) * 4;
     if (smem > 48 * 1024) PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::build_fields_kernel, 1024));
     ptk::build_fields_kernel<<<c->R(), 256, smem, c->stream>>>(c->dev());
     PT_CUDA(cudaGetLastError());
@@ -197,15 +199,12 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
         }
     } else if (c->variant == PT_VARIANT_FIELD) {
         const size_t smem = ptk::field_smem_bytes(c->L, c->q, c->site_order == PT_ORDER_RANDOM);
-        if (c->site_order == PT_ORDER_RANDOM) {
-            PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::sweep_field_kernel<true>, 1024));
-            ptk::sweep_field_kernel<true><<<c->R(), ptk::FIELD_THREADS, smem, c->stream>>>(d, (long long)c->sweep, n_sweeps,
-                                                                                           swap_mode == 1 ? 1 : 0);
-        } else {
-            PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::sweep_field_kernel<false>, 1024));
-            ptk::sweep_field_kernel<false><<<c->R(), ptk::FIELD_THREADS, smem, c->stream>>>(d, (long long)c->sweep, n_sweeps,
-                                                                                            swap_mode == 1 ? 1 : 0);
-        }
+        typedef void (*field_kernel_t)(ptk::Dev, long long, int, int);
+        const bool rnd = c->site_order == PT_ORDER_RANDOM, wide = c->bits() == 8;
+        const field_kernel_t kern = rnd ? (wide ? ptk::sweep_field_kernel<true, 8> : ptk::sweep_field_kernel<true, 4>)
+                                        : (wide ? ptk::sweep_field_kernel<false, 8> : ptk::sweep_field_kernel<false, 4>);
+        PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)kern, 1024));
+        kern<<<c->R(), ptk::FIELD_THREADS, smem, c->stream>>>(d, (long long)c->sweep, n_sweeps, swap_mode == 1 ? 1 : 0);
     } else {
         c->fields_valid = false;
         if (!c->direct_kern) c->direct_kern = ptk::select_direct_kernel(d, c->r_hi, c->device, &c->coresident);
@@ -244,7 +243,7 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
     *out = nullptr;
     if (L < 8 || (L % 8) != 0) return fail(PT_EINVAL, "L must be >= 8 and a multiple of 8");
     if (L > (1 << 20)) return fail(PT_EINVAL, "L too large");
-    if (q < 2 || q > 16) return fail(PT_EINVAL, "q must be in 2..16");
+    if (q < 2 || q > ptk::PT_QMAX) return fail(PT_EINVAL, "q must be in 2..64");
     if (!(sigma > 0.0) || !std::isfinite(sigma)) return fail(PT_EINVAL, "sigma must be finite and > 0");
     if (n_ens < 1 || n_rep < 1) return fail(PT_EINVAL, "n_ens and n_rep must be >= 1");
     if ((long long)n_ens * n_rep > (1 << 24)) return fail(PT_EINVAL, "too many replicas");
@@ -275,7 +274,7 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
     c->L = L; c->q = q; c->sigma = sigma; c->n_ens = n_ens; c->n_rep = n_rep; c->seed = seed;
     c->ens_base = ens_base; c->device = dev; c->variant = variant;
     const int R = c->R();
-    const int W = L / 8;
+    const int W = q <= 16 ? L / 8 : L / 4;
 
 #define PT_CUDA_C(call)                                                                                   \
     do {                                                                                                  \
@@ -469,7 +468,7 @@ int pt_observables(pt_ctx* c, pt_obs* out) {
 int pt_get_spins_dev(pt_ctx* c, uint8_t* out_dev) {
     if (!c || !out_dev) return fail(PT_EINVAL, "NULL argument");
     DeviceGuard guard(c->device);
-    const long long nwords = (long long)c->R() * (c->L / 8);
+    const long long nwords = (long long)c->R() * c->words();
     ptk::unpack_spins_kernel<<<(unsigned)((nwords + 255) / 256), 256, 0, c->stream>>>(c->dev(), out_dev);
     PT_CUDA(cudaGetLastError());
     return pt_sync(c);
@@ -501,7 +500,7 @@ int upload_spins(pt_ctx* c, const uint8_t* in) {
     PT_CUDA(cudaMemcpyAsync(&flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     PT_CUDA(cudaStreamSynchronize(c->stream));
     if (flag) return fail(PT_EINVAL, "colour outside 1..q");
-    const long long nwords = (long long)c->R() * (c->L / 8);
+    const long long nwords = (long long)c->R() * c->words();
     ptk::pack_spins_kernel<<<(unsigned)((nwords + 255) / 256), 256, 0, c->stream>>>(c->dev(), c->d_stage);
     PT_CUDA(cudaGetLastError());
     c->fields_valid = false;

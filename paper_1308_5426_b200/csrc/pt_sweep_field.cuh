@@ -29,13 +29,16 @@ constexpr int FIELD_THREADS = 512;
 // colour a -- and with it the proposed colour k + (k >= a) -- is read at the step's turn, not at the start of the
 // sweep; the scan over 32 consecutive STEPS is otherwise the same: the first accepting step is the next change.
 //
+// BITS: 4 bits per spin (q <= 16, W = L/8 words) or 8 (16 < q <= 64, W = L/4 words); the arithmetic is the same.
+//
 // dynamic smem layout (32-bit words): J[L] | theta[L] | sp[W] | bq[W] | h[q*L]
 //                            RANDOM: J[L] | theta[L] | sp[W] | site[L] | kk[L/4] | h[q*L]
 __host__ __device__ inline size_t field_smem_bytes(int L, int q, bool random_order = false) {
-    return (size_t)(2 * L + (L / 8) + (random_order ? L + L / 4 : L / 8) + q * L) * 4;
+    const int W = q <= 16 ? L / 8 : L / 4;
+    return (size_t)(2 * L + W + (random_order ? L + L / 4 : W) + q * L) * 4;
 }
 
-template <bool RANDOM>
+template <bool RANDOM, int BITS>
 __global__ void __launch_bounds__(FIELD_THREADS, 1)
 sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
     extern __shared__ uint32_t smem_f[];
@@ -48,7 +51,9 @@ sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
     uint8_t* kk = (uint8_t*)(site + L);                     // ... and its draw k in 0..q-2
     int32_t* h = RANDOM ? (int32_t*)(kk + L) : (int32_t*)(bq + W);
     __shared__ int s_flip[5];
-    __shared__ int s_cnt[16];
+    __shared__ int s_cnt[PT_QMAX];
+    constexpr int PER = 32 / BITS;
+    constexpr uint32_t CMASK = (1u << BITS) - 1u;
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int e = blockIdx.x / d.n_rep, t = blockIdx.x % d.n_rep;
@@ -76,18 +81,18 @@ sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
                 theta[n] = accept_threshold(uniform53(p.w1, p.w2), scale);
             }
         }
-        // proposals and thresholds of all sites (A6, A7, A9), one word of 8 sites per thread
+        // proposals and thresholds of all sites (A6, A7, A9), one word of PER sites per thread
         for (int w = tid; !RANDOM && w < W; w += FIELD_THREADS) {
             const uint32_t word = sp[w];
             uint32_t bword = 0;
 #pragma unroll
-            for (int n = 0; n < 8; ++n) {
-                const int i = 8 * w + n;
+            for (int n = 0; n < PER; ++n) {
+                const int i = PER * w + n;
                 const Philox4 p = philox4x32_10((uint32_t)i, sweep, (uint32_t)t, c3, d.key0, d.key1);
-                const uint32_t a = (word >> (4 * n)) & 15u;
+                const uint32_t a = (word >> (BITS * n)) & CMASK;
                 const uint32_t k = __umulhi(p.w0, (uint32_t)(q - 1));
                 const uint32_t b = k + (k >= a ? 1u : 0u);
-                bword |= b << (4 * n);
+                bword |= b << (BITS * n);
                 theta[i] = accept_threshold(uniform53(p.w1, p.w2), scale);
             }
             bq[w] = bword;
@@ -104,9 +109,9 @@ sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
                     bool acc = false;
                     if (n < L) {
                         if (RANDOM) i = site[n];
-                        a = get_nibble(sp, i);
+                        a = get_colour(sp, i, BITS);
                         if (RANDOM) { const int k = kk[n]; b = k + (k >= a ? 1 : 0); }
-                        else b = get_nibble(bq, i);
+                        else b = get_colour(bq, i, BITS);
                         dE = h[a * L + i] - h[b * L + i];
                         acc = dE <= theta[n];
                     }
@@ -136,8 +141,8 @@ sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
                 hb[j] += Jv;
             }
             if (tid == 0) {
-                const int sh = (fs & 7) << 2;
-                sp[fs >> 3] = (sp[fs >> 3] & ~(15u << sh)) | ((uint32_t)b << sh);
+                const int sh = (fs % PER) * BITS;
+                sp[fs / PER] = (sp[fs / PER] & ~(CMASK << sh)) | ((uint32_t)b << sh);
                 E += s_flip[3];
                 oa.acc += 1;
             }
@@ -145,7 +150,7 @@ sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
             __syncthreads();
         }
         // a8: sample after the sweep, before the swap event (A15)
-        const int nmax = count_nmax(sp, W, q, s_cnt);
+        const int nmax = count_nmax(sp, W, q, BITS, s_cnt);
         if (tid == 0) { oa.att += L; oa.sample(E, nmax); }
         __syncthreads();
     }

@@ -57,7 +57,7 @@ sweep_float_kernel(Dev d, double* __restrict__ Ef, long long sweep0, int n_sweep
     uint8_t* c = reinterpret_cast<uint8_t*>(us + L);
     uint8_t* bq = c + L;
     __shared__ T s_part[FLOAT_THREADS];
-    __shared__ int s_cnt[16];
+    __shared__ int s_cnt[PT_QMAX];
     __shared__ int s_last;
 
     const int tid = threadIdx.x;
@@ -66,7 +66,7 @@ sweep_float_kernel(Dev d, double* __restrict__ Ef, long long sweep0, int n_sweep
     const size_t x = (size_t)e * d.n_rep + st;
     uint32_t* g_sp = d.spins + x * W;
     for (int r = tid; r < L; r += FLOAT_THREADS) Jf[r] = (T)ldexp((double)d.Jq[r], -24);
-    for (int i = tid; i < L; i += FLOAT_THREADS) c[i] = (uint8_t)get_nibble(g_sp, i);
+    for (int i = tid; i < L; i += FLOAT_THREADS) c[i] = (uint8_t)get_colour(g_sp, i, d.bits);
     T E = (T)Ef[x];                       // thread 0's copy is the running energy
     const double beta = d.beta[t];
     const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_SWEEP;
@@ -120,7 +120,7 @@ sweep_float_kernel(Dev d, double* __restrict__ Ef, long long sweep0, int n_sweep
             __syncthreads();
         }
         // a8: sample after the sweep (A15); the accumulators see the running energy in fixed point
-        if (tid < 16) s_cnt[tid] = 0;
+        if (tid < PT_QMAX) s_cnt[tid] = 0;
         __syncthreads();
         for (int i = tid; i < L; i += FLOAT_THREADS) atomicAdd(&s_cnt[c[i]], 1);
         __syncthreads();
@@ -136,8 +136,8 @@ sweep_float_kernel(Dev d, double* __restrict__ Ef, long long sweep0, int n_sweep
 
     for (int w = tid; w < W; w += FLOAT_THREADS) {
         uint32_t word = 0;
-#pragma unroll
-        for (int n = 0; n < 8; ++n) word |= (uint32_t)c[8 * w + n] << (4 * n);
+        const int per = 32 / d.bits;
+        for (int n = 0; n < per; ++n) word |= (uint32_t)c[per * w + n] << (d.bits * n);
         g_sp[w] = word;
     }
     if (tid == 0) {

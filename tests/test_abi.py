@@ -48,7 +48,7 @@ def test_no_cpu_fallback(lib_path):
 
 def test_argument_validation_before_any_device_work(lib_path):
     from paper_1308_5426_b200 import pt
-    for kw in [dict(L=12), dict(q=1), dict(q=17), dict(sigma=-0.5), dict(n_ens=0), dict(betas=[float("inf"), 1.0])]:
+    for kw in [dict(L=12), dict(q=1), dict(q=65), dict(sigma=-0.5), dict(n_ens=0), dict(betas=[float("inf"), 1.0])]:
         args = dict(L=64, q=3, sigma=0.5, n_ens=1, n_rep=2, betas=[1.0, 0.5], seed=1)
         args.update(kw)
         with pytest.raises(pt.PTError) as ei:

@@ -196,6 +196,68 @@ def test_ragged_and_edge_shapes(pt, oracle):
         assert_same_state(g, o, "shape L=%d q=%d" % (L, q))
 
 
+@pytest.mark.parametrize("L,q,sigma,n_ens,n_rep", [(64, 17, 0.5, 2, 5), (200, 33, 0.45, 1, 4), (512, 64, 0.8, 1, 3),
+                                                  (1024, 24, 0.3, 1, 6)])
+def test_more_than_16_colours(pt, oracle, L, q, sigma, n_ens, n_rep):
+    """SURVEY.md 8(f) NEXT-2, "q > 16 (wider packing)": 8 bits per spin (4 sites per word) in the field variant
+    (sequential and random site order) and the floating-point variants; the direct kernels (nibble tables) refuse.
+    Hot start, sweeps with swaps, set_spins / get_spins, recount, state round trip: all bit-identical to the oracle."""
+    b = inputs.geometric_betas(0.5, 2.5, n_rep)
+    g = pt.PT(L, q, sigma, n_ens, n_rep, b, 1717)
+    o = oracle.Oracle(L, q, sigma, n_ens, n_rep, b, 1717)
+    assert g.get_variant() == "field"
+    assert g.get_spins().max() > 16 and g.get_spins().max() <= q
+    assert_same_state(g, o, "hot start q=%d" % q)
+    np.testing.assert_array_equal(g.energy(recompute=True), o.energy(recompute=True))
+    with pytest.raises(pt.PTError):
+        g.set_variant("direct")
+    for k in (1, 30):
+        g.sweeps(k, 1)
+        o.sweeps(k, 1, field=True, threads=THREADS)
+        assert_same_state(g, o, "q=%d after +%d" % (q, k))
+    s = inputs.random_spins(n_ens, n_rep, L, q, seed=q)
+    g.set_spins(s)
+    o.set_spins(s)
+    np.testing.assert_array_equal(g.get_spins(), s)
+    bad = s.copy()
+    bad[0, 0, 3] = q + 1
+    with pytest.raises(pt.PTError):
+        g.set_spins(bad)
+    g.sweeps(7, 3)
+    o.sweeps(7, 3, field=True, threads=THREADS)
+    assert_same_state(g, o, "q=%d after set_spins" % q)
+    # checkpoint / resume through pt_get_state / pt_set_state
+    st = g.get_state()
+    g2 = pt.PT(L, q, sigma, n_ens, n_rep, b, 1717)
+    g2.set_state(*st)
+    for h in (g, g2):
+        h.set_site_order("random")
+    o.set_site_order("random")
+    g.sweeps(9, 1)
+    g2.sweeps(9, 1)
+    o.sweeps(9, 1, field=True, threads=THREADS)
+    assert_same_state(g, o, "q=%d random order" % q)
+    np.testing.assert_array_equal(g2.get_spins(), g.get_spins())
+    np.testing.assert_array_equal(g2.energy(), g.energy())
+    for h in (g, g2):
+        h.set_site_order("sequential")
+    o.set_site_order("sequential")
+    g.set_variant("fp64")            # exact sums: the integer trajectory
+    g.sweeps(4, 1)
+    o.sweeps(4, 1, field=True, threads=THREADS)
+    np.testing.assert_array_equal(g.get_spins(), o.get_spins())
+    np.testing.assert_array_equal(g.energy(), o.energy())
+    np.testing.assert_array_equal(g.energy(recompute=True), o.energy())
+    for h in (g, g2, o):
+        h.close()
+
+
+def test_field_table_capacity_beyond_16_colours(pt):
+    """L*q*4 bytes of local fields must fit in shared memory: q = 64 at L = 1024 does not (PT_ECAPACITY)."""
+    with pytest.raises(pt.PTError):
+        pt.PT(1024, 64, 0.5, 1, 2, [0.5, 1.0], 1)
+
+
 def test_ens_base_shards_ensembles(pt, oracle):
     """Two contexts with ens_base 0 and 2 reproduce ensembles 0-1 and 2-3 of one 4-ensemble context."""
     L, q, n_rep = 64, 3, 4
@@ -216,7 +278,7 @@ def test_errors(pt):
     with pytest.raises(pt.PTError) as ei:
         pt.PT(12, 3, 0.5, 1, 1, [1.0], 1)
     assert ei.value.code == -1
-    for bad in [dict(q=1), dict(q=17), dict(sigma=0.0), dict(sigma=float("nan")), dict(betas=[-1.0])]:
+    for bad in [dict(q=1), dict(q=65), dict(sigma=0.0), dict(sigma=float("nan")), dict(betas=[-1.0])]:
         kw = dict(L=64, q=3, sigma=0.5, n_ens=1, n_rep=1, betas=[1.0], seed=1)
         kw.update(bad)
         with pytest.raises(pt.PTError):

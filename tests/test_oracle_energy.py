@@ -25,7 +25,7 @@ def make(oracle, L, q, sigma, n_rep=3, seed=7):
     return oracle.Oracle(L, q, sigma, 1, n_rep, np.linspace(0.3, 1.2, n_rep), seed)
 
 
-@pytest.mark.parametrize("L,q,sigma", [(8, 3, 0.5), (16, 2, 0.3), (64, 5, 0.8), (128, 16, 0.1)])
+@pytest.mark.parametrize("L,q,sigma", [(8, 3, 0.5), (16, 2, 0.3), (64, 5, 0.8), (128, 16, 0.1), (64, 37, 0.6), (48, 64, 0.4)])
 def test_total_energy_matches_definition(oracle, L, q, sigma):
     o = make(oracle, L, q, sigma)
     Jq = o.get_couplings().astype(np.int64)
@@ -59,7 +59,7 @@ def test_hot_start_is_philox_uniform(oracle):
     assert cnt.min() > 40 and cnt.max() < 120
 
 
-@pytest.mark.parametrize("L,q,sigma", [(8, 3, 0.5), (32, 4, 0.4), (64, 8, 0.3)])
+@pytest.mark.parametrize("L,q,sigma", [(8, 3, 0.5), (32, 4, 0.4), (64, 8, 0.3), (40, 29, 0.7)])
 def test_delta_e_is_energy_difference(oracle, L, q, sigma):
     """T4: dE(i, a->b) == E(after) - E(before), both by the O(L^2) definition above."""
     o = make(oracle, L, q, sigma, n_rep=1)

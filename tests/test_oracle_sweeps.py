@@ -99,10 +99,11 @@ def test_chain_samples_exact_boltzmann_L8_q3(oracle, swap_every, field):
     assert ob["near_ties"].sum() == 0
 
 
-def test_beta_zero_delta_is_one_over_q(oracle):
+@pytest.mark.parametrize("q", [4, 20])
+def test_beta_zero_delta_is_one_over_q(oracle, q):
     """beta=0: every proposal accepted, stationary law uniform, <delta>=1/q so
-    <E> = -(1/q)(L/2) sum_r Jq[r] (north_star pin)."""
-    L, q = 32, 4
+    <E> = -(1/q)(L/2) sum_r Jq[r] (north_star pin); q = 20: the same closed form beyond 16 colours."""
+    L = 32
     o = oracle.Oracle(L, q, 0.5, 1, 2, [0.0, 0.0], 3)
     Jsum = int(o.get_couplings().astype(np.int64).sum())
     o.sweeps(100, swap_every=1)
@@ -140,10 +141,11 @@ def replay_sweep(oracle, c, E, Jq, q, beta, key, sweep, slot, ens):
     return c, E
 
 
-def test_sweep_and_swap_replay_in_python(oracle):
+@pytest.mark.parametrize("q", [3, 23])
+def test_sweep_and_swap_replay_in_python(oracle, q):
     """Site order, counter layout, proposal rule, strict u<p, swap stages and slot keying:
-    three sweeps with swaps replayed here and compared bit for bit."""
-    L, q, R, ens = 16, 3, 4, 1
+    three sweeps with swaps replayed here and compared bit for bit (q = 23: more than 16 colours)."""
+    L, R, ens = 16, 4, 1
     seed = 0x0123456789ABCDEF
     key = [seed & 0xFFFFFFFF, seed >> 32]
     betas = np.array([1.1, 0.9, 0.6, 0.3])
@@ -174,7 +176,7 @@ def test_sweep_and_swap_replay_in_python(oracle):
     assert o.sweep_counter() == 3
 
 
-@pytest.mark.parametrize("L,q,sigma,R", [(64, 3, 0.5, 8), (128, 8, 0.3, 5)])
+@pytest.mark.parametrize("L,q,sigma,R", [(64, 3, 0.5, 8), (128, 8, 0.3, 5), (64, 33, 0.5, 4)])
 def test_field_mode_equals_direct_mode_and_recount(oracle, L, q, sigma, R):
     """north_star pin: incremental local-field energy == O(L^2) recompute after every sweep,
     and the field trajectory is the direct-sum trajectory bit for bit."""
@@ -235,7 +237,7 @@ def test_swap_invariants(oracle):
 
 
 def test_create_rejects_invalid_arguments(oracle):
-    bad = [dict(L=7), dict(L=0), dict(q=1), dict(q=17), dict(sigma=0.0), dict(sigma=float("nan")),
+    bad = [dict(L=7), dict(L=0), dict(q=1), dict(q=65), dict(sigma=0.0), dict(sigma=float("nan")),
            dict(n_ens=0), dict(betas=[-1.0, 1.0]), dict(sigma=0.01, L=4096)]
     for kw in bad:
         args = dict(L=16, q=3, sigma=0.5, n_ens=1, n_rep=2, betas=[0.5, 1.0], seed=1)
