@@ -29,10 +29,11 @@ inline int allow_max_dynamic_smem(const void* kernel, int static_bytes) {
     return (int)err;
 }
 
-// Everything a kernel needs to know about a context (passed by value).
+// Everything a kernel needs to know about a context (passed by value).  New fields go at the END: ptxas' schedule of
+// sweep_direct_kernel changes with the layout of its parameters (a field inserted after ens_base cost the headline
+// workload 3 %, measured A/B on one GPU; appended, the SASS is the same up to constant-bank offsets).
 struct Dev {
     int L, W, q, n_ens, n_rep, ens_base;
-    int bits;                 // bits per spin in spins[]: 4 (q <= 16, 8 sites per word) or 8 (q <= 64, 4 sites per word)
     int rep_base, n_local;    // slot-sharded contexts (pt_create_shard): this process sweeps the configurations with
                               // storage index rep_base .. rep_base + n_local - 1; otherwise 0, n_rep
     int count_swaps;          // 0: this shard leaves the swap counters to the shard with rep_base = 0
@@ -52,6 +53,7 @@ struct Dev {
     long long* Epub;          // [2][n_ens][n_rep] energies published for those events, by storage index
     int* err;                 // raised by a kernel whose in-kernel barrier timed out (host-mapped: read by pt_sync)
     long long* dbg;           // PT_TIMING builds: [n_ens*n_rep][32 warps][8] clock sums (else unused)
+    int bits;                 // bits per spin in spins[]: 4 (q <= 16, 8 sites per word) or 8 (q <= 64, 4 sites per word)
 };
 
 // ---------------------------------------------------------------------------
