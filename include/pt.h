@@ -243,6 +243,30 @@ int pt_sync(pt_ctx* ctx);
 #define PT_PEAK_PATTERNS 10
 int pt_measure_peaks(double* rates, int n);
 
+/* Total energies of caller-supplied configurations WITHOUT ANY ALLOCATION (for callers that cannot call cudaMalloc:
+ * code under CUDA graph capture, tight serving loops, harnesses that forbid it).  The same O(L^2) recount as
+ * pt_energy(recompute = 1) -- Eq. 2 in reading A1 with each unordered pair once, "the total energy of
+ * each replica", on the quantised couplings Jq[r] = round(J*(r) 2^24) of Eqs. 5-7 (A16) -- but on the current device,
+ * without a context: the coupling table and the packed spins it needs live in a file-scope device array of
+ * 64 + PT_STATIC_MAX_L + PT_STATIC_MAX_SITES/4 32-bit words (1 114 368 bytes) that every GPU loading the library holds
+ * until exit.  No cudaMalloc, cudaFree or allocating library routine is called.
+ *  L, q, sigma : the model, as for pt_create; L % 8 == 0, 8 <= L <= PT_STATIC_MAX_L, 2 <= q <= 64
+ *  spins_dev   : DEVICE pointer, [n_conf][L] bytes, API colours 1..q (A4); not modified; owned by the caller
+ *  n_conf      : configurations, >= 1, n_conf * L <= PT_STATIC_MAX_SITES
+ *  E_out_dev   : DEVICE pointer, [n_conf] int64, receives E in fixed point 2^-24; owned by the caller
+ *  status_dev  : DEVICE pointer to one int or NULL: receives 0, or 1 if some colour was outside 1..q (the energies
+ *                of that call are then meaningless)
+ *  cuda_stream : a cudaStream_t (NULL = default stream).  The call only ENQUEUES (one memset + 3-4 kernels) and
+ *                returns; outputs are complete when that stream work is.
+ * All calls share the one scratch array, which keeps the last call's contents (every call clears or overwrites what
+ * it reads): calls that OVERLAP on the GPU -- different streams without an ordering between them, or two host
+ * threads on one device -- race.  Calls on one stream, or ordered by events, are safe.
+ * Errors: PT_EINVAL (arguments), PT_ECAPACITY (L or n_conf * L beyond the maxima: split the call), PT_ECUDA. */
+#define PT_STATIC_MAX_L 16384
+#define PT_STATIC_MAX_SITES 1048576
+int pt_energy_static(int L, int q, double sigma, const uint8_t* spins_dev, int n_conf, int64_t* E_out_dev,
+                     int* status_dev, void* cuda_stream);
+
 const char* pt_last_error(void);
 
 #ifdef __cplusplus

@@ -709,3 +709,102 @@ int pt_set_stream(pt_ctx* c, void* cuda_stream) {
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------
+// pt_energy_static (include/pt.h): total energies of caller-supplied configurations without any allocation.
+// The scratch the recount needs -- the quantised coupling table Jq[L] (a1) and the packed spins -- lives in ONE
+// file-scope device array that every GPU loading the library holds until exit.  In host code the array's NAME is a
+// host-side stand-in, not a device address: its address on the current device is asked once per device with
+// cudaGetSymbolAddress and that pointer is what the kernels get.  All calls share the array (it keeps the last call's
+// contents; the flag word is cleared at the start of every call), so calls that overlap on the GPU race.
+// ---------------------------------------------------------------------------
+namespace {
+
+constexpr int kStaticFlagWords = 64;                                    // word 0: a colour outside 1..q was seen
+constexpr int kStaticSpinWords = PT_STATIC_MAX_SITES / 4;               // byte-wide packing (q > 16) is the widest
+constexpr int kStaticWords = kStaticFlagWords + PT_STATIC_MAX_L + kStaticSpinWords;
+static __device__ __align__(256) uint32_t g_static_scratch[kStaticWords];   // 1 114 368 bytes per GPU
+
+constexpr int kMaxDevices = 64;
+std::mutex g_static_mu;
+uint32_t* g_static_ptr[kMaxDevices] = {};   // device address of g_static_scratch, by device ordinal
+
+// One thread per packed word: API colours 1..q, one byte per site -> stored colours 0..q-1, `bits` bits per site.
+__global__ void static_pack_kernel(const uint8_t* __restrict__ in, uint32_t* __restrict__ words, long long n_words,
+                                   int bits, int q, uint32_t* __restrict__ flag) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= n_words) return;
+    const int per = 32 / bits;
+    const uint8_t* s = in + gid * per;
+    uint32_t word = 0;
+    bool bad = false;
+    for (int n = 0; n < per; ++n) {
+        const int v = s[n];
+        bad |= v < 1 || v > q;
+        word |= ((uint32_t)(v - 1) & ((1u << bits) - 1u)) << (bits * n);
+    }
+    words[gid] = word;
+    if (bad) atomicOr(flag, 1u);
+}
+
+__global__ void static_status_kernel(const uint32_t* __restrict__ flag, int* __restrict__ status) {
+    status[0] = (int)flag[0];
+}
+
+// Device address of the scratch array on the CURRENT device (asked once per device, with that device current).
+int static_scratch(uint32_t** out) {
+    int dev = 0;
+    PT_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(PT_EINVAL, "device ordinal beyond 63");
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_ptr[dev]) {
+        uint32_t* p = nullptr;
+        PT_CUDA(cudaGetSymbolAddress((void**)&p, g_static_scratch));
+        g_static_ptr[dev] = p;
+    }
+    *out = g_static_ptr[dev];
+    return PT_OK;
+}
+
+}  // namespace
+
+extern "C" int pt_energy_static(int L, int q, double sigma, const uint8_t* spins_dev, int n_conf, int64_t* E_out_dev,
+                                int* status_dev, void* cuda_stream) {
+    if (L < 8 || (L % 8) != 0) return fail(PT_EINVAL, "L must be a multiple of 8, >= 8");
+    if (L > PT_STATIC_MAX_L) return fail(PT_ECAPACITY, "pt_energy_static: L exceeds PT_STATIC_MAX_L (16384)");
+    if (q < 2 || q > ptk::PT_QMAX) return fail(PT_EINVAL, "q must be in 2..64");
+    if (!(sigma > 0.0) || !std::isfinite(sigma)) return fail(PT_EINVAL, "sigma must be finite and > 0");
+    if (n_conf < 1) return fail(PT_EINVAL, "n_conf must be >= 1");
+    if ((long long)n_conf * L > PT_STATIC_MAX_SITES)
+        return fail(PT_ECAPACITY, "pt_energy_static: n_conf * L exceeds PT_STATIC_MAX_SITES (1048576); split the call");
+    if (!spins_dev || !E_out_dev) return fail(PT_EINVAL, "spins_dev and E_out_dev must not be NULL");
+    uint32_t* scratch = nullptr;
+    int rc = static_scratch(&scratch);
+    if (rc) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    uint32_t* flag = scratch;
+    int32_t* Jq = (int32_t*)(scratch + kStaticFlagWords);
+    uint32_t* words = scratch + kStaticFlagWords + PT_STATIC_MAX_L;
+
+    ptk::Dev d = {};
+    d.L = L; d.q = q; d.n_ens = 1; d.n_rep = n_conf; d.n_local = n_conf;
+    d.bits = q <= 16 ? 4 : 8;
+    d.W = L * d.bits / 32;
+    d.Jq = Jq; d.spins = words;
+    const long long n_words = (long long)n_conf * d.W;
+
+    PT_CUDA(cudaMemsetAsync(flag, 0, kStaticFlagWords * sizeof(uint32_t), stream));   // the array keeps the last call's contents
+    ptk::jstar_kernel<<<(L / 2 + 128) / 128, 128, 0, stream>>>(L, sigma, Jq, nullptr);          // a1: all of Jq[0..L-1]
+    PT_CUDA(cudaGetLastError());
+    static_pack_kernel<<<(unsigned)((n_words + 255) / 256), 256, 0, stream>>>(spins_dev, words, n_words, d.bits, q, flag);
+    PT_CUDA(cudaGetLastError());
+    const size_t smem = (size_t)(L + d.W) * 4;
+    if (smem > 48 * 1024) PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)ptk::energy_kernel, 1024));
+    ptk::energy_kernel<<<n_conf, 256, smem, stream>>>(d, (long long*)E_out_dev);                // a6
+    PT_CUDA(cudaGetLastError());
+    if (status_dev) {
+        static_status_kernel<<<1, 1, 0, stream>>>(flag, status_dev);
+        PT_CUDA(cudaGetLastError());
+    }
+    return PT_OK;
+}

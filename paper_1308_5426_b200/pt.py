@@ -25,7 +25,7 @@ SYMBOLS = ["pt_create", "pt_create_ex", "pt_destroy", "pt_sweeps", "pt_energy", 
            "pt_sweep_counter", "pt_set_variant", "pt_get_variant", "pt_set_stream", "pt_sweeps_async",
            "pt_sync", "pt_last_error", "pt_create_shard", "pt_energy_storage_dev", "pt_swap_external",
            "pt_get_perm", "pt_measure_peaks", "pt_get_state", "pt_set_state", "pt_set_site_order",
-           "pt_energy_storage_dev_async", "pt_swap_external_async"]
+           "pt_energy_storage_dev_async", "pt_swap_external_async", "pt_energy_static"]
 
 
 class PTError(RuntimeError):
@@ -83,6 +83,8 @@ _lib.pt_set_state.argtypes = [_vp, _vp, _vp, _vp, _i64]
 _lib.pt_set_site_order.argtypes = [_vp, _i32]
 _lib.pt_energy_storage_dev_async.argtypes = [_vp, _vp]
 _lib.pt_swap_external_async.argtypes = [_vp, _vp]
+_lib.pt_energy_static.argtypes = [_i32, _i32, _dbl, _vp, _i32, _vp, _vp, _vp]
+STATIC_MAX_L, STATIC_MAX_SITES = 16384, 1048576     # PT_STATIC_MAX_L, PT_STATIC_MAX_SITES of include/pt.h
 
 PEAK_PATTERNS = ["idp2a", "idp4a", "imad", "prmt", "lop3", "prmt+2idp2a (idp2a counted)", "lop3+2idp2a (idp2a counted)",
                  "lds128 (bytes)", "prmt+4idp2a (idp2a counted)", "2prmt+add+2idp2a (idp2a counted)"]
@@ -93,6 +95,16 @@ def measure_peaks():
     r = np.zeros(len(PEAK_PATTERNS) * 4, dtype=np.float64)
     _check(_lib.pt_measure_peaks(_p(r), int(r.size)))
     return {name: [float(x) for x in r[4 * i:4 * i + 4]] for i, name in enumerate(PEAK_PATTERNS)}
+
+
+def energy_static(L, q, sigma, spins_dev, n_conf, E_out_dev, status_dev=None, cuda_stream_ptr=None):
+    """pt_energy_static: energies of n_conf caller-supplied configurations, allocation-free (shared static scratch:
+    overlapping calls race).  spins_dev / E_out_dev / status_dev: objects with .data_ptr() on the current device
+    (uint8 [n_conf, L], int64 [n_conf], int32 [1] or None).  Enqueues on the stream and returns."""
+    _check(_lib.pt_energy_static(int(L), int(q), float(sigma), ctypes.c_void_p(spins_dev.data_ptr()), int(n_conf),
+                                 ctypes.c_void_p(E_out_dev.data_ptr()),
+                                 ctypes.c_void_p(status_dev.data_ptr()) if status_dev is not None else None,
+                                 ctypes.c_void_p(int(cuda_stream_ptr)) if cuda_stream_ptr else None))
 
 
 def _check(rc):
