@@ -66,7 +66,9 @@ typedef enum {
  * Environment: PT_VARIANT=direct|field|auto sets the variant chosen by pt_create; PT_PERSISTENT=0|1|2 the launch
  * policy of the direct variant (0: one launch per swap interval; 1, default: persistent launches with the swap events
  * inside the kernel for contexts that take at least a third of the SMs; 2: whenever all replicas can be co-resident);
- * PT_MINB=1|2 forces the 168- or the 80-register build of the direct sweep kernel (experiments; default: by size). */
+ * PT_MINB=1|2 forces the 168- or the 80-register build of the direct sweep kernel (experiments; default: by size).
+ * PT_FAR=1 (L = 4096, q <= 8) selects the far form of the bulk sum (8-bit coupling residuals beyond 1000 sites;
+ * bit-identical results, measured slower than the default form: an experiment kept for reference). */
 enum { PT_VARIANT_AUTO = 0, PT_VARIANT_FIELD = 1, PT_VARIANT_DIRECT = 2, PT_VARIANT_FP32 = 3, PT_VARIANT_FP64 = 4 };
 /* PT_VARIANT_FP32 / PT_VARIANT_FP64: the paper's own arithmetic as a COMPARISON variant ("single
  * precision ... rounding errors"; :110-124: one thread block per replica, each of its 128 threads sums a subset of the

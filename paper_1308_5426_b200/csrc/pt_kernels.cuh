@@ -54,6 +54,9 @@ struct Dev {
     int* err;                 // raised by a kernel whose in-kernel barrier timed out (host-mapped: read by pt_sync)
     long long* dbg;           // PT_TIMING builds: [n_ens*n_rep][32 warps][8] clock sums (else unused)
     int bits;                 // bits per spin in spins[]: 4 (q <= 16, 8 sites per word) or 8 (q <= 64, 4 sites per word)
+    int far;                  // direct variant, L = 4096: the couplings of every far j-range (jr = 16..47) lie within 255 of
+                              // their minimum, which is < 2^15 (pt_sweep_direct.cuh, FAR); at the end of the struct: the
+                              // order of the kernel parameters changes the schedule of the sweep kernel
 };
 
 // ---------------------------------------------------------------------------

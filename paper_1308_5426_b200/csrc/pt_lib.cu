@@ -68,6 +68,7 @@ struct pt_ctx {
     long long rowsum = 0;  // sum_r Jq[r]
     int rep_base = 0, n_local = 0;   // slot-sharded context: local storage indices (n_local = 0: not sharded)
     int r_hi = 0;  // largest r <= L/2 with Jq[r] >= 2^16 (direct variant: reach of the high halves)
+    int far_ok = 0;  // L = 4096: every far j-range of the direct kernel fits 8-bit residuals (pt_sweep_direct.cuh, FAR)
     int32_t* d_Jq = nullptr;
     uint32_t* d_Jpair = nullptr;
     double* d_beta = nullptr;
@@ -105,6 +106,7 @@ struct pt_ctx {
         d.Jq = d_Jq; d.Jpair = d_Jpair; d.beta = d_beta; d.thr_scale = d_scale;
         d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done; d.dbg = d_dbg; d.gen = d_gen; d.Epub = d_Epub; d.err = d_err;
         d.rep_base = rep_base; d.n_local = n_local ? n_local : n_rep; d.count_swaps = rep_base == 0 ? 1 : 0;
+        d.far = far_ok;
         return d;
     }
 };
@@ -335,6 +337,23 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
     for (int r = 1; r <= L / 2; ++r)
         if (Jq[r] >= 65536) c->r_hi = r;
     c->rowsum = rowsum;
+    if (L == 4096 && getenv("PT_FAR") && getenv("PT_FAR")[0] == '1') {   // opt-in: measured slower than the plain form
+        // FAR: the far half of bulk thread (g, jr) holds Jq[r], r = R0 - 45 .. R0 (mod L), R0 = gbase + 14 - (1024 + 32 jr):
+        // it needs max - min <= 255 and 0 < min < 2^15 for every thread
+        bool ok = true;
+        for (int jr = 0; jr < 64 && ok; ++jr)
+            for (int g = 0; g < 4 && ok; ++g) {
+                const int gbase = 16 * (g >> 1) + (g & 1);
+                const int R0 = ((gbase + 14 - (1024 + 32 * jr)) % L + L) % L;
+                int lo = INT32_MAX, hi = 0;
+                for (int n = 0; n < 46; ++n) {
+                    const int v = Jq[((R0 - n) % L + L) % L];
+                    lo = std::min(lo, v); hi = std::max(hi, v);
+                }
+                ok = hi - lo <= 255 && lo < 32768 && lo > 0;
+            }
+        c->far_ok = ok ? 1 : 0;
+    }
     {
         // PT_VARIANT=direct|field|auto overrides the default choice (an impossible request is an error)
         int want = PT_VARIANT_AUTO;

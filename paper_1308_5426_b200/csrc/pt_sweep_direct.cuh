@@ -81,7 +81,7 @@ constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 32 * DIRECT_CHAIN_WARPS;
 // the 80-register build of the same code (768 threads x 80 registers fill the register file of an SM).
 constexpr int DIRECT_BIG_BULK = 640;
 constexpr int DIRECT_BIG_THREADS = DIRECT_BIG_BULK + 32 * DIRECT_CHAIN_WARPS;
-constexpr int DIRECT_STATIC_SMEM = 13 * 1024;   // upper bound of the sweep kernel's static shared memory (12544 B)
+constexpr int DIRECT_STATIC_SMEM = 14 * 1024;   // upper bound of the sweep kernel's static shared memory (13568 B)
 constexpr int DIRECT_NPAIR = 39;   // packed coupling pairs per thread and half: 64 + 2*7 couplings
 constexpr int ENERGY_MAX_THREADS = 512, ENERGY_NPAIR = 35;   // energy_direct_kernel: 4 sites x 64 j per thread
 constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: the 224 sites (56 quads) around a block
@@ -341,13 +341,43 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
 }
 
+// FAR (template parameter; L = 4096, q <= 8, one near quad per thread, and d.far: checked by the host).  Beyond a
+// distance of about 1000 sites the couplings a bulk thread holds differ from their minimum Jmin by less than 256.
+// With Jq = Jmin + res,
+//   sum_j Jq[i-j] s'_i(c_j) = sum_j res[i-j] s'_i(c_j) + Jmin (32 + n_a - n_b),
+// n_c = sites of colour c among the 32 of the range: the first sum takes ONE IDP.4A per four pair terms (8-bit
+// residuals) instead of two IDP.2A, the second is a look-up in the colour counts of the range's block (one PRMT +
+// one IDP.2A per site).  So that every bulk warp gains the same, every thread takes half a near range and half a far
+// range: thread (g, jr) sums the 32 sites j of block kb + jr (jr < 32) resp. kb + 64 + jr (the near half: distances
+// below 1024, IDP.2A on 16-bit halves as before) and the 32 sites of block kb + 32 + jr (the far half).  The counts
+// of a block (s_cnt8: 8 bytes, colours 0..7) are recounted by a bulk warp when the block has been decided; a far
+// range is at least 31 blocks away from the blocks in flight.
+__device__ __forceinline__ uint32_t dp2a_lo_s32_u32(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("dp2a.lo.s32.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+__device__ __forceinline__ uint32_t dp4a_u32_u32(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t d;
+    asm("dp4a.u32.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+    return d;
+}
+// one warp: colour counts of block blk (4 words) -> cnt8[blk]
+__device__ __forceinline__ void recount_block(const uint32_t* sp, uint2* cnt8, int blk, int lane) {
+    const uint32_t x = sp[4 * blk + (lane >> 3)];
+    int v = __popc(match_nibbles(x, (uint32_t)(lane & 7)));
+    v += __shfl_xor_sync(0xffffffffu, v, 8);
+    v += __shfl_xor_sync(0xffffffffu, v, 16);
+    if (lane < 8) reinterpret_cast<uint8_t*>(cnt8 + blk)[lane] = (uint8_t)v;
+}
+
 // NEARQ = 0: the bulk warps sum both 16-bit halves of every coupling.  NEARQ = 1, 2, 4: they sum the low halves
 // only, plus the high halves of NEARQ of the 56 quads of sites within distance 95 of the block (requires
 // r_hi <= 95 and NEARQ * L/64 >= 56).  NJR64: L == 4096 (64 j-ranges as a compile-time constant).
 // MINB: minimum CTAs per SM the register allocation must allow (1: up to 168 registers, for large L; 2: 80 registers,
 // so that several hundred small replicas can be co-resident for persistent launches); 3 stands for the L > 4096
 // build: one CTA of up to DIRECT_BIG_THREADS threads per SM, 80 registers.
-template <int NEARQ, bool NJR64, bool Q16, int MINB>
+template <int NEARQ, bool NJR64, bool Q16, int MINB, bool FAR = false>
 __global__ void __launch_bounds__(MINB == 3 ? DIRECT_BIG_THREADS : DIRECT_MAX_THREADS, MINB == 3 ? 1 : MINB)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi) {
     // swap_mode 0: no swap event; 1: one event at the end of the launch (last-arriving CTA, nobody waits);
@@ -384,6 +414,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     // done[s]: the chain warps have decided the block of buffer s and written its spins (one arrival).
     __shared__ __align__(8) uint64_t s_full[2], s_done[2];
     __shared__ __align__(16) int s_xch[2][32][4];   // partial sums exchanged between the chain warps
+    __shared__ uint2 s_cnt8[128];                   // FAR: colour counts of the 32-site blocks
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int e = swap_mode == 3 ? 0 : blockIdx.x / d.n_rep;
@@ -427,9 +458,51 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         const int NJR = NJR64 ? 64 : L / 64;
         const bool active = jr < NJR;
         // couplings of this thread: pair tt holds Jq[r], Jq[r-1] with r = R0 - 2 tt  (mod L)
-        uint32_t PL[DIRECT_NPAIR];
+        constexpr int NPL = FAR ? 45 : DIRECT_NPAIR;   // FAR: 23 pairs of the near half, 22 fours of the far half
+        uint32_t PL[NPL];
         uint32_t PH[FULL_HI ? DIRECT_NPAIR : 1];
-        {
+        uint32_t jpm = 0u, jmin32 = 0u;   // FAR: Jmin | -Jmin << 16 and 32 Jmin of the far half
+        // FAR: first site of the near half and of the far half, relative to the block start
+        const int jn = jr < 32 ? 32 * jr : L - 1024 + 32 * (jr - 32), jf = 1024 + 32 * jr;
+        if (FAR) {
+            {   // near half: pair tt holds the low halves of Jq[r], Jq[r-1], r = R0 - 2 tt (mod L)
+                const int H = L / 2;
+                const uint32_t* lo = d.Jpair + (size_t)(2 * par) * H;
+                int r = ((gbase + 14 - jn) % L + L) % L;
+#pragma unroll
+                for (int tt = 0; tt < 23; ++tt) {
+                    PL[tt] = __ldg(lo + ((r - par) >> 1));
+                    r -= 2;
+                    r += r < 0 ? L : 0;
+                }
+            }
+            {   // far half: four tt holds Jq[r] - Jmin, .., Jq[r-3] - Jmin, r = R0 - 2 tt (mod L), one byte each
+                const int R0 = ((gbase + 14 - jf) % L + L) % L;
+                int jmin = 0x7fffffff;
+                for (int n = 0; n < 46; ++n) {
+                    int r = R0 - n;
+                    r += r < 0 ? L : 0;
+                    jmin = min(jmin, __ldg(d.Jq + r));
+                }
+                int r = R0;
+#pragma unroll
+                for (int tt = 0; tt < 22; ++tt) {
+                    uint32_t qd = 0u;
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) {
+                        int rc = r - c;
+                        rc += rc < 0 ? L : 0;
+                        qd |= (uint32_t)(__ldg(d.Jq + rc) - jmin) << (8 * c);
+                    }
+                    PL[23 + tt] = qd;
+                    r -= 2;
+                    r += r < 0 ? L : 0;
+                }
+                jpm = ((uint32_t)jmin & 0xffffu) | ((uint32_t)(-jmin) << 16);
+                jmin32 = 32u * (uint32_t)jmin;
+            }
+            PH[0] = 0u;
+        } else {
             const int H = L / 2;
             const int R0 = ((gbase + 14 - 64 * jr) % L + L) % L;
             const uint32_t* lo = d.Jpair + (size_t)(2 * par) * H;
@@ -475,6 +548,8 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         }
         cta_sync();
         if (swap_mode == 3) { t = s_slot; scale = d.thr_scale[t]; }
+        if (FAR)   // colour counts of all blocks (read after the barrier that follows the first DRAW)
+            for (int blk = warp; blk < NB; blk += NTB >> 5) recount_block(m.sp, s_cnt8, blk, lane);
 
         for (int s = 0; s < n_sweeps; ++s) {
             PT_T0(t_draw);
@@ -486,8 +561,10 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             PT_T0(t_loop);
             // per-thread cursors, advanced by one block (32 sites = 4 words) per block
             const uint2* lutp = m.lut + gbase;   // (table of colours 8..15: L entries further)
-            int wj = 8 * jr;                                    // first word of this thread's j-range
+            int wj = FAR ? jn >> 3 : 8 * jr;                    // first word of this thread's j-range (FAR: of its near half)
+            int wjf = jf >> 3;                                  // FAR: first word of the far half
             // the second half of the last range is block kb-1, which is being decided: sweep-start copy
+            // (FAR: the near half of jr = 63 IS block kb-1)
             const uint32_t* sp2 = (jr == NJR - 1) ? m.sp0 : m.sp;
             int wn[NQ];                                         // NEAR: word of quad n = jr + NJR*iq
 #pragma unroll
@@ -500,13 +577,17 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 // also frees buffer kb&1), block kb-1 as at the start of the sweep, blocks >= kb untouched
                 if (kb >= 2) mbar_wait(&s_done[kb & 1], (uint32_t)(phase0 + (kb >> 1) - 1) & 1u);
                 PT_T0(t_b);
+                // FAR: block kb-2 is final: its colour counts (a far range reads them 30 blocks later at the earliest)
+                int rcv = 0;
+                if (FAR && kb >= 2 && warp == (kb & 7))
+                    rcv = __popc(match_nibbles(m.sp[4 * (kb - 2) + (lane >> 3)], (uint32_t)(lane & 7)));
                 uint32_t val[DIRECT_SITES] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
                 if (active) {
                     int wj2 = wj + 4;
                     wj2 -= wj2 >= W ? W : 0;
-                    const uint4 wa = *reinterpret_cast<const uint4*>(m.sp + wj);
-                    const uint4 wb = *reinterpret_cast<const uint4*>(sp2 + wj2);
-                    const uint32_t words[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
+                    const uint4 wa = *reinterpret_cast<const uint4*>((FAR ? sp2 : m.sp) + wj);
+                    const uint4 wb = *reinterpret_cast<const uint4*>(FAR ? m.sp + wjf : sp2 + wj2);
+                    const uint32_t words[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};   // FAR: near half | far half
                     uint2 lt[DIRECT_SITES], ltb[DIRECT_SITES];
 #pragma unroll
                     for (int mm = 0; mm < DIRECT_SITES; ++mm) {
@@ -523,6 +604,42 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                     uint32_t alo[DIRECT_SITES], alo2[DIRECT_SITES], ahi[DIRECT_SITES];
 #pragma unroll
                     for (int mm = 0; mm < DIRECT_SITES; ++mm) { alo[mm] = 0u; alo2[mm] = 0u; ahi[mm] = 0u; }
+                    if (FAR) {
+                        // far half, Jmin (32 + n_a - n_b) from the colour counts of its block
+                        int B = kb + 32 + jr;
+                        B -= B >= NB ? NB : 0;
+                        const uint2 cn = s_cnt8[B];
+                        const uint4 sb = *reinterpret_cast<const uint4*>(m.selb + (kb << 5) + 16 * (g >> 1));
+                        const uint32_t sbw[4] = {sb.x >> (8 * par), sb.y >> (8 * par), sb.z >> (8 * par), sb.w >> (8 * par)};
+#pragma unroll
+                        for (int mm = 0; mm < DIRECT_SITES; ++mm) {
+                            // byte of site gbase + 2 mm: a | b << 4 -> PRMT bytes 0, 1 = counts of a, b
+                            const uint32_t selc = (mm & 1) ? (sbw[mm >> 1] >> 16) : sbw[mm >> 1];
+                            alo[mm] = dp2a_lo_s32_u32(jpm, prmt(cn.x, cn.y, selc), jmin32);
+                        }
+                        // near half: as below, 8 steps of four sites
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) {
+                            const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
+#pragma unroll
+                            for (int mm = 0; mm < DIRECT_SITES; ++mm) {
+                                const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
+                                const int tt = 7 - mm + 2 * u;
+                                alo[mm] = __dp2a_lo(PL[tt], S, alo[mm]);
+                                alo2[mm] = __dp2a_hi(PL[tt + 1], S, alo2[mm]);
+                            }
+                        }
+                        // far half, residual sums: one IDP.4A per four pair terms
+#pragma unroll
+                        for (int u = 0; u < 8; ++u) {
+                            const uint32_t sel = (u & 1) ? (words[4 + (u >> 1)] >> 16) : words[4 + (u >> 1)];
+#pragma unroll
+                            for (int mm = 0; mm < DIRECT_SITES; ++mm) {
+                                uint32_t& acc = (u & 1) ? alo2[mm] : alo[mm];
+                                acc = dp4a_u32_u32(PL[23 + 7 - mm + 2 * u], prmt(lt[mm].x, lt[mm].y, sel), acc);
+                            }
+                        }
+                    } else {
 #pragma unroll
                     for (int u = 0; u < 16; ++u) {
                         const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
@@ -538,6 +655,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                                 ahi[mm] = __dp2a_hi(PH[FULL_HI ? tt + 1 : 0], S, ahi[mm]);
                             }
                         }
+                    }
                     }
                     if (NEARQ) {
 #pragma unroll
@@ -558,6 +676,8 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                     lutp += 32;
                     wj += 4;
                     wj -= wj >= W ? W : 0;
+                    wjf += 4;
+                    wjf -= wjf >= W ? W : 0;
 #pragma unroll
                     for (int iq = 0; iq < NQ; ++iq) {
                         wn[iq] += 4;
@@ -582,11 +702,17 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&s_full[kb & 1]);
+                if (FAR && kb >= 2 && warp == (kb & 7)) {   // behind the arrival: nobody waits for this
+                    rcv += __shfl_xor_sync(0xffffffffu, rcv, 8);
+                    rcv += __shfl_xor_sync(0xffffffffu, rcv, 16);
+                    if (lane < 8) reinterpret_cast<uint8_t*>(s_cnt8 + kb - 2)[lane] = (uint8_t)rcv;
+                }
                 PT_ACC(1, t_b);
             }
             PT_ACC(2, t_loop);
             PT_T0(t_end);
             cta_sync();  // the chain warp has decided the last block and published its sums
+            if (FAR && warp < 2) recount_block(m.sp, s_cnt8, NB - 2 + warp, lane);
             PT_ACC(6, t_end);
             PT_T0(t_nm);
             // a8 (the chain warps' owner thread samples the observables; every thread helps counting colours)
@@ -903,7 +1029,7 @@ typedef void (*direct_kernel_t)(Dev, long long, int, int, int, int);
 // minb = 1: up to 168 registers per thread (fastest block sums); minb = 2: 80 registers, twice the CTAs per SM.
 inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb) {
 #ifdef PT_ONLY_HEADLINE   // development builds: only the configs[3] instantiation (fast to compile)
-    return sweep_direct_kernel<1, true, false, 1>;
+    return d.far ? sweep_direct_kernel<1, true, false, 1, true> : sweep_direct_kernel<1, true, false, 1>;
 #else
     const bool l4096 = d.L == 4096;
     const int nq = direct_nearq(d.L, r_hi);
@@ -914,7 +1040,8 @@ inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb) {
     if (d.q <= 8) {
         if (minb == 1) {
             switch (nq) {
-                case 1: return l4096 ? sweep_direct_kernel<1, true, false, 1> : sweep_direct_kernel<1, false, false, 1>;
+                case 1: return l4096 ? (d.far ? sweep_direct_kernel<1, true, false, 1, true> : sweep_direct_kernel<1, true, false, 1>)
+                                     : sweep_direct_kernel<1, false, false, 1>;
                 case 2: return sweep_direct_kernel<2, false, false, 1>;
                 case 4: return sweep_direct_kernel<4, false, false, 1>;
                 default: return l4096 ? sweep_direct_kernel<0, true, false, 1> : sweep_direct_kernel<0, false, false, 1>;

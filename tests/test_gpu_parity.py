@@ -484,6 +484,19 @@ def test_cfg3_200_sweeps_bit_exact(pt, oracle):
     assert_same_state(g, o, "cfg3 after 200 sweeps")
 
 
+def test_far_form_of_the_bulk_sum_is_bit_exact(pt, oracle, monkeypatch):
+    """PT_FAR=1 (an experiment kept in the tree, slower than the default form: DESIGN.md section 10): beyond 1000
+    sites the couplings are summed as 8-bit residuals over a per-thread minimum (IDP.4A) plus a colour-count term.
+    Integers: the trajectory must not change."""
+    monkeypatch.setenv("PT_FAR", "1")
+    w = inputs.config(3)
+    g, o = make_pair(pt, oracle, w, "direct")
+    for n in (1, 2, 37):   # ordinary launch, persistent launches; counts carried across launches
+        g.sweeps(n, w.swap_every)
+        o.sweeps(n, w.swap_every, field=True, threads=THREADS)
+        assert_same_state(g, o, "cfg3, far form, %d more sweeps" % n)
+
+
 @pytest.mark.parametrize("L,q,sigma", [(128, 16, 0.6), (256, 9, 0.2), (1024, 12, 0.9), (2048, 9, 0.5)])
 def test_direct_variant_with_more_than_8_colours(pt, oracle, L, q, sigma):
     """Colours 8..15 use the second 8-byte table of a site (two PRMTs OR-ed); both variants against the oracle."""
