@@ -54,6 +54,15 @@ struct Dev {
     int* err;                 // raised by a kernel whose in-kernel barrier timed out (host-mapped: read by pt_sync)
     long long* dbg;           // PT_TIMING builds: [n_ens*n_rep][32 warps][8] clock sums (else unused)
     int bits;                 // bits per spin in spins[]: 4 (q <= 16, 8 sites per word) or 8 (q <= 64, 4 sites per word)
+    // Helper CTAs of a persistent launch of the direct variant (pt_sweep_direct.cuh, HELPERS; n_help = 0: none).
+    // Appended at the end of the struct: the order of the kernel parameters changes the schedule of the sweep kernel.
+    int n_help;               // CTAs beyond the n_rep sweep CTAs: they sum part of the pair terms of other replicas
+    int help_cap;             // block tasks per helper and sweep
+    int help_end;             // blocks HELP_K0 .. help_end - 1 of a sweep can be served
+    unsigned long long* hs;   // [n_rep][L] helper block sums by storage index and site: sum | stamp << 32
+    int* Apub;                // [2][n_rep] accepted changes of the sweep, published with Epub
+    uint32_t* spub;           // [2][n_rep][W] spins as decided, by sweep parity and storage index
+    unsigned* mprog;          // [n_rep] decided blocks in units of 16 (launch-local, monotone), by storage index
 };
 
 // ---------------------------------------------------------------------------
