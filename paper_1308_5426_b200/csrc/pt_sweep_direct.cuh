@@ -77,6 +77,17 @@ constexpr int DIRECT_SITES = 8;     // sites of a block per bulk thread (4 threa
 constexpr int DIRECT_MAX_BULK = 256;
 constexpr int DIRECT_CHAIN_WARPS = 4;                       // one per SM sub-partition
 constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 32 * DIRECT_CHAIN_WARPS;
+// PREP (the configs[3] instantiation: L = 4096, q <= 8, one near quad per thread): a fourth warp group computes the
+// correction rows of every block (they depend on the proposals only, not on anything decided in the sweep) one or
+// two blocks ahead and hands them to the chain warps through shared memory, so that the chain -- whose serial
+// latency sets the pace of the hot replicas -- only loads them.  16 warps need the register file split by role
+// (setmaxnreg): 168 registers per bulk thread, 88 per chain and prep thread.
+constexpr int DIRECT_PREP_WARPS = 4;
+constexpr int DIRECT_PREP_THREADS = DIRECT_MAX_BULK + 32 * (DIRECT_CHAIN_WARPS + DIRECT_PREP_WARPS);   // 512
+constexpr int DIRECT_PREP_ROWS_BYTES = 2 * 4 * 4 * 32 * 16;   // rows[2 buffers][4 warps][4][32 lanes] int4
+__host__ __device__ constexpr bool direct_prep(int nearq, bool njr64, bool q16, int minb) {
+    return njr64 && nearq == 1 && !q16 && minb == 1;
+}
 // L > 4096 (the paper's benchmark range reaches L = 10240): more j-ranges, hence more bulk threads, with
 // the 80-register build of the same code (768 threads x 80 registers fill the register file of an SM).
 constexpr int DIRECT_BIG_BULK = 640;
@@ -341,6 +352,33 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
 }
 
+// CORR: the correction rows of chain warp cw for block i0/32, lane = site l.  If site f of the previous block (rows
+// f = 8cw+j: cp) or of the own block (co) accepts a_f -> b_f, dE_l changes by Jq[dist] (s'_l(b_f) - s'_l(a_f)),
+// dist = l + 32 - f resp. l - f (nothing for dist <= 0): Jp[j], Jo[j] hold Jq[dist].  From the colours at the start
+// of the sweep and the proposals (selb) and the site's own table: nothing here depends on what the sweep decides.
+template <bool Q16>
+__device__ __forceinline__ void direct_corr_rows(const DirectSmem& m, int L, int i0, int cw, int lane, const int (&Jp)[8],
+                                                 const int (&Jo)[8], int4& cp0, int4& cp1, int4& co0, int4& co1) {
+    const uint2 tab = m.lut[i0 + lane];
+    const uint2 tabb = Q16 ? m.lutb[i0 + lane] : make_uint2(0u, 0u);
+    int ipv = i0 - 32 + 8 * cw;
+    ipv += ipv < 0 ? L : 0;
+    const uint2 sfp = *reinterpret_cast<const uint2*>(m.selb + ipv);            // a | b << 4 of 8 sites
+    const uint2 sfo = *reinterpret_cast<const uint2*>(m.selb + i0 + 8 * cw);
+    int cp[8], co[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        const uint32_t wp = j < 4 ? sfp.x : sfp.y, wo = j < 4 ? sfo.x : sfo.y;
+        // selector byte j: nibble 0 = a_f, nibble 1 = b_f (the two higher nibbles pick bytes that the
+        // dot product weights with 0); byte 0 of the result = s'_l(a_f), byte 1 = s'_l(b_f)
+        const uint32_t sp_ = wp >> (8 * (j & 3)), so_ = wo >> (8 * (j & 3));
+        cp[j] = Jp[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, sp_, sp_ ^ 0x8888u), 0);
+        co[j] = Jo[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, so_, so_ ^ 0x8888u), 0);
+    }
+    cp0 = make_int4(cp[0], cp[1], cp[2], cp[3]); cp1 = make_int4(cp[4], cp[5], cp[6], cp[7]);
+    co0 = make_int4(co[0], co[1], co[2], co[3]); co1 = make_int4(co[4], co[5], co[6], co[7]);
+}
+
 // NEARQ = 0: the bulk warps sum both 16-bit halves of every coupling.  NEARQ = 1, 2, 4: they sum the low halves
 // only, plus the high halves of NEARQ of the 56 quads of sites within distance 95 of the block (requires
 // r_hi <= 95 and NEARQ * L/64 >= 56).  NJR64: L == 4096 (64 j-ranges as a compile-time constant).
@@ -348,7 +386,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 // so that several hundred small replicas can be co-resident for persistent launches); 3 stands for the L > 4096
 // build: one CTA of up to DIRECT_BIG_THREADS threads per SM, 80 registers.
 template <int NEARQ, bool NJR64, bool Q16, int MINB>
-__global__ void __launch_bounds__(MINB == 3 ? DIRECT_BIG_THREADS : DIRECT_MAX_THREADS, MINB == 3 ? 1 : MINB)
+__global__ void __launch_bounds__(MINB == 3 ? DIRECT_BIG_THREADS
+                                            : (direct_prep(NEARQ, NJR64, Q16, MINB) ? DIRECT_PREP_THREADS : DIRECT_MAX_THREADS),
+                                  MINB == 3 ? 1 : MINB)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi) {
     // swap_mode 0: no swap event; 1: one event at the end of the launch (last-arriving CTA, nobody waits);
     // 2: persistent launch, an event inside the kernel after every sweep whose index is a multiple of swap_every;
@@ -358,7 +398,8 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     constexpr int NQ = NEARQ ? NEARQ : 1;
     extern __shared__ uint32_t smem_d[];
     const int L = d.L, W = d.W, q = d.q;
-    const int NT = blockDim.x, NTB = NT - 32 * DIRECT_CHAIN_WARPS;
+    constexpr bool PREP = direct_prep(NEARQ, NJR64, Q16, MINB);
+    const int NT = blockDim.x, NTB = NT - 32 * (DIRECT_CHAIN_WARPS + (PREP ? DIRECT_PREP_WARPS : 0));
     const int NB = L >> 5;
     DirectSmem m;
     m.theta = (int32_t*)smem_d;
@@ -370,6 +411,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     m.selb = (uint8_t*)(m.bq + W);
     m.part = (uint32_t*)(m.selb + L);
     m.Jz = (int32_t*)(m.part + 64);
+    int4* s_rows = (int4*)(m.Jz + 96);   // PREP: [2][4 warps][4][32 lanes]: cp[0..3], cp[4..7], co[0..3], co[4..7] of a lane
     __shared__ int s_cnt[16];
     __shared__ long long s_E;   // running energy of this configuration (owner: lane 0 of chain warp 0)
     __shared__ int s_slot;
@@ -383,6 +425,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     // full[s]: the block sums of buffer s are complete (one arrival per bulk warp);
     // done[s]: the chain warps have decided the block of buffer s and written its spins (one arrival).
     __shared__ __align__(8) uint64_t s_full[2], s_done[2];
+    __shared__ __align__(8) uint64_t s_rowsfull[2];   // PREP: the correction rows of buffer s are written (one arrival per prep warp)
     __shared__ __align__(16) int s_xch[2][32][4];   // partial sums exchanged between the chain warps
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -421,6 +464,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
 
     if (tid < NTB) {
         // =========================== BULK warps ===========================
+        if (PREP) asm volatile("setmaxnreg.inc.sync.aligned.u32 168;");
         // thread -> (site group g, j-range jr); group g = the 8 sites 16(g>>1) + (g&1) + {0,2,..,14}
         const int g = tid & 3, jr = tid >> 2;
         const int par = g & 1, gbase = 16 * (g >> 1) + par;
@@ -472,6 +516,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         if (tid == 0) {
             mbar_init(&s_full[0], NTB >> 5); mbar_init(&s_full[1], NTB >> 5);
             mbar_init(&s_done[0], 1); mbar_init(&s_done[1], 1);
+            if (PREP) { mbar_init(&s_rowsfull[0], DIRECT_PREP_WARPS); mbar_init(&s_rowsfull[1], DIRECT_PREP_WARPS); }
         }
         cta_sync();
         if (swap_mode == 3) { t = s_slot; scale = d.thr_scale[t]; }
@@ -605,8 +650,9 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             for (int n = 0; n < 8; ++n) d.dbg[((size_t)blockIdx.x * 32 + warp) * 8 + n] += tacc[n];
         }
 #endif
-    } else {
+    } else if (!PREP || warp < (NTB >> 5) + DIRECT_CHAIN_WARPS) {
         // =========================== CHAIN warps ===========================
+        if (PREP) asm volatile("setmaxnreg.dec.sync.aligned.u32 88;");
         // Four warps, one per SM sub-partition (a warp gets about a fifth of its scheduler's issue slots next to
         // four bulk warps, so the work of a block is spread over all four schedulers).  Every warp keeps the
         // slack y_l of all 32 sites (lane = site); warp cw owns the correction rows f = 8cw..8cw+7 and adds
@@ -650,24 +696,14 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 const int th = m.theta[i0 + lane];
                 const int wsp = (i0 >> 3) + (lane & 3);
                 const uint32_t w_old = m.sp[wsp], w_new = m.bq[wsp];
-                const uint2 tab = m.lut[i0 + lane];
-                const uint2 tabb = Q16 ? m.lutb[i0 + lane] : make_uint2(0u, 0u);
-                int ipv = i0 - 32 + 8 * cw;
-                ipv += ipv < 0 ? L : 0;
-                const uint2 sfp = *reinterpret_cast<const uint2*>(m.selb + ipv);            // a | b << 4 of 8 sites
-                const uint2 sfo = *reinterpret_cast<const uint2*>(m.selb + i0 + 8 * cw);
-                int cp[8], co[8];
-#pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const uint32_t wp = j < 4 ? sfp.x : sfp.y, wo = j < 4 ? sfo.x : sfo.y;
-                    // selector byte j: nibble 0 = a_f, nibble 1 = b_f (the two higher nibbles pick bytes that the
-                    // dot product weights with 0); byte 0 of the result = s'_l(a_f), byte 1 = s'_l(b_f)
-                    const uint32_t sp_ = wp >> (8 * (j & 3)), so_ = wo >> (8 * (j & 3));
-                    cp[j] = Jp[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, sp_, sp_ ^ 0x8888u), 0);
-                    co[j] = Jo[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, so_, so_ ^ 0x8888u), 0);
+                int4 cp0, cp1, co0, co1;
+                if (PREP) {   // written by prep warp cw one or two blocks ago
+                    mbar_wait(&s_rowsfull[k & 1], (uint32_t)(phase0 + (k >> 1)) & 1u);
+                    const int4* rw = s_rows + ((k & 1) * DIRECT_PREP_WARPS + cw) * 128 + lane;
+                    cp0 = rw[0]; cp1 = rw[32]; co0 = rw[64]; co1 = rw[96];
+                } else {
+                    direct_corr_rows<Q16>(m, L, i0, cw, lane, Jp, Jo, cp0, cp1, co0, co1);
                 }
-                const int4 cp0 = make_int4(cp[0], cp[1], cp[2], cp[3]), cp1 = make_int4(cp[4], cp[5], cp[6], cp[7]);
-                const int4 co0 = make_int4(co[0], co[1], co[2], co[3]), co1 = make_int4(co[4], co[5], co[6], co[7]);
                 // changes accepted in block k-1, which the bulk sum saw as it was before: this warp's rows, known
                 // before the wait; they ride along with the first round below (one exchange less per block)
                 int pc = 0;
@@ -781,6 +817,43 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             for (int n = 0; n < 8; ++n) d.dbg[((size_t)blockIdx.x * 32 + warp) * 8 + n] += tacc[n];
         }
 #endif
+    } else {
+        // =========================== PREP warps ===========================
+        // Warp pw computes the correction rows of chain warp pw (CORR) for block k as soon as the rows' buffer k & 1
+        // is free (the chain is done with block k-2): they depend on the sweep's proposals only.
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 88;");
+        const int pw = warp - (NTB >> 5) - DIRECT_CHAIN_WARPS;
+        int Jp[8], Jo[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {
+            const int dp = lane + 32 - (8 * pw + j), dn = lane - (8 * pw + j);
+            Jp[j] = __ldg(d.Jq + dp);               // 1 <= dp <= 63 < L
+            Jo[j] = dn > 0 ? __ldg(d.Jq + dn) : 0;
+        }
+        PT_LOAD_STATE();
+        cta_sync();
+        if (swap_mode == 3) { t = s_slot; scale = d.thr_scale[t]; }
+        for (int s = 0; s < n_sweeps; ++s) {
+            direct_draw<Q16>(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
+            cta_sync();
+            const int phase0 = s * (NB >> 1);
+            for (int k = 0; k < NB; ++k) {
+                if (k >= 2) mbar_wait(&s_done[k & 1], (uint32_t)(phase0 + (k >> 1) - 1) & 1u);
+                int4 cp0, cp1, co0, co1;
+                direct_corr_rows<Q16>(m, L, k << 5, pw, lane, Jp, Jo, cp0, cp1, co0, co1);
+                int4* rw = s_rows + ((k & 1) * DIRECT_PREP_WARPS + pw) * 128 + lane;
+                rw[0] = cp0; rw[32] = cp1; rw[64] = co0; rw[96] = co1;
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&s_rowsfull[k & 1]);
+            }
+            cta_sync();   // (the same CTA-wide barriers as the bulk and chain warps)
+            direct_nmax(m.sp, W, q, s_cnt);
+            cta_sync();
+            if (swap_mode == 2 && (sweep0 + s + 1) % swap_every == 0) {
+                t = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, &s_E, event++);
+                scale = s_scale[t];
+            }
+        }
     }
 
     cta_sync();
@@ -934,12 +1007,19 @@ inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb) {
 #endif
 }
 
+// The PREP instantiation runs 512 threads (a fourth warp group) and keeps the correction rows in dynamic shared memory.
+inline bool direct_kernel_is_prep(direct_kernel_t kern) { return kern == (direct_kernel_t)sweep_direct_kernel<1, true, false, 1>; }
+inline int direct_kernel_threads(direct_kernel_t kern, int L) { return direct_kernel_is_prep(kern) ? DIRECT_PREP_THREADS : direct_threads(L); }
+inline size_t direct_kernel_smem(direct_kernel_t kern, int L, int q) {
+    return direct_smem_bytes(L, q) + (direct_kernel_is_prep(kern) ? DIRECT_PREP_ROWS_BYTES : 0);
+}
+
 // CTAs of a sweep kernel variant that can be resident on the device at once (0 on error).
 inline int direct_coresident(direct_kernel_t kern, const Dev& d, int device) {
-    const size_t smem = direct_smem_bytes(d.L, d.q);
+    const size_t smem = direct_kernel_smem(kern, d.L, d.q);
     if (allow_max_dynamic_smem((const void*)kern, DIRECT_STATIC_SMEM) != 0) return 0;
     int per_sm = 0, n_sm = 0, coop = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, direct_threads(d.L), smem) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, direct_kernel_threads(kern, d.L), smem) != cudaSuccess) return 0;
     if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return 0;
     if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device) != cudaSuccess || !coop) return 0;
     return per_sm * n_sm;
@@ -976,11 +1056,11 @@ inline direct_kernel_t select_direct_kernel(const Dev& d, int r_hi, int device, 
 // sweeps of configs[2].)
 inline int launch_sweep_direct(direct_kernel_t kern, const Dev& d, long long sweep0, int n_sweeps, int swap_mode,
                                int swap_every, int r_hi, cudaStream_t stream) {
-    const size_t smem = direct_smem_bytes(d.L, d.q);
+    const size_t smem = direct_kernel_smem(kern, d.L, d.q);
     cudaError_t err = cudaSuccess;   // (the shared-memory attribute was set once, in direct_coresident)
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(swap_mode == 3 ? d.n_local : d.n_ens * d.n_rep));
-    cfg.blockDim = dim3((unsigned)direct_threads(d.L));
+    cfg.blockDim = dim3((unsigned)direct_kernel_threads(kern, d.L));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
