@@ -298,6 +298,7 @@ def run_ours(args):
         dram_per_launch = DRAM_BYTES_PER_LAUNCH_FIXED + DRAM_BYTES_PER_SWEEP * K / max(1, launches)
         lanes = peaks["idp2a"][1] or IDP_LANES_PER_CLK_PER_SM          # IDP.2A alone, 2 warps per sub-partition
         lanes_mix = peaks["prmt+2idp2a (idp2a counted)"][1]            # ... next to one PRMT per two IDP.2A
+        lanes_tile = peaks["bulk tile, near form (idp2a counted)"][1]  # ... in the kernel's own tile
         peak = N_SM * lanes * MACS_PER_IDP_LANE * f_hz / 1e12
         persistent = launches == 1 and K > 1 and variant == "direct"
         roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tmac/s", "frac": achieved / peak,
@@ -305,6 +306,10 @@ def run_ours(args):
                     "kernel": "sweep_%s_kernel" % variant,
                     "idp2a_lanes_per_clk_per_sm": lanes, "idp2a_lanes_in_bulk_mix": lanes_mix,
                     "frac_of_mix_ceiling": achieved / peak * lanes / lanes_mix if lanes_mix else None,
+                    # the rate at which an SM runs the kernel's own bulk tile (8 sites x 16 steps on table and coupling
+                    # registers, nothing else on the SM): what the instruction mix allows on 148 SMs
+                    "idp2a_lanes_in_bulk_tile": lanes_tile,
+                    "frac_of_tile_ceiling": achieved / peak * lanes / lanes_tile if lanes_tile else None,
                     "launch": "persistent (cooperative, swap events inside the kernel)" if persistent
                               else "one launch per swap interval",
                     "note": "algorithmic work = sweeps*n_rep*L^2 = %.3e integer multiply-accumulates per launch (one per "

@@ -239,10 +239,13 @@ int pt_sync(pt_ctx* ctx);
  * and SM of pattern p with w = 1..4 warps per SM sub-partition, timed with clock64() inside the kernel (median over
  * the SMs).  Patterns: 0 IDP.2A, 1 IDP.4A, 2 IMAD, 3 PRMT, 4 LOP3, 5 the bulk loop's mix of 1 PRMT + 2 IDP.2A
  * (counting the IDP.2A only), 6 1 LOP3 + 2 IDP.2A (ditto), 7 LDS.128 in bytes per clock and SM, 8 1 PRMT + 4 IDP.2A,
- * 9 the mirror-paired mix 2 PRMT + 1 ADD + 2 IDP.2A (IDP.2A counted; 4 pair terms per IDP.2A lane-operation).
+ * 9 the mirror-paired mix 2 PRMT + 1 ADD + 2 IDP.2A (IDP.2A counted; 4 pair terms per IDP.2A lane-operation),
+ * 10 the bulk tile of the direct sweep kernel as it stands (8 sites x 16 steps: one PRMT on the site's two table
+ * registers and two IDP.2A on 39 packed coupling registers per step and site; IDP.2A counted), 11 the same tile in the
+ * far form of PT_FAR (one PRMT and one IDP.4A per step and site; the IDP.4A counted, each standing for two IDP.2A).
  * One IDP.2A lane-operation is two multiply-accumulates (one per pair term of the energy sum).
  * n = number of doubles `rates` holds, >= 4 * PT_PEAK_PATTERNS.  Errors: PT_EINVAL, PT_ENOMEM, PT_ECUDA. */
-#define PT_PEAK_PATTERNS 10
+#define PT_PEAK_PATTERNS 12
 int pt_measure_peaks(double* rates, int n);
 
 /* Total energies of caller-supplied configurations WITHOUT ANY ALLOCATION (for callers that cannot call cudaMalloc:

@@ -21,11 +21,17 @@ enum PeakPattern {
     PEAK_LDS128 = 7,       // LDS.128 (conflict-free); rate in bytes per clock
     PEAK_MIX_BULK4 = 8,    // 1 PRMT + 4 IDP.2A (both coupling halves); rate counts IDP.2A only
     PEAK_MIX_MIRROR = 9,   // 2 PRMT + 1 ADD + 2 IDP.2A (mirror-paired pair terms, 8 per group); rate counts IDP.2A only
-    PEAK_N = 10
+    PEAK_TILE_NEAR = 10,   // the bulk tile of sweep_direct_kernel as it stands: 8 sites x 16 steps, per step and site one
+                           // PRMT on the site's two table registers and two IDP.2A on packed coupling registers (39 of
+                           // them, as in the kernel); rate counts IDP.2A only
+    PEAK_TILE_FAR = 11,    // the same tile in the far form (PT_FAR): one PRMT and ONE IDP.4A per step and site; rate counts
+                           // the IDP.4A (each covers the four pair terms that take two IDP.2A in the near form)
+    PEAK_N = 12
 };
 
 constexpr int PEAK_UNROLL = 16;   // independent dependency chains per thread
 constexpr int PEAK_ITERS = 512;
+constexpr int PEAK_TILE_ITERS = 64;   // tiles (8 sites x 16 steps = 128 look-ups) per thread in the tile patterns
 
 // out[blockIdx.x] = clocks the CTA needed; sink keeps the results alive.
 template <int PATTERN>
@@ -41,8 +47,39 @@ __global__ void __launch_bounds__(512, 1) peak_kernel(long long* __restrict__ cl
         a[i] = (seed ^ (0x9E3779B9u * (i + 1))) + tid;
         b[i] = (seed + 0x01010101u * i) & 0x07070707u;
     }
+    // the tile patterns: registers as the bulk warps of sweep_direct_kernel hold them
+    uint32_t PLt[40], ltt[16], wt[8];
+    if (PATTERN == PEAK_TILE_NEAR || PATTERN == PEAK_TILE_FAR) {
+#pragma unroll
+        for (int i = 0; i < 40; ++i) PLt[i] = seed * (i + 3) + tid;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) ltt[i] = (seed + i * 0x01010101u) & 0x03030303u;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) wt[i] = (seed * (i + 7) + tid) & 0x77777777u;
+    }
     __syncthreads();
     const long long t0 = clock64();
+    if (PATTERN == PEAK_TILE_NEAR || PATTERN == PEAK_TILE_FAR) {
+        for (int it = 0; it < PEAK_TILE_ITERS; ++it) {
+#pragma unroll
+            for (int u = 0; u < 16; ++u) {
+                const uint32_t sel = (u & 1) ? (wt[u >> 1] >> 16) : wt[u >> 1];
+#pragma unroll
+                for (int mm = 0; mm < 8; ++mm) {
+                    uint32_t S;
+                    asm volatile("prmt.b32 %0, %1, %2, %3;" : "=r"(S) : "r"(ltt[2 * mm]), "r"(ltt[2 * mm + 1]), "r"(sel));
+                    const int tt = 7 - mm + 2 * u;
+                    if (PATTERN == PEAK_TILE_NEAR) {
+                        asm volatile("dp2a.lo.u32.u32 %0, %1, %2, %0;" : "+r"(acc[mm]) : "r"(PLt[tt]), "r"(S));
+                        asm volatile("dp2a.hi.u32.u32 %0, %1, %2, %0;" : "+r"(acc[8 + mm]) : "r"(PLt[tt + 1]), "r"(S));
+                    } else {
+                        asm volatile("dp4a.u32.u32 %0, %1, %2, %0;" : "+r"(acc[8 * (u & 1) + mm]) : "r"(PLt[tt]), "r"(S));
+                    }
+                }
+            }
+            wt[it & 7] ^= acc[it & 7] & 0x77777777u;
+        }
+    } else
     for (int it = 0; it < PEAK_ITERS; ++it) {
 #pragma unroll
         for (int i = 0; i < PEAK_UNROLL; ++i) {
@@ -103,6 +140,8 @@ inline double peak_counted_ops(int pattern) {
     if (pattern == PEAK_MIX_BULK || pattern == PEAK_MIX_LOP || pattern == PEAK_MIX_MIRROR) return 2.0 * base;
     if (pattern == PEAK_MIX_BULK4) return 4.0 * base;
     if (pattern == PEAK_LDS128) return 16.0 * base;   // bytes per thread
+    if (pattern == PEAK_TILE_NEAR) return 2.0 * 128.0 * PEAK_TILE_ITERS;
+    if (pattern == PEAK_TILE_FAR) return 128.0 * PEAK_TILE_ITERS;
     return base;
 }
 
@@ -119,6 +158,8 @@ inline peak_kernel_t peak_kernel_of(int pattern) {
         case PEAK_LDS128: return peak_kernel<PEAK_LDS128>;
         case PEAK_MIX_BULK4: return peak_kernel<PEAK_MIX_BULK4>;
         case PEAK_MIX_MIRROR: return peak_kernel<PEAK_MIX_MIRROR>;
+        case PEAK_TILE_NEAR: return peak_kernel<PEAK_TILE_NEAR>;
+        case PEAK_TILE_FAR: return peak_kernel<PEAK_TILE_FAR>;
         default: return nullptr;
     }
 }

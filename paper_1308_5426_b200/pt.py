@@ -87,7 +87,8 @@ _lib.pt_energy_static.argtypes = [_i32, _i32, _dbl, _vp, _i32, _vp, _vp, _vp]
 STATIC_MAX_L, STATIC_MAX_SITES = 16384, 1048576     # PT_STATIC_MAX_L, PT_STATIC_MAX_SITES of include/pt.h
 
 PEAK_PATTERNS = ["idp2a", "idp4a", "imad", "prmt", "lop3", "prmt+2idp2a (idp2a counted)", "lop3+2idp2a (idp2a counted)",
-                 "lds128 (bytes)", "prmt+4idp2a (idp2a counted)", "2prmt+add+2idp2a (idp2a counted)"]
+                 "lds128 (bytes)", "prmt+4idp2a (idp2a counted)", "2prmt+add+2idp2a (idp2a counted)",
+                 "bulk tile, near form (idp2a counted)", "bulk tile, far form (idp4a counted)"]
 
 
 def measure_peaks():
