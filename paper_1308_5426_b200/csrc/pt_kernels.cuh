@@ -32,6 +32,19 @@ inline int allow_max_dynamic_smem(const void* kernel, int static_bytes) {
 // Everything a kernel needs to know about a context (passed by value).  New fields go at the END: ptxas' schedule of
 // sweep_direct_kernel changes with the layout of its parameters (a field inserted after ens_base cost the headline
 // workload 3 %, measured A/B on one GPU; appended, the SASS is the same up to constant-bank offsets).
+// Parameters and buffers of the helper CTAs of a persistent launch (pt_sweep_direct.cuh, HELPERS), in device memory.
+struct HelpDev {
+    int n_help;               // CTAs beyond the n_rep sweep CTAs: they sum part of the pair terms of other replicas
+    int help_cap;             // block tasks per helper and sweep
+    int help_end;             // blocks help_k0 .. help_end - 1 of a sweep can be served
+    int help_k0;              // first block of a sweep that can be served
+    int help_whot;            // weight of a hot slot in the split of a helper's capacity (a cold slot: 1)
+    unsigned long long* hs;   // [n_rep][L] helper block sums by storage index and site: sum | stamp << 32
+    int* Apub;                // [2][n_rep] accepted changes of the sweep, published with Epub
+    uint32_t* spub;           // [2][n_rep][W] spins as decided, by sweep parity and storage index
+    unsigned* mprog;          // [n_rep] decided blocks in units of 16 (launch-local, monotone), by storage index
+};
+
 struct Dev {
     int L, W, q, n_ens, n_rep, ens_base;
     int rep_base, n_local;    // slot-sharded contexts (pt_create_shard): this process sweeps the configurations with
@@ -57,6 +70,8 @@ struct Dev {
     int far;                  // direct variant, L = 4096: the couplings of every far j-range (jr = 16..47) lie within 255 of
                               // their minimum, which is < 2^15 (pt_sweep_direct.cuh, FAR); at the end of the struct: the
                               // order of the kernel parameters changes the schedule of the sweep kernel
+    const struct HelpDev* hlp; // helper CTAs of a persistent launch (pt_sweep_direct.cuh, HELPERS), else nullptr.  One pointer at
+                              // the end of the struct: more kernel parameters change the schedule of the sweep kernel
 };
 
 // ---------------------------------------------------------------------------

@@ -95,6 +95,13 @@ struct pt_ctx {
     int coresident = -1;   // direct variant: CTAs that fit on the device at once (-1: not asked yet)
     ptk::direct_kernel_t direct_kern = nullptr;   // the sweep kernel instantiation this context uses
     int persistent_policy = 1;   // 0 never, 1 when the context fills the device and the call is long enough, 2 whenever possible
+    // helper CTAs of persistent launches (pt_sweep_direct.cuh, HELPERS): decided and allocated at the first such launch
+    int n_help = -1, help_cap = 0;
+    ptk::HelpDev* d_hlp = nullptr;   // parameters and buffer pointers, in device memory
+    unsigned long long* d_hs = nullptr;
+    int* d_Apub = nullptr;
+    uint32_t* d_spub = nullptr;
+    unsigned* d_mprog = nullptr;
 
     int R() const { return n_ens * n_rep; }
     int bits() const { return q <= 16 ? 4 : 8; }     // bits per spin in d_spins
@@ -107,6 +114,7 @@ struct pt_ctx {
         d.spins = d_spins; d.E = d_E; d.perm = d_perm; d.obs = d_obs; d.h = d_h; d.done = d_done; d.dbg = d_dbg; d.gen = d_gen; d.Epub = d_Epub; d.err = d_err;
         d.rep_base = rep_base; d.n_local = n_local ? n_local : n_rep; d.count_swaps = rep_base == 0 ? 1 : 0;
         d.far = far_ok;
+        d.hlp = nullptr;   // set by the persistent launch that uses helpers
         return d;
     }
 };
@@ -124,6 +132,7 @@ void free_ctx(pt_ctx* c) {
     if (c->h_err) cudaFreeHost(c->h_err);
     cudaFree(c->d_stage);
     cudaFree(c->d_Ef);
+    cudaFree(c->d_hs); cudaFree(c->d_Apub); cudaFree(c->d_spub); cudaFree(c->d_mprog); cudaFree(c->d_hlp);
     if (c->h_stage) cudaFreeHost(c->h_stage);
     delete c;
 }
@@ -172,6 +181,46 @@ int resolve_variant(int L, int q, long long rowsum, int variant, int* out) {
     return PT_OK;
 }
 
+// Helper CTAs for persistent launches with a swap event after every sweep (pt_sweep_direct.cuh, HELPERS): as many as
+// the device has room for beyond the n_rep sweep CTAs, if the context runs the configs[3] instantiation of the sweep
+// kernel (L = 4096, q <= 8, one near quad per thread) with one ensemble.  PT_HELPERS=<n> caps their number (0: none),
+// PT_HELP_CAP=<tasks per helper and sweep>, PT_HELP_END=<blocks 2 .. end-1 are served> (experiments).
+int helpers(pt_ctx* c) {
+    if (c->n_help >= 0) return c->n_help;
+    c->n_help = 0;
+    if (c->n_ens != 1 || c->n_local ||
+        c->direct_kern != (ptk::direct_kernel_t)ptk::sweep_direct_kernel<1, true, false, 1, false, true>)
+        return 0;
+    const char* env = getenv("PT_HELPERS");
+    int n = c->coresident - c->R();
+    if (env) n = std::min(n, atoi(env));
+    if (n < 1 || c->n_rep > ptk::HELP_MAX_CLIENTS * n) return 0;
+    auto env_int = [](const char* name, int dflt) { const char* e = getenv(name); return e ? atoi(e) : dflt; };
+    ptk::HelpDev h = {};
+    h.n_help = n;
+    h.help_cap = env_int("PT_HELP_CAP", 240);
+    h.help_end = env_int("PT_HELP_END", c->L / 32);
+    h.help_k0 = env_int("PT_HELP_K0", 16);
+    h.help_whot = env_int("PT_HELP_WHOT", 6);
+    if (h.help_cap < 1 || h.help_k0 < 1 || h.help_end <= h.help_k0 || h.help_end > c->L / 32 || h.help_whot < 1 ||
+        ptk::direct_help_smem_bytes(c->L, h.help_cap) + ptk::DIRECT_STATIC_SMEM > (size_t)kSmemLimit)
+        return 0;
+    const size_t R = (size_t)c->R();
+    if (cudaMalloc(&c->d_hs, R * c->L * sizeof(unsigned long long)) != cudaSuccess ||
+        cudaMalloc(&c->d_Apub, 2 * R * sizeof(int)) != cudaSuccess ||
+        cudaMalloc(&c->d_spub, 2 * R * c->words() * sizeof(uint32_t)) != cudaSuccess ||
+        cudaMalloc(&c->d_mprog, R * sizeof(unsigned)) != cudaSuccess ||
+        cudaMalloc(&c->d_hlp, sizeof(ptk::HelpDev)) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    h.hs = c->d_hs; h.Apub = c->d_Apub; h.spub = c->d_spub; h.mprog = c->d_mprog;
+    if (cudaMemcpy(c->d_hlp, &h, sizeof(h), cudaMemcpyHostToDevice) != cudaSuccess) { cudaGetLastError(); return 0; }
+    c->help_cap = h.help_cap;
+    c->n_help = n;
+    return n;
+}
+
 // Enqueue one launch covering n_sweeps sweeps.  swap_mode 0: no swap event, 1: one at the end of the launch,
 // 2 (direct variant only): persistent launch with an event after every sweep whose index divides by swap_every.
 int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
@@ -210,8 +259,14 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
     } else {
         c->fields_valid = false;
         if (!c->direct_kern) c->direct_kern = ptk::select_direct_kernel(d, c->r_hi, c->device, &c->coresident);
-        int rc = ptk::launch_sweep_direct(c->direct_kern, d, (long long)c->sweep, n_sweeps, swap_mode, swap_every,
-                                          c->r_hi, c->stream);
+        ptk::Dev dl = d;
+        if (swap_mode == 2 && swap_every == 1 && helpers(c) > 0) {
+            dl.hlp = c->d_hlp;
+            PT_CUDA(cudaMemsetAsync(c->d_hs, 0, (size_t)c->R() * c->L * sizeof(unsigned long long), c->stream));
+            PT_CUDA(cudaMemsetAsync(c->d_mprog, 0, (size_t)c->R() * sizeof(unsigned), c->stream));
+        }
+        int rc = ptk::launch_sweep_direct(c->direct_kern, dl, (long long)c->sweep, n_sweeps, swap_mode, swap_every,
+                                          c->r_hi, c->stream, dl.hlp ? c->n_help : 0, c->help_cap);
         if (rc) return fail(PT_ECUDA, std::string("sweep_direct launch: ") + cudaGetErrorString((cudaError_t)rc));
     }
     PT_CUDA(cudaGetLastError());
@@ -317,8 +372,8 @@ int pt_create_ex(pt_ctx** out, int L, int q, double sigma, int n_ens, int n_rep,
         c->persistent_policy = (env && env[0] == '0') ? 0 : (env && env[0] == '2') ? 2 : 1;
     }
 #ifdef PT_TIMING
-    PT_CUDA_C(cudaMalloc(&c->d_dbg, (size_t)R * 32 * 8 * sizeof(long long)));
-    PT_CUDA_C(cudaMemset(c->d_dbg, 0, (size_t)R * 32 * 8 * sizeof(long long)));
+    PT_CUDA_C(cudaMalloc(&c->d_dbg, (size_t)(R + 64) * 32 * 8 * sizeof(long long)));
+    PT_CUDA_C(cudaMemset(c->d_dbg, 0, (size_t)(R + 64) * 32 * 8 * sizeof(long long)));
 #endif
 
     std::vector<double> scale(n_rep);
@@ -643,8 +698,8 @@ int pt_get_perm(pt_ctx* c, int32_t* perm) {
 // Development builds only (-DPT_TIMING): per-warp clock sums of the sweep kernel, [R][32][8].
 int pt_debug_timing(pt_ctx* c, long long* out) {
     if (!c || !out || !c->d_dbg) return fail(PT_EINVAL, "no timing buffer");
-    PT_CUDA(cudaMemcpy(out, c->d_dbg, (size_t)c->R() * 32 * 8 * sizeof(long long), cudaMemcpyDeviceToHost));
-    PT_CUDA(cudaMemset(c->d_dbg, 0, (size_t)c->R() * 32 * 8 * sizeof(long long)));
+    PT_CUDA(cudaMemcpy(out, c->d_dbg, (size_t)(c->R() + 64) * 32 * 8 * sizeof(long long), cudaMemcpyDeviceToHost));
+    PT_CUDA(cudaMemset(c->d_dbg, 0, (size_t)(c->R() + 64) * 32 * 8 * sizeof(long long)));
     return PT_OK;
 }
 #endif

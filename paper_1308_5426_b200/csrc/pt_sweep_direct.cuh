@@ -69,6 +69,7 @@
 // slot -> storage permutation (direct_swap_in_kernel); the configuration keeps
 // its CTA and shared memory, the temperature, RNG slot and accumulators move.
 #pragma once
+#include <type_traits>
 #include "pt_kernels.cuh"
 
 namespace ptk {
@@ -87,6 +88,39 @@ constexpr int ENERGY_MAX_THREADS = 512, ENERGY_NPAIR = 35;   // energy_direct_ke
 constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: the 224 sites (56 quads) around a block
 constexpr int DIRECT_NEAR_QUADS = 56;
 constexpr int DIRECT_MAX_PERSIST_REP = 512;   // replicas per ensemble in a persistent launch (static shared arrays)
+
+// HELPERS (persistent launches of the configs[3] instantiation only).  A device has more SMs than an ensemble has
+// replicas (148 against 128): the spare SMs run helper CTAs.  For a block of 32 sites the j-ranges 0..31 (bulk warps
+// 0..3, one per SM sub-partition: the sites of the block itself and the 63 blocks after it, cyclically) do not
+// depend on anything decided in the last 64 blocks, so another SM can sum them ahead of time from a copy of the
+// spins.  Helper h serves the slots h, h + n_help, ...; each client gets a window of K consecutive blocks (K from the
+// helper's capacity, double weight for slots that accepted more than 30 % in the last sweep; windows staggered over
+// the sweep).  In its window a sweep CTA leaves the main loop of bulk warps 0..3 out and its chain warps add the
+// helper's sums, which arrive through global memory as 64-bit words (sum | sweep stamp << 32: the data is its own
+// flag).  Integer sums: the result does not depend on who summed what.
+constexpr int HELP_K0 = 2;            // first block that can be served (the helper draws its clients' proposals first)
+constexpr int HELP_MAX_CLIENTS = 8;   // slots per helper
+constexpr int HELP_GROUPS = 3;        // 4-warp groups of a helper CTA, one task (client, block) at a time each
+struct HelpPlan { int K, o; };        // window: blocks o .. o + K - 1
+__device__ inline HelpPlan help_plan(const uint8_t* hot, int t, int n_help, int n_rep, int cap, int end, int whot, int k0) {
+    const int h = t % n_help, j = t / n_help;
+    int wsum = 0, ncl = 0;
+    for (int t2 = h; t2 < n_rep; t2 += n_help) { wsum += hot[t2] ? whot : 1; ++ncl; }
+    const int span = end - k0;
+    int K = cap * (hot[t] ? whot : 1) / wsum;
+    K = K < span ? K : span;
+    HelpPlan pl;
+    pl.K = K;
+    pl.o = k0 + (ncl > 1 ? j * (span - K) / (ncl - 1) : 0);
+    return pl;
+}
+// dynamic shared memory of a helper CTA (32-bit words): spc[HELP_MAX_CLIENTS][W] | lut[(cap + 8) * 32] uint2 |
+// gpart[3][2][32] | task lists [3][cap / 3 + 8] (16 bits each)
+__host__ __device__ inline int help_group_tasks(int cap) { return cap / HELP_GROUPS + 8; }
+__host__ __device__ inline size_t direct_help_smem_bytes(int L, int cap) {
+    return (size_t)(HELP_MAX_CLIENTS * (L / 8) + 2 * (cap + 8) * 32 + HELP_GROUPS * 2 * 32 +
+                    (HELP_GROUPS * help_group_tasks(cap) + 1) / 2) * 4;
+}
 
 __host__ __device__ inline size_t direct_smem_bytes(int L, int q);
 __host__ __device__ inline bool direct_applies(int L, int q) {
@@ -261,19 +295,28 @@ struct PersistSmem {
     int* perm;          // [n_rep] slot -> storage
     long long* Eall;    // [n_rep] energies by storage index
     int* slot;          // result
+    uint8_t* hot;       // [n_rep] HELPERS: the slot accepted more than 30 % of its proposals in the last sweep
 };
+// st < 0: observer (a helper CTA): it neither publishes nor arrives, but waits for the event and follows it.
 __device__ __forceinline__ int direct_swap_in_kernel(const Dev& d, const PersistSmem& ps, int e, uint32_t sweep, int st,
-                                                     const long long* s_E, int event) {
+                                                     const long long* s_E, int event, bool help = false, int n_acc = 0) {
     const int n_rep = d.n_rep;
     long long* Epub = d.Epub + ((size_t)(event & 1) * d.n_ens + e) * n_rep;
+    int* Apub = help ? d.hlp->Apub + (size_t)(event & 1) * n_rep : nullptr;   // (HELPERS: one ensemble)
     if (threadIdx.x == 0) {
-        __stcg(Epub + st, *s_E);
-        // release: the energy is visible to whoever observes the arrival (cheaper than a full __threadfence)
-        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(d.gen + e) : "memory");
+        if (st >= 0) {
+            __stcg(Epub + st, *s_E);
+            if (help) __stcg(Apub + st, n_acc);
+            // release: the energy is visible to whoever observes the arrival (cheaper than a full __threadfence)
+            asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(d.gen + e) : "memory");
+        }
         wait_arrivals(d.gen + e, (unsigned)n_rep * (unsigned)(event + 1), d.err);
     }
     cta_sync();
-    for (int t2 = threadIdx.x; t2 < n_rep; t2 += blockDim.x) ps.Eall[t2] = __ldcg(Epub + t2);
+    for (int t2 = threadIdx.x; t2 < n_rep; t2 += blockDim.x) {
+        ps.Eall[t2] = __ldcg(Epub + t2);
+        if (help) ps.hot[t2] = 10 * __ldcg(Apub + ps.perm[t2]) > 3 * d.L;   // by slot, before the event moves anything
+    }
     cta_sync();
     const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_SWAP;
     pt_obs* obs = d.obs + (size_t)e * n_rep;
@@ -291,6 +334,7 @@ __device__ __forceinline__ int direct_swap_in_kernel(const Dev& d, const Persist
         }
         cta_sync();
     }
+    if (st < 0) return -1;
     for (int t2 = threadIdx.x; t2 < n_rep; t2 += blockDim.x)
         if (ps.perm[t2] == st) *ps.slot = t2;
     cta_sync();
@@ -371,13 +415,218 @@ __device__ __forceinline__ void recount_block(const uint32_t* sp, uint2* cnt8, i
     if (lane < 8) reinterpret_cast<uint8_t*>(cnt8 + blk)[lane] = (uint8_t)v;
 }
 
+// A helper CTA (HELPERS above): 3 groups of 4 warps; thread (g, jr) of a group holds the couplings of bulk thread
+// (g, jr), jr = 0..31, of a sweep CTA.  Per sweep: follow the swap event, copy the clients' spins as they are at the
+// start of the sweep, draw the proposals of the sites in the clients' windows (the same Philox stream as the client's
+// own DRAW) and then work through the tasks (block, client) in block order, task n by group n % 3.  A block sum goes
+// to hd.hs as sum | stamp << 32.  The j-ranges 0..31 of block kb are the blocks kb .. kb + 63 (cyclically): for
+// kb <= 64 all of them are still as at the start of the sweep; beyond, the wrapped ones (blocks 0 .. kb - 65) must
+// be final: the sweep CTAs publish their blocks as they decide them (spub, mprog in units of 16 blocks) and the
+// helper refreshes its copies chunk by chunk, 16 blocks before the first task that needs the chunk.
+__device__ __forceinline__ void direct_helper_cta(const Dev& d, uint32_t* smem, const PersistSmem& ps, long long sweep0,
+                                                  int n_sweeps) {
+    const HelpDev hd = *d.hlp;
+    const int L = d.L, W = d.W, q = d.q, NB = L >> 5, R = d.n_rep, H = hd.n_help;
+    const int tid = threadIdx.x, lane = tid & 31, NT = blockDim.x;
+    const int h = (int)blockIdx.x - R;
+    const int gi = tid >> 7, tg = tid & 127, wg = tg >> 5;   // group, thread and warp inside the group
+    const int g = tg & 3, jr = tg >> 2, par = g & 1, gbase = 16 * (g >> 1) + par;
+    uint32_t* spc = smem;                                            // [HELP_MAX_CLIENTS][W]
+    uint2* hlut = (uint2*)(spc + HELP_MAX_CLIENTS * W);              // [(cap + 8) * 32]
+    uint32_t* gpart = (uint32_t*)(hlut + (hd.help_cap + 8) * 32);     // [HELP_GROUPS][2][32]
+    uint16_t* tasks = (uint16_t*)(gpart + HELP_GROUPS * 2 * 32);      // [HELP_GROUPS][TG]: block | client << 8
+    const int TG = help_group_tasks(hd.help_cap);
+    __shared__ int s_cl[HELP_MAX_CLIENTS][5];   // slot, storage index, K, o, first table entry
+    __shared__ int s_ncl, s_ntask, s_kbmax;
+    uint32_t PL[DIRECT_NPAIR];
+    {
+        const int Hh = L / 2;
+        const int R0 = ((gbase + 14 - 64 * jr) % L + L) % L;
+        const uint32_t* lo = d.Jpair + (size_t)(2 * par) * Hh;
+        int r = R0;
+#pragma unroll
+        for (int tt = 0; tt < DIRECT_NPAIR; ++tt) {
+            PL[tt] = __ldg(lo + ((r - par) >> 1));
+            r -= 2;
+            r += r < 0 ? L : 0;
+        }
+    }
+    for (int t2 = tid; t2 < R; t2 += NT) { ps.perm[t2] = d.perm[t2]; ps.hot[t2] = 1; }
+    if (tid < HELP_GROUPS * 2 * 32) gpart[tid] = 0u;
+    cta_sync();
+    const uint32_t c3 = ((uint32_t)d.ens_base << 4) | TAG_SWEEP;
+    int gcnt = 0;   // tasks this group has done (buffer of the group's block sums = gcnt & 1)
+#ifdef PT_TIMING
+    long long hacc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    const long long h_start = clock64();
+#endif
+    for (int s = 0; s < n_sweeps; ++s) {
+        const uint32_t sweep = (uint32_t)(sweep0 + s + 1);
+#ifdef PT_TIMING
+        const long long h_t0 = clock64();
+#endif
+        if (s > 0) direct_swap_in_kernel(d, ps, 0, (uint32_t)(sweep0 + s), -1, nullptr, s - 1, true, 0);
+        if (tid == 0) {
+            int ncl = 0, off = 0;
+            for (int t = h; t < R && ncl < HELP_MAX_CLIENTS; t += H) {
+                const HelpPlan pl = help_plan(ps.hot, t, H, R, hd.help_cap, hd.help_end, hd.help_whot, hd.help_k0);
+                s_cl[ncl][0] = t; s_cl[ncl][1] = ps.perm[t]; s_cl[ncl][2] = pl.K; s_cl[ncl][3] = pl.o; s_cl[ncl][4] = off;
+                off += pl.K * 32;
+                ++ncl;
+            }
+            s_ncl = ncl;
+            s_ntask = off >> 5;
+            int kbmax = 0;
+            for (int j = 0; j < ncl; ++j)
+                if (s_cl[j][2] > 0 && s_cl[j][3] + s_cl[j][2] - 1 > kbmax) kbmax = s_cl[j][3] + s_cl[j][2] - 1;
+            s_kbmax = kbmax;
+        }
+        cta_sync();
+        const int ncl = s_ncl;
+        // the tasks (block, client) in block order; task n goes to group n % 3
+        {
+            const int span = hd.help_end - hd.help_k0;
+            for (int idx = tid; idx < ncl * span; idx += NT) {
+                const int j = idx / span, x = idx - j * span;
+                if (x >= s_cl[j][2]) continue;
+                const int kb = s_cl[j][3] + x;
+                int n = 0;
+                for (int j2 = 0; j2 < ncl; ++j2) {
+                    const int before = min(max(kb - s_cl[j2][3], 0), s_cl[j2][2]);   // tasks of client j2 in earlier blocks
+                    n += before + ((j2 < j && (unsigned)(kb - s_cl[j2][3]) < (unsigned)s_cl[j2][2]) ? 1 : 0);
+                }
+                tasks[(n % HELP_GROUPS) * TG + n / HELP_GROUPS] = (uint16_t)(kb | (j << 8));
+            }
+        }
+        for (int j = 0; j < ncl; ++j) {
+            const int st = s_cl[j][1];
+            const uint32_t* src = s == 0 ? d.spins + (size_t)st * W : hd.spub + ((size_t)((s - 1) & 1) * R + st) * W;
+            for (int w = tid; w < W; w += NT) spc[j * W + w] = __ldcg(src + w);
+        }
+        cta_sync();
+        for (int j = 0; j < ncl; ++j) {
+            const int t = s_cl[j][0], K = s_cl[j][2], o = s_cl[j][3], off = s_cl[j][4];
+            for (int n = tid; n < 32 * K; n += NT) {
+                const int i = 32 * o + n;
+                const uint32_t a = (uint32_t)get_nibble(spc + j * W, i);
+                const Philox4 p = philox4x32_10((uint32_t)i, sweep, (uint32_t)t, c3, d.key0, d.key1);
+                const uint32_t k = __umulhi(p.w0, (uint32_t)(q - 1));
+                const uint32_t b = k + (k >= a ? 1u : 0u);
+                unsigned long long ta = 0x0101010101010101ull;
+                ta += 1ull << (8 * a);
+                ta -= 1ull << (8 * b);
+                hlut[off + n] = make_uint2((uint32_t)ta, (uint32_t)(ta >> 32));
+            }
+        }
+        cta_sync();
+#ifdef PT_TIMING
+        const long long h_t1 = clock64();
+        hacc[0] += h_t1 - h_t0;
+#endif
+        int chunk = 0;
+        const int ntask = s_ntask, kbmax = s_kbmax;
+        for (int idx = 0;; ++idx) {
+            const bool more = HELP_GROUPS * idx + gi < ntask;
+            const unsigned tk = more ? tasks[gi * TG + idx] : 0u;
+            const int kb = more ? (int)(tk & 255u) : kbmax + 1, j = (int)(tk >> 8);
+            // every group passes the same refresh points (also the groups that have no task behind them)
+            while (65 + 16 * chunk <= kbmax && kb >= 65 + 16 * chunk) {
+                // the tasks from here on read blocks 16 chunk .. 16 chunk + 15 as decided in this sweep
+                const int kr = 65 + 16 * chunk;
+                if (tid < ncl && s_cl[tid][2] > 0 && s_cl[tid][3] + s_cl[tid][2] > kr)
+                    wait_arrivals(hd.mprog + s_cl[tid][1], (unsigned)(s * (NB >> 4) + chunk + 1), d.err);
+                cta_sync();
+                for (int j2 = 0; j2 < ncl; ++j2) {
+                    if (!(s_cl[j2][2] > 0 && s_cl[j2][3] + s_cl[j2][2] > kr)) continue;
+                    const uint32_t* src = hd.spub + ((size_t)(s & 1) * R + s_cl[j2][1]) * W + 64 * chunk;
+                    for (int w = tid; w < 64; w += NT) spc[j2 * W + 64 * chunk + w] = __ldcg(src + w);
+                }
+                cta_sync();
+                ++chunk;
+            }
+            if (!more) break;
+            {
+                const int o = s_cl[j][3];
+#ifdef PT_TIMING
+                const long long h_t2 = clock64();
+#endif
+                const uint32_t* sp = spc + j * W;
+                const uint2* lutp = hlut + s_cl[j][4] + (kb - o) * 32 + gbase;
+                int wj = 4 * kb + 8 * jr;
+                wj -= wj >= W ? W : 0;
+                int wj2 = wj + 4;
+                wj2 -= wj2 >= W ? W : 0;
+                const uint4 wa = *reinterpret_cast<const uint4*>(sp + wj);
+                const uint4 wb = *reinterpret_cast<const uint4*>(sp + wj2);
+                const uint32_t words[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
+                uint2 lt[DIRECT_SITES];
+#pragma unroll
+                for (int mm = 0; mm < DIRECT_SITES; ++mm) lt[mm] = lutp[2 * mm];
+                uint32_t alo[DIRECT_SITES], alo2[DIRECT_SITES];
+#pragma unroll
+                for (int mm = 0; mm < DIRECT_SITES; ++mm) { alo[mm] = 0u; alo2[mm] = 0u; }
+#pragma unroll
+                for (int u = 0; u < 16; ++u) {
+                    const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
+#pragma unroll
+                    for (int mm = 0; mm < DIRECT_SITES; ++mm) {
+                        const uint32_t S = prmt(lt[mm].x, lt[mm].y, sel);
+                        const int tt = 7 - mm + 2 * u;
+                        alo[mm] = __dp2a_lo(PL[tt], S, alo[mm]);
+                        alo2[mm] = __dp2a_hi(PL[tt + 1], S, alo2[mm]);
+                    }
+                }
+                uint32_t val[DIRECT_SITES];
+#pragma unroll
+                for (int mm = 0; mm < DIRECT_SITES; ++mm) val[mm] = alo[mm] + alo2[mm];
+                uint32_t* gp = gpart + (gi * 2 + (gcnt & 1)) * 32;
+                {
+                    uint32_t v4[4], v2[2];
+                    const bool u4 = lane & 16, u3 = lane & 8, u2 = lane & 4;
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+                        v4[i] = (u4 ? val[i + 4] : val[i]) + __shfl_xor_sync(0xffffffffu, u4 ? val[i] : val[i + 4], 16);
+#pragma unroll
+                    for (int i = 0; i < 2; ++i)
+                        v2[i] = (u3 ? v4[i + 2] : v4[i]) + __shfl_xor_sync(0xffffffffu, u3 ? v4[i] : v4[i + 2], 8);
+                    const uint32_t v1 = (u2 ? v2[1] : v2[0]) + __shfl_xor_sync(0xffffffffu, u2 ? v2[0] : v2[1], 4);
+                    const int msite = (u2 ? 1 : 0) + (u3 ? 2 : 0) + (u4 ? 4 : 0);
+                    atomicAdd(&gp[gbase + 2 * msite], v1);
+                }
+                asm volatile("bar.sync %0, 128;" ::"r"(2 + gi) : "memory");
+                if (wg == 0) {
+                    const uint32_t v = gp[lane];
+                    gp[lane] = 0u;   // this buffer is used again two tasks later, behind the next task's barrier
+                    __stcg(hd.hs + (size_t)s_cl[j][1] * L + 32 * kb + lane,
+                           (unsigned long long)v | ((unsigned long long)(uint32_t)(s + 1) << 32));
+                }
+                ++gcnt;
+#ifdef PT_TIMING
+                hacc[1] += clock64() - h_t2;
+                hacc[2] += 1;
+#endif
+            }
+        }
+#ifdef PT_TIMING
+        hacc[3] += clock64() - h_t1;
+#endif
+        cta_sync();
+    }
+#ifdef PT_TIMING
+    if (lane == 0 && d.dbg) {
+        hacc[4] = clock64() - h_start;
+        for (int n = 0; n < 8; ++n) d.dbg[((size_t)blockIdx.x * 32 + (tid >> 5)) * 8 + n] += hacc[n];
+    }
+#endif
+}
+
 // NEARQ = 0: the bulk warps sum both 16-bit halves of every coupling.  NEARQ = 1, 2, 4: they sum the low halves
 // only, plus the high halves of NEARQ of the 56 quads of sites within distance 95 of the block (requires
 // r_hi <= 95 and NEARQ * L/64 >= 56).  NJR64: L == 4096 (64 j-ranges as a compile-time constant).
 // MINB: minimum CTAs per SM the register allocation must allow (1: up to 168 registers, for large L; 2: 80 registers,
 // so that several hundred small replicas can be co-resident for persistent launches); 3 stands for the L > 4096
 // build: one CTA of up to DIRECT_BIG_THREADS threads per SM, 80 registers.
-template <int NEARQ, bool NJR64, bool Q16, int MINB, bool FAR = false>
+template <int NEARQ, bool NJR64, bool Q16, int MINB, bool FAR = false, bool HELPT = false>
 __global__ void __launch_bounds__(MINB == 3 ? DIRECT_BIG_THREADS : DIRECT_MAX_THREADS, MINB == 3 ? 1 : MINB)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi) {
     // swap_mode 0: no swap event; 1: one event at the end of the launch (last-arriving CTA, nobody waits);
@@ -407,9 +656,23 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     __shared__ int s_perm[DIRECT_MAX_PERSIST_REP];
     __shared__ long long s_Eall[DIRECT_MAX_PERSIST_REP];
     __shared__ double s_scale[DIRECT_MAX_PERSIST_REP];
+    // HELPERS only (no shared memory in the other instantiations): hot flags by slot, this sweep's window (K, o),
+    // accepted changes of the sweep
+    __shared__ uint8_t s_hot[HELPT ? DIRECT_MAX_PERSIST_REP : 1];
+    __shared__ int s_hk[HELPT ? 2 : 1], s_nacc;
     PersistSmem ps;
-    ps.perm = s_perm; ps.Eall = s_Eall; ps.slot = &s_slot;
+    ps.perm = s_perm; ps.Eall = s_Eall; ps.slot = &s_slot; ps.hot = s_hot;
     int event = 0;   // swap events so far in this (persistent) launch
+    // HELPERS: only this instantiation (configs[3]: L = 4096, q <= 8, one near quad per thread), one ensemble,
+    // persistent launch with a swap event after every sweep
+    constexpr bool HELP = HELPT;
+    HelpDev hd = {};
+    if (HELP && d.hlp) hd = *d.hlp;
+    const bool help = HELP && hd.n_help > 0 && swap_mode == 2 && swap_every == 1;
+    if (HELP && help && (int)blockIdx.x >= d.n_rep) {
+        direct_helper_cta(d, smem_d, ps, sweep0, n_sweeps);
+        return;
+    }
     // full[s]: the block sums of buffer s are complete (one arrival per bulk warp);
     // done[s]: the chain warps have decided the block of buffer s and written its spins (one arrival).
     __shared__ __align__(8) uint64_t s_full[2], s_done[2];
@@ -436,6 +699,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             for (int t2 = tid; t2 < d.n_rep; t2 += NT) {                     \
                 s_perm[t2] = d.perm[(size_t)e * d.n_rep + t2];               \
                 s_scale[t2] = d.thr_scale[t2];                               \
+                if (HELPT) s_hot[t2] = 1;                                    \
             }                                                                \
     } while (0)
 #ifdef PT_TIMING
@@ -553,9 +817,16 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
 
         for (int s = 0; s < n_sweeps; ++s) {
             PT_T0(t_draw);
+            if (HELP && help && tid == 0) {
+                const HelpPlan pl = help_plan(s_hot, t, hd.n_help, d.n_rep, hd.help_cap, hd.help_end, hd.help_whot, hd.help_k0);
+                s_hk[0] = pl.K; s_hk[HELPT ? 1 : 0] = pl.o;
+            }
             direct_draw<Q16>(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
             cta_sync();
             PT_ACC(0, t_draw);
+            // HELPERS: in the window, bulk warps 0..3 (j-ranges 0..31) leave their main loop to the helper
+            const int hK = (HELP && help && warp < 4) ? s_hk[0] : 0, ho = (HELP && help) ? s_hk[HELPT ? 1 : 0] : 0;
+            uint32_t* spubp = (HELP && help) ? hd.spub + ((size_t)(s & 1) * d.n_rep + st) * W : nullptr;
             // the four barriers are initialised once per launch; every sweep completes NB/2 phases of each
             const int phase0 = s * (NB >> 1);
             PT_T0(t_loop);
@@ -572,11 +843,23 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 wn[iq] = ((jr + NJR * iq) >> 1) - 12;
                 wn[iq] += wn[iq] < 0 ? W : 0;
             }
-            for (int kb = 0; kb < NB; ++kb) {
+            // SKIP (HELPERS, bulk warps 0..3 inside the window): the main loop of the block is the helper's
+            auto bulk_block = [&](const int kb, auto skip_t) {
+                constexpr bool SKIP = decltype(skip_t)::value;
                 // block kb is summed against: blocks < kb-1 final (the chain warp is done with block kb-2, which
                 // also frees buffer kb&1), block kb-1 as at the start of the sweep, blocks >= kb untouched
                 if (kb >= 2) mbar_wait(&s_done[kb & 1], (uint32_t)(phase0 + (kb >> 1) - 1) & 1u);
                 PT_T0(t_b);
+                if (HELP && help && warp == 7 && kb >= 2) {
+                    // HELPERS: block kb-2 is final: a copy for the helpers (this sweep's wrapped ranges, the next
+                    // sweep's start), and after every 16 blocks the progress counter
+                    if (lane < 4) __stcg(spubp + 4 * (kb - 2) + lane, m.sp[4 * (kb - 2) + lane]);
+                    if ((kb & 15) == 1) {
+                        if (lane < 4) __threadfence();
+                        __syncwarp();
+                        if (lane == 0) *(volatile unsigned*)(hd.mprog + st) = (unsigned)(s * (NB >> 4) + ((kb - 1) >> 4));
+                    }
+                }
                 // FAR: block kb-2 is final: its colour counts (a far range reads them 30 blocks later at the earliest)
                 int rcv = 0;
                 if (FAR && kb >= 2 && warp == (kb & 7))
@@ -639,7 +922,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                                 acc = dp4a_u32_u32(PL[23 + 7 - mm + 2 * u], prmt(lt[mm].x, lt[mm].y, sel), acc);
                             }
                         }
-                    } else {
+                    } else if (!SKIP) {
 #pragma unroll
                     for (int u = 0; u < 16; ++u) {
                         const uint32_t sel = (u & 1) ? (words[u >> 1] >> 16) : words[u >> 1];
@@ -708,10 +991,28 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                     if (lane < 8) reinterpret_cast<uint8_t*>(s_cnt8 + kb - 2)[lane] = (uint8_t)rcv;
                 }
                 PT_ACC(1, t_b);
+            };
+            if constexpr (!HELP) {
+                for (int kb = 0; kb < NB; ++kb) bulk_block(kb, std::false_type{});
+            } else {
+                // blocks [0, k1) and [k2, NB) in full, [k1, k2) (the helper's window, bulk warps 0..3 only) without the main loop
+                const int k1 = (HELP && hK > 0) ? ho : NB, k2 = (HELP && hK > 0) ? ho + hK : NB;
+                for (int seg = 0; seg < 2; ++seg) {
+                    const int lo = seg ? k2 : 0, hi = seg ? NB : k1;
+                    for (int kb = lo; kb < hi; ++kb) bulk_block(kb, std::false_type{});
+                    if (HELP && seg == 0)
+                        for (int kb = k1; kb < k2; ++kb) bulk_block(kb, std::true_type{});
+                }
             }
             PT_ACC(2, t_loop);
             PT_T0(t_end);
             cta_sync();  // the chain warp has decided the last block and published its sums
+            if (HELP && help && warp == 7) {   // the last two blocks and the closing progress count
+                if (lane < 8) __stcg(spubp + 4 * (NB - 2) + lane, m.sp[4 * (NB - 2) + lane]);
+                if (lane < 8) __threadfence();
+                __syncwarp();
+                if (lane == 0) *(volatile unsigned*)(hd.mprog + st) = (unsigned)((s + 1) * (NB >> 4));
+            }
             if (FAR && warp < 2) recount_block(m.sp, s_cnt8, NB - 2 + warp, lane);
             PT_ACC(6, t_end);
             PT_T0(t_nm);
@@ -720,7 +1021,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             cta_sync();
             PT_ACC(7, t_nm);
             if (swap_mode == 2 && (sweep0 + s + 1) % swap_every == 0) {
-                t = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, &s_E, event++);
+                t = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, &s_E, event++, help, HELPT ? s_nacc : 0);
                 scale = s_scale[t];
             }
             PT_ACC(3, t_end);
@@ -766,10 +1067,16 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             direct_draw<Q16>(d, m, (uint32_t)(sweep0 + s + 1), t, c3, scale);
             cta_sync();
             const int phase0 = s * (NB >> 1);
+            // HELPERS: window of this sweep, the helper's sums (by storage index) and the copy of the decided blocks
+            const int hK = (HELP && help) ? s_hk[0] : 0, ho = (HELP && help) ? s_hk[HELPT ? 1 : 0] : 0;
+            const unsigned long long* hsp = (HELP && help) ? hd.hs + (size_t)st * L + lane : nullptr;
+            unsigned long long hs_next = 0ull;
             long long dE_acc = 0;
             int n_acc = 0;
             uint32_t mp = 0u;   // accept mask of the previous block
-            for (int k = 0; k < NB; ++k) {
+            // WIN (HELPERS, inside the window): the helper's sums are added to the block sums
+            auto chain_block = [&](const int k, auto win_t) {
+                constexpr bool WIN = decltype(win_t)::value;
                 const int i0 = k << 5;
                 // independent of the bulk: threshold, the words of the block for the final update, and the
                 // correction rows (from the colours at the start of the sweep and the proposals: selb)
@@ -782,6 +1089,9 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 ipv += ipv < 0 ? L : 0;
                 const uint2 sfp = *reinterpret_cast<const uint2*>(m.selb + ipv);            // a | b << 4 of 8 sites
                 const uint2 sfo = *reinterpret_cast<const uint2*>(m.selb + i0 + 8 * cw);
+                unsigned long long hs_cur = hs_next;   // asked for one block ahead (it may not have been there yet)
+                if (WIN && k + 1 < ho + hK)
+                    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(hs_next) : "l"(hsp + 32 * (k + 1)) : "memory");
                 int cp[8], co[8];
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
@@ -803,7 +1113,32 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 }
                 mbar_wait(&s_full[k & 1], (uint32_t)(phase0 + (k >> 1)) & 1u);
                 PT_T0(t_c);
-                const uint32_t S = m.part[(k & 1) * 32 + lane];
+                uint32_t S = m.part[(k & 1) * 32 + lane];
+                if (WIN) {
+                    // the helper's part of the block sums: every lane waits for its own word to carry this sweep's stamp
+                    const uint32_t stamp = (uint32_t)(s + 1);
+                    PT_T0(t_p);
+                    unsigned polls = 0u;
+                    unsigned long long t0 = 0ull;
+                    while (__any_sync(0xffffffffu, (uint32_t)(hs_cur >> 32) != stamp)) {
+                        if ((uint32_t)(hs_cur >> 32) != stamp)
+                            asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(hs_cur) : "l"(hsp + 32 * k) : "memory");
+                        if ((++polls & 255u) == 0u) {
+                            unsigned long long now;
+                            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+                            if (t0 == 0ull) t0 = now;
+                            if (now - t0 > DIRECT_BARRIER_TIMEOUT_NS || *(volatile int*)d.err != 0) {
+                                *(volatile int*)d.err = 1;
+                                break;
+                            }
+                        }
+                    }
+                    S += (uint32_t)hs_cur;
+                    PT_ACC(6, t_p);
+#ifdef PT_TIMING
+                    tacc[7] += polls;
+#endif
+                }
                 // slack y = theta - dE: the site accepts iff y >= 0 (theta <= 2^30 and |dE| < 2^30: no overflow)
                 int y = th - (int)(S - rowsum);
                 PT_ACC(1, t_c);
@@ -853,7 +1188,8 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
 #endif
                 if (cw == 0 && lane < 4) {
                     const uint32_t nm = expand_bits_to_nibbles(mask >> (8 * lane));
-                    m.sp[wsp] = (w_old & ~nm) | (w_new & nm);
+                    const uint32_t w_dec = (w_old & ~nm) | (w_new & nm);
+                    m.sp[wsp] = w_dec;
                 }
                 // every chain warp has read the block sums of buffer k&1 (without rounds there is no other barrier
                 // between a slow warp's read and this point) before they are cleared and the buffer is handed back
@@ -867,6 +1203,19 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 }
                 mp = mask;
                 PT_ACC(0, t_c);
+            };
+            if constexpr (!HELP) {
+                for (int k = 0; k < NB; ++k) chain_block(k, std::false_type{});
+            } else {
+                const int k1 = (HELP && hK > 0) ? ho : NB, k2 = (HELP && hK > 0) ? ho + hK : NB;
+                for (int seg = 0; seg < 2; ++seg) {
+                    const int lo = seg ? k2 : 0, hi = seg ? NB : k1;
+                    for (int k = lo; k < hi; ++k) chain_block(k, std::false_type{});
+                    if (HELP && seg == 0 && k1 < k2) {
+                        asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(hs_next) : "l"(hsp + 32 * k1) : "memory");
+                        for (int k = k1; k < k2; ++k) chain_block(k, std::true_type{});
+                    }
+                }
             }
             for (int o = 16; o > 0; o >>= 1) dE_acc += __shfl_xor_sync(0xffffffffu, dE_acc, o);
             if (owner) s_E += dE_acc;
@@ -877,10 +1226,11 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 oa.acc += n_acc;
                 oa.att += L;
                 oa.sample(s_E, nmax);
+                if (HELPT) s_nacc = n_acc;
             }
             cta_sync();
             if (swap_mode == 2 && (sweep0 + s + 1) % swap_every == 0) {
-                const int t_new = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, &s_E, event++);
+                const int t_new = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, &s_E, event++, help, HELPT ? s_nacc : 0);
                 if (t_new != t) {   // the accumulators belong to the slot: hand them over when the slot changes
                     if (owner) {
                         oa.flush(d.obs + (size_t)e * d.n_rep + t);
@@ -1028,6 +1378,11 @@ typedef void (*direct_kernel_t)(Dev, long long, int, int, int, int);
 // r_hi = largest r <= L/2 with Jq[r] >= 2^16 (0 if none).
 // minb = 1: up to 168 registers per thread (fastest block sums); minb = 2: 80 registers, twice the CTAs per SM.
 inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb) {
+    // PT_HELPERS=<n> (n > 0; L = 4096, q <= 8, one ensemble): the instantiation with helper CTAs (HELPERS above)
+    const char* eh = getenv("PT_HELPERS");
+    const bool want_help = eh && atoi(eh) > 0 && d.n_ens == 1 && d.L == 4096 && d.q <= 8 && !d.far && minb == 1 &&
+                           direct_nearq(d.L, r_hi) == 1;
+    if (want_help) return sweep_direct_kernel<1, true, false, 1, false, true>;
 #ifdef PT_ONLY_HEADLINE   // development builds: only the configs[3] instantiation (fast to compile)
     return d.far ? sweep_direct_kernel<1, true, false, 1, true> : sweep_direct_kernel<1, true, false, 1>;
 #else
@@ -1102,11 +1457,13 @@ inline direct_kernel_t select_direct_kernel(const Dev& d, int r_hi, int device, 
 // contexts that still use swap_mode 1 it was slower than ordinary launches: 0.41-0.48 s against 0.39 s for 10000
 // sweeps of configs[2].)
 inline int launch_sweep_direct(direct_kernel_t kern, const Dev& d, long long sweep0, int n_sweeps, int swap_mode,
-                               int swap_every, int r_hi, cudaStream_t stream) {
-    const size_t smem = direct_smem_bytes(d.L, d.q);
+                               int swap_every, int r_hi, cudaStream_t stream, int n_help = 0, int help_cap = 0) {
+    size_t smem = direct_smem_bytes(d.L, d.q);
+    const bool help = swap_mode == 2 && n_help > 0;
+    if (help && direct_help_smem_bytes(d.L, help_cap) > smem) smem = direct_help_smem_bytes(d.L, help_cap);
     cudaError_t err = cudaSuccess;   // (the shared-memory attribute was set once, in direct_coresident)
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)(swap_mode == 3 ? d.n_local : d.n_ens * d.n_rep));
+    cfg.gridDim = dim3((unsigned)(swap_mode == 3 ? d.n_local : d.n_ens * d.n_rep + (help ? n_help : 0)));
     cfg.blockDim = dim3((unsigned)direct_threads(d.L));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
