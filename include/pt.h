@@ -50,13 +50,18 @@ typedef enum {
     PT_EOVERFLOW = -2, /* sum_r Jq[r] >= 2^31: dE would not fit int32 (sigma too small) */
     PT_ENOMEM = -3,    /* host or device allocation failed */
     PT_ECUDA = -4,     /* CUDA runtime error, no device, or not an sm_100 device */
-    PT_ECAPACITY = -5  /* no sweep variant fits the shared memory of one SM for (L,q) */
+    PT_ECAPACITY = -5  /* no sweep variant fits the shared memory of one SM (field variant: of a cluster of 8 SMs) for (L,q) */
 } pt_status;
 
 /* Sweep variants (pt_set_variant).  Both produce bit-identical trajectories.
  *  PT_VARIANT_FIELD : per-colour local fields h[k][i] = sum_{j!=i} Jq[|i-j|][s_j==k]
  *                     kept in shared memory; a proposal costs O(1), an accepted
- *                     change updates two columns of h (north_star (3)).
+ *                     change updates two columns of h (north_star (3)).  Where
+ *                     L*q*4 bytes + tables exceed one SM's 227 KB, a replica takes
+ *                     a thread-block cluster of 2, 4 or 8 CTAs, each holding the
+ *                     fields of L/C consecutive sites (sequential site order only;
+ *                     needs L % (8 C) == 0; DSMEM carries one 16-byte record per
+ *                     accepted change to every CTA of the cluster).
  *  PT_VARIANT_DIRECT: dE = sum_j Jq[|i-j|]([s_j==a]-[s_j==b]) summed directly
  *                     (PAPER.md:118-124), for blocks of 32 consecutive sites at a
  *                     time, with exact integer corrections for the changes
@@ -66,7 +71,9 @@ typedef enum {
  * Environment: PT_VARIANT=direct|field|auto sets the variant chosen by pt_create; PT_PERSISTENT=0|1|2 the launch
  * policy of the direct variant (0: one launch per swap interval; 1, default: persistent launches with the swap events
  * inside the kernel for contexts that take at least a third of the SMs; 2: whenever all replicas can be co-resident);
- * PT_MINB=1|2 forces the 168- or the 80-register build of the direct sweep kernel (experiments; default: by size).
+ * PT_MINB=1|2|4 forces the 168-, the 80- or (1024 < L <= 2048) the 128-register build of the direct sweep kernel
+ * (experiments; default: by size and replica count).  PT_FIELD_CLUSTER=2|4|8 runs the field variant on clusters of
+ * that size also where one CTA would hold the replica (tests, measurements).
  * PT_FAR=1 (L = 4096, q <= 8) selects the far form of the bulk sum (8-bit coupling residuals beyond 1000 sites;
  * bit-identical results, measured slower than the default form: an experiment kept for reference). */
 enum { PT_VARIANT_AUTO = 0, PT_VARIANT_FIELD = 1, PT_VARIANT_DIRECT = 2, PT_VARIANT_FP32 = 3, PT_VARIANT_FP64 = 4 };
@@ -113,7 +120,7 @@ typedef struct {
  *  q      : number of colours, 2 <= q <= 64.  q <= 16: 4 bits per spin, every variant.  16 < q <= 64: 8 bits per
  *           spin (4 spins per word); the field and the floating-point variants only (the direct kernels are built
  *           on nibble tables), so PT_VARIANT_AUTO resolves to PT_VARIANT_FIELD and needs L*q*4 bytes + tables of
- *           shared memory (PT_ECAPACITY beyond that)
+ *           shared memory, of one SM or spread over a cluster of up to 8 (PT_ECAPACITY beyond that)
  *  sigma  : decay exponent of Eq. 4, finite and > 0
  *  n_ens  : independent ensembles (same model, different random streams) >= 1
  *  n_rep  : replicas per ensemble >= 1

@@ -114,6 +114,16 @@ struct pt_ctx {
 namespace {
 
 bool field_fits(int L, int q) { return ptk::field_smem_bytes(L, q) + 512 <= kSmemLimit; }
+// Local-field variant over a thread-block cluster (sweep_field_cluster_kernel): can C CTAs hold the replica?
+bool field_cluster_fits(int L, int q, int C) {
+    return ptk::field_cluster_divides(L, C) && ptk::field_cluster_smem_bytes(L, q, C) + 4096 <= kSmemLimit;
+}
+// Smallest portable cluster size (2, 4, 8) whose CTAs hold the local fields of one replica; 0 if none does.
+int field_cluster_size(int L, int q) {
+    for (int C = 2; C <= ptk::FIELD_CLUSTER_MAX; C *= 2)
+        if (field_cluster_fits(L, q, C)) return C;
+    return 0;
+}
 bool direct_applies(int L, int q) { return ptk::direct_applies(L, q); }
 
 void free_ctx(pt_ctx* c) {
@@ -152,6 +162,19 @@ int ensure_fields(pt_ctx* c) {
     return PT_OK;
 }
 
+// Cluster size the local-field sweep of this context runs with (0: one CTA per replica).  A replica whose fields do
+// not fit in one SM takes the smallest cluster that holds them; PT_FIELD_CLUSTER=2|4|8 (tests, measurements) asks
+// for a cluster also where one CTA would do.  Sequential site order only.
+int field_cluster_of(const pt_ctx* c) {
+    if (c->site_order == PT_ORDER_RANDOM) return 0;
+    const char* env = getenv("PT_FIELD_CLUSTER");
+    if (env && env[0] >= '2' && env[0] <= '8' && env[1] == 0) {
+        const int C = env[0] - '0';
+        if ((C == 2 || C == 4 || C == 8) && field_cluster_fits(c->L, c->q, C)) return C;
+    }
+    return field_fits(c->L, c->q) ? 0 : field_cluster_size(c->L, c->q);
+}
+
 // rowsum = sum_r Jq[r]: the direct variant keeps theta - dE in int32 and needs |dE| <= rowsum < 2^30 - 1.
 int resolve_variant(int L, int q, long long rowsum, int variant, int* out) {
     const bool direct_ok = direct_applies(L, q) && rowsum < (1ll << 30) - 1;
@@ -161,7 +184,8 @@ int resolve_variant(int L, int q, long long rowsum, int variant, int* out) {
             return fail(PT_EINVAL, "direct variant needs L % 64 == 0, 64 <= L <= 10240 (L <= 9664 for q > 8: shared memory) "
                                    "and sum_r Jq[r] < 2^30 - 1");
     } else if (variant == PT_VARIANT_FIELD) {
-        if (!field_fits(L, q)) return fail(PT_ECAPACITY, "local-field table (L*q*4 bytes) does not fit in shared memory");
+        if (!field_fits(L, q) && !field_cluster_size(L, q))
+            return fail(PT_ECAPACITY, "local-field table (L*q*4 bytes) does not fit in the shared memory of a cluster of 8 SMs");
     } else if (variant == PT_VARIANT_FP32 || variant == PT_VARIANT_FP64) {
         const size_t smem = variant == PT_VARIANT_FP32 ? ptk::float_smem_bytes<float>(L) : ptk::float_smem_bytes<double>(L);
         if (smem + 2048 > kSmemLimit) return fail(PT_ECAPACITY, "couplings and uniforms (L*14 or L*18 bytes) do not fit in shared memory");
@@ -199,6 +223,25 @@ int launch_sweeps(pt_ctx* c, int n_sweeps, int swap_mode, int swap_every) {
             ptk::sweep_float_kernel<double><<<c->R(), ptk::FLOAT_THREADS, ptk::float_smem_bytes<double>(c->L), c->stream>>>(
                 d, c->d_Ef, (long long)c->sweep, n_sweeps, swap_mode == 1 ? 1 : 0);
         }
+    } else if (c->variant == PT_VARIANT_FIELD && field_cluster_of(c) > 0) {
+        // one thread-block cluster per replica: the local fields are spread over the shared memory of C SMs
+        const int C = field_cluster_of(c);
+        typedef void (*field_kernel_t)(ptk::Dev, long long, int, int);
+        const field_kernel_t kern = c->bits() == 8 ? ptk::sweep_field_cluster_kernel<8> : ptk::sweep_field_cluster_kernel<4>;
+        PT_CUDA((cudaError_t)ptk::allow_max_dynamic_smem((const void*)kern, 4096));
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(c->R() * C));
+        cfg.blockDim = dim3((unsigned)ptk::FIELD_THREADS);
+        cfg.dynamicSmemBytes = ptk::field_cluster_smem_bytes(c->L, c->q, C);
+        cfg.stream = c->stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)C;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        PT_CUDA(cudaLaunchKernelEx(&cfg, kern, d, (long long)c->sweep, n_sweeps, swap_mode == 1 ? 1 : 0));
     } else if (c->variant == PT_VARIANT_FIELD) {
         const size_t smem = ptk::field_smem_bytes(c->L, c->q, c->site_order == PT_ORDER_RANDOM);
         typedef void (*field_kernel_t)(ptk::Dev, long long, int, int);

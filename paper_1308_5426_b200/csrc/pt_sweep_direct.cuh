@@ -80,6 +80,8 @@ constexpr int DIRECT_MAX_THREADS = DIRECT_MAX_BULK + 32 * DIRECT_CHAIN_WARPS;
 // L > 4096 (the paper's benchmark range reaches L = 10240): more j-ranges, hence more bulk threads, with
 // the 80-register build of the same code (768 threads x 80 registers fill the register file of an SM).
 constexpr int DIRECT_BIG_BULK = 640;
+// 1024 < L <= 2048: 128 bulk + 128 chain threads; two such CTAs per SM with 128 registers per thread
+constexpr int DIRECT_MID_THREADS = 256;
 constexpr int DIRECT_BIG_THREADS = DIRECT_BIG_BULK + 32 * DIRECT_CHAIN_WARPS;
 constexpr int DIRECT_STATIC_SMEM = 14 * 1024;   // upper bound of the sweep kernel's static shared memory (13568 B)
 constexpr int DIRECT_NPAIR = 39;   // packed coupling pairs per thread and half: 64 + 2*7 couplings
@@ -377,8 +379,10 @@ __device__ __forceinline__ void recount_block(const uint32_t* sp, uint2* cnt8, i
 // MINB: minimum CTAs per SM the register allocation must allow (1: up to 168 registers, for large L; 2: 80 registers,
 // so that several hundred small replicas can be co-resident for persistent launches); 3 stands for the L > 4096
 // build: one CTA of up to DIRECT_BIG_THREADS threads per SM, 80 registers.
+// MINB = 4 stands for the L <= 2048 build: CTAs of at most DIRECT_MID_THREADS threads, two per SM, 128 registers.
 template <int NEARQ, bool NJR64, bool Q16, int MINB, bool FAR = false>
-__global__ void __launch_bounds__(MINB == 3 ? DIRECT_BIG_THREADS : DIRECT_MAX_THREADS, MINB == 3 ? 1 : MINB)
+__global__ void __launch_bounds__(MINB == 3 ? DIRECT_BIG_THREADS : MINB == 4 ? DIRECT_MID_THREADS : DIRECT_MAX_THREADS,
+                                  MINB == 3 ? 1 : MINB == 4 ? 2 : MINB)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi) {
     // swap_mode 0: no swap event; 1: one event at the end of the launch (last-arriving CTA, nobody waits);
     // 2: persistent launch, an event inside the kernel after every sweep whose index is a multiple of swap_every;
@@ -1037,6 +1041,13 @@ inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb) {
         if (d.q <= 8) return nq == 1 ? sweep_direct_kernel<1, false, false, 3> : sweep_direct_kernel<0, false, false, 3>;
         return nq == 1 ? sweep_direct_kernel<1, false, true, 3> : sweep_direct_kernel<0, false, true, 3>;
     }
+    if (minb == 4) {   // 128 registers, two CTAs of at most DIRECT_MID_THREADS threads per SM (nq is 2 or 4 for these L)
+        if (d.q <= 8)
+            return nq == 2 ? sweep_direct_kernel<2, false, false, 4>
+                 : nq == 4 ? sweep_direct_kernel<4, false, false, 4> : sweep_direct_kernel<0, false, false, 4>;
+        return nq == 2 ? sweep_direct_kernel<2, false, true, 4>
+             : nq == 4 ? sweep_direct_kernel<4, false, true, 4> : sweep_direct_kernel<0, false, true, 4>;
+    }
     if (d.q <= 8) {
         if (minb == 1) {
             switch (nq) {
@@ -1073,23 +1084,67 @@ inline int direct_coresident(direct_kernel_t kern, const Dev& d, int device) {
 }
 
 // The kernel a context uses, and how many of its CTAs fit on the device at once (a persistent launch, swap_mode 2,
-// needs all n_ens * n_rep of them).  The 168-register build while all replicas fit in one wave of it; with more
-// replicas than that and L < 2048 the 80-register build, which puts more CTAs on an SM (co-resident or not: where they are
-// not, measured 5-13 % faster at L = 256..1536 with 600..1200 replicas, equal at L = 1024 with 740 and 2.5 % slower
-// with 1200, profiles/r1_g_paper_shapes.md).  From L = 2048
-// on the 80-register build is slower in every case measured (0.250 against 0.194 ms per sweep at L = 2048 with 400
-// replicas although it makes them co-resident; a factor 2 at L = 4096), so it is never picked there.
-// PT_MINB=1|2 (experiments) forces the 168- or, for L <= 4096, the 80-register build.
+// needs all n_ens * n_rep of them).  Three register allocations of the same code: MINB = 1 (up to 168 registers, one
+// CTA per SM at L >= 1088), MINB = 2 (80 registers), MINB = 4 (128 registers, two CTAs of at most 256 threads per SM:
+// 1024 < L <= 2048).  The 168-register build while all replicas fit in one wave of it.  Beyond one wave:
+//  * L <= 1024: the 80-register build (co-resident or not: measured 5-13 % faster at L = 256..1024 with 600..1200
+//    replicas, equal at L = 1024 with 740, 2.5 % slower with 1200, profiles/r1_g_paper_shapes.md);
+//  * 1024 < L <= 2048: whichever of the three has the lowest  waves x (time of a wave),  waves = ceil(replicas / CTAs
+//    resident at once), with the wave times measured at L = 1088, 1536, 2048 with 32..1200 replicas
+//    (profiles/r2_f_two_ctas_per_sm.md): 1 : 1.3-1.5 : 2.55 for 1, 2 and 3 CTAs per SM -- two CTAs of 128 registers
+//    share an SM at 1.3x the time of one (at L = 2048 a CTA has one bulk warp per sub-partition and a block takes
+//    3.5x the clocks of its IDP.2A stream, so a second CTA fills the gaps): 0.163 against 0.191 ms per sweep at
+//    L = 2048 with 400 replicas, 0.434 against 0.544 with 1200; the 80-register build is a factor 1.5 slower at
+//    L = 2048 and never picked there;
+//  * L > 2048: the 168-register build (the 80-register one: a factor 2 slower at L = 4096).
+// A context of fewer than a third of the SMs in CTAs (one of the 40 handles of configs[4]) shares the GPU with others:
+// at 1024 < L <= 2048 it takes the 128-register build where that costs a lone context nothing (low-half bulk sums,
+// q <= 8: 0.0738 against 0.0745 ms at L = 2048 with 32 replicas), so that two of them fit on an SM.
+// PT_MINB=1|2|4 (experiments) forces the 168-, for L <= 4096 the 80-, for 1024 < L <= 2048 the 128-register build.
 inline direct_kernel_t select_direct_kernel(const Dev& d, int r_hi, int device, int* coresident) {
     direct_kernel_t k1 = direct_kernel_variant(d, r_hi, 1);
     int c1 = direct_coresident(k1, d, device);
     const char* env = getenv("PT_MINB");
     const bool force1 = env && env[0] == '1';
     const bool force2 = env && env[0] == '2' && d.L <= 64 * (DIRECT_MAX_BULK / 4);
-    if (force2 || (d.n_ens * d.n_rep > c1 && d.L < 2048 && !force1)) {
+    const bool mid = direct_threads(d.L) <= DIRECT_MID_THREADS && direct_threads(d.L) > 192;   // 1024 < L <= 2048
+    const bool force4 = env && env[0] == '4' && mid;
+    const int R = d.n_ens * d.n_rep;
+    int n_sm = 0;
+    if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) n_sm = 0;
+    if (force1 || c1 <= 0) {
+    } else if (force2) {
+        k1 = direct_kernel_variant(d, r_hi, 2);
+        c1 = direct_coresident(k1, d, device);
+    } else if (force4) {
+        k1 = direct_kernel_variant(d, r_hi, 4);
+        c1 = direct_coresident(k1, d, device);
+    } else if (mid) {
+        const int nq = direct_nearq(d.L, r_hi);
+        if (R > c1) {
+            const double w4 = (d.q <= 8 && nq == 2) ? 1.3 : (d.q <= 8 && nq == 4) ? 1.4 : 1.5, w2 = 2.55;
+            direct_kernel_t k4 = direct_kernel_variant(d, r_hi, 4);
+            const int c4 = direct_coresident(k4, d, device);
+            double best = (double)((R + c1 - 1) / c1);
+            direct_kernel_t kb = k1;
+            int cb = c1;
+            if (c4 > c1 && w4 * ((R + c4 - 1) / c4) < best) { best = w4 * ((R + c4 - 1) / c4); kb = k4; cb = c4; }
+            if (d.L < 2048) {
+                direct_kernel_t k2 = direct_kernel_variant(d, r_hi, 2);
+                const int c2 = direct_coresident(k2, d, device);
+                if (c2 > c1 && w2 * ((R + c2 - 1) / c2) < best) { best = w2 * ((R + c2 - 1) / c2); kb = k2; cb = c2; }
+            }
+            k1 = kb;
+            c1 = cb;
+        } else if (3 * R < n_sm && d.q <= 8 && nq == 2) {
+            direct_kernel_t k4 = direct_kernel_variant(d, r_hi, 4);
+            const int c4 = direct_coresident(k4, d, device);
+            if (c4 > c1) { k1 = k4; c1 = c4; }
+        }
+    } else if (R > c1 && d.L < 2048) {
         direct_kernel_t k2 = direct_kernel_variant(d, r_hi, 2);
         const int c2 = direct_coresident(k2, d, device);
-        if (force2 || c2 > c1) { k1 = k2; c1 = c2; }
+        if (c2 > c1) { k1 = k2; c1 = c2; }
     }
     if (coresident) *coresident = c1;
     return k1;

@@ -161,4 +161,197 @@ sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
     if (do_swap) arrive_and_swap(d, e, (uint32_t)(sweep0 + n_sweeps));
 }
 
+
+// ---------------------------------------------------------------------------
+// Local-field variant beyond one SM's shared memory (north_star (3): "one CTA or
+// thread-block cluster per replica ... (or DSMEM)"): one thread-block CLUSTER of C = 2, 4 or 8 CTAs per replica.
+// CTA c of the cluster owns the sites lo .. lo + L/C - 1, lo = c L/C: their packed spins, proposals, thresholds and
+// the columns h[k][i] of the local fields live in ITS shared memory (q L/C words instead of q L); every CTA keeps the
+// half coupling table Jq[0..L/2] (Jq[r] = Jq[L-r], A3).  The sweep is the same sequential scan as above: the CTA that
+// owns the next site scans its slice for the next accepting site (warp 0, 32 sites at a time) and writes ONE record
+// -- next position, site, colours a -> b, dE -- into the shared memory of EVERY CTA of the cluster through DSMEM
+// (mapa + st.shared::cluster); after a cluster barrier (release/acquire) every CTA applies the change to its own
+// columns, h[a][j] -= Jq[|j-f|], h[b][j] += Jq[|j-f|] for its L/C sites j, so a column update takes 1/C of the time
+// it takes a single CTA.  A record without a site hands the scan to the next CTA at the end of a slice.  Records are
+// double buffered by step parity: record n+2 is written only after every CTA has arrived at barrier n+1, i.e. after
+// it has read record n.  All CTAs see all records, so each keeps the running energy; CTA 0 owns the observables and
+// gets the colour counts of the other slices through DSMEM.  Sequential site order only (A5).
+// dynamic smem (32-bit words): J[L/2 + 8] | theta[L/C] | sp[W/C] | bq[W/C] | h[q L/C]
+// ---------------------------------------------------------------------------
+constexpr int FIELD_CLUSTER_MAX = 8;   // portable cluster size
+
+__host__ __device__ inline size_t field_cluster_smem_bytes(int L, int q, int C) {
+    const int Ls = L / C, Ws = q <= 16 ? Ls / 8 : Ls / 4;
+    return (size_t)((L / 2 + 8) + Ls + 2 * Ws + q * Ls) * 4;
+}
+// every slice is a whole number of packed words
+__host__ __device__ inline bool field_cluster_divides(int L, int C) { return (L % (8 * C)) == 0; }
+
+__device__ __forceinline__ unsigned cluster_ctarank() {
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ unsigned cluster_nctarank() {
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+    return r;
+}
+// all threads of all CTAs of the cluster; the arriving threads' shared-memory writes (local and remote) are visible
+// to every thread behind the wait
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// address of the same shared-memory variable in CTA `rank` of the cluster (shared::cluster window)
+__device__ __forceinline__ uint32_t cluster_map(const void* p, unsigned rank) {
+    uint32_t a = (uint32_t)__cvta_generic_to_shared(p), r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_cluster_v4(uint32_t addr, int4 v) {
+    asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w)
+                 : "memory");
+}
+__device__ __forceinline__ void st_cluster_b32(uint32_t addr, int v) {
+    asm volatile("st.shared::cluster.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+
+template <int BITS>
+__global__ void __launch_bounds__(FIELD_THREADS, 1)
+sweep_field_cluster_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
+    extern __shared__ uint32_t smem_fc[];
+    constexpr int PER = 32 / BITS;
+    constexpr uint32_t CMASK = (1u << BITS) - 1u;
+    const int C = (int)cluster_nctarank(), cr = (int)cluster_ctarank();
+    const int L = d.L, q = d.q, H = L / 2;
+    const int Ls = L / C, Ws = Ls / PER, lo = cr * Ls;
+    int32_t* J = (int32_t*)smem_fc;
+    int32_t* theta = J + (H + 8);
+    uint32_t* sp = (uint32_t*)(theta + Ls);
+    uint32_t* bq = sp + Ws;
+    int32_t* h = (int32_t*)(bq + Ws);
+    __shared__ __align__(16) int s_rec[2][4];                    // the step's record, written by the scanning CTA
+    __shared__ int s_cnt[PT_QMAX];
+    __shared__ int s_call[FIELD_CLUSTER_MAX][PT_QMAX];           // CTA 0: colour counts of every slice
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int rep = blockIdx.x / C;                              // clusters are C consecutive CTAs of the grid
+    const int e = rep / d.n_rep, t = rep % d.n_rep;
+    const int st = d.perm[rep];
+    const size_t x = (size_t)e * d.n_rep + st;
+    uint32_t* g_sp = d.spins + x * d.W + lo / PER;
+    int32_t* g_h = d.h + x * (size_t)q * L + lo;
+
+    for (int r = tid; r <= H; r += FIELD_THREADS) J[r] = d.Jq[r];
+    for (int w = tid; w < Ws; w += FIELD_THREADS) sp[w] = g_sp[w];
+    for (int k = 0; k < q; ++k)
+        for (int jj = tid; jj < Ls; jj += FIELD_THREADS) h[k * Ls + jj] = g_h[(size_t)k * L + jj];
+    long long E = d.E[x];
+    const double scale = d.thr_scale[t];
+    const uint32_t c3 = ((uint32_t)(d.ens_base + e) << 4) | TAG_SWEEP;
+    ObsAcc oa;
+    __syncthreads();
+    cluster_sync_all();   // every CTA of the cluster is running: its shared memory may be written from now on
+    int par = 0;
+
+    for (int s = 0; s < n_sweeps; ++s) {
+        const uint32_t sweep = (uint32_t)(sweep0 + s + 1);
+        // proposals and thresholds of the own sites (A6, A7, A9)
+        for (int w = tid; w < Ws; w += FIELD_THREADS) {
+            const uint32_t word = sp[w];
+            uint32_t bword = 0;
+#pragma unroll
+            for (int n = 0; n < PER; ++n) {
+                const int ii = PER * w + n;
+                const Philox4 p = philox4x32_10((uint32_t)(lo + ii), sweep, (uint32_t)t, c3, d.key0, d.key1);
+                const uint32_t a = (word >> (BITS * n)) & CMASK;
+                const uint32_t k = __umulhi(p.w0, (uint32_t)(q - 1));
+                const uint32_t b = k + (k >= a ? 1u : 0u);
+                bword |= b << (BITS * n);
+                theta[ii] = accept_threshold(uniform53(p.w1, p.w2), scale);
+            }
+            bq[w] = bword;
+        }
+        __syncthreads();
+
+        int pos = 0;   // next site of the sweep (global index): the same in every CTA of the cluster
+        while (pos < L) {
+            if (pos / Ls == cr && warp == 0) {
+                int nxt = lo + Ls, fs = -1, fab = 0, fdE = 0;   // no site found: the scan moves on to the next slice
+                for (int base = pos - lo; base < Ls; base += 32) {
+                    const int n = base + lane;
+                    int a = 0, b = 0, dE = 0;
+                    bool acc = false;
+                    if (n < Ls) {
+                        a = get_colour(sp, n, BITS);
+                        b = get_colour(bq, n, BITS);
+                        dE = h[a * Ls + n] - h[b * Ls + n];
+                        acc = dE <= theta[n];
+                    }
+                    const unsigned m = __ballot_sync(0xffffffffu, acc);
+                    if (m) {
+                        const int src = __ffs(m) - 1;
+                        fs = lo + base + src;
+                        nxt = fs + 1;
+                        fab = __shfl_sync(0xffffffffu, a | (b << 8), src);
+                        fdE = __shfl_sync(0xffffffffu, dE, src);
+                        break;
+                    }
+                }
+                if (lane < C) st_cluster_v4(cluster_map(&s_rec[par][0], (unsigned)lane), make_int4(nxt, fs, fab, fdE));
+                __syncwarp();
+            }
+            cluster_sync_all();
+            const int4 rec = *reinterpret_cast<const int4*>(&s_rec[par][0]);
+            par ^= 1;
+            const int fs = rec.y;
+            if (fs >= 0) {
+                const int a = rec.z & 255, b = rec.z >> 8;
+                int32_t* ha = h + a * Ls;
+                int32_t* hb = h + b * Ls;
+                for (int jj = tid; jj < Ls; jj += FIELD_THREADS) {
+                    int dist = lo + jj - fs;
+                    dist = dist < 0 ? -dist : dist;
+                    dist = dist > H ? L - dist : dist;
+                    const int32_t Jv = J[dist];   // J[0] = 0: the site's own field is unchanged
+                    ha[jj] -= Jv;
+                    hb[jj] += Jv;
+                }
+                if (tid == 0) {
+                    E += rec.w;
+                    oa.acc += 1;
+                    if (fs >= lo && fs < lo + Ls) {
+                        const int ii = fs - lo, sh = (ii % PER) * BITS;
+                        sp[ii / PER] = (sp[ii / PER] & ~(CMASK << sh)) | ((uint32_t)b << sh);
+                    }
+                }
+            }
+            pos = rec.x;
+            __syncthreads();
+        }
+        // a8: sample after the sweep, before the swap event (A15); the colour counts of the slices meet in CTA 0
+        count_nmax(sp, Ws, q, BITS, s_cnt);
+        if (tid < q) st_cluster_b32(cluster_map(&s_call[cr][tid], 0u), s_cnt[tid]);
+        cluster_sync_all();
+        if (cr == 0 && tid == 0) {
+            int nmax = 0;
+            for (int k = 0; k < q; ++k) {
+                int c = 0;
+                for (int cc = 0; cc < C; ++cc) c += s_call[cc][k];
+                nmax = max(nmax, c);
+            }
+            oa.att += L;
+            oa.sample(E, nmax);
+        }
+        __syncthreads();
+    }
+
+    for (int w = tid; w < Ws; w += FIELD_THREADS) g_sp[w] = sp[w];
+    for (int k = 0; k < q; ++k)
+        for (int jj = tid; jj < Ls; jj += FIELD_THREADS) g_h[(size_t)k * L + jj] = h[k * Ls + jj];
+    if (cr == 0 && tid == 0) { d.E[x] = E; oa.flush(d.obs + rep); }
+    cluster_sync_all();   // nobody leaves while its shared memory may still be addressed
+    if (do_swap && cr == 0) arrive_and_swap(d, e, (uint32_t)(sweep0 + n_sweeps));
+}
+
 }  // namespace ptk

@@ -196,6 +196,38 @@ def test_ragged_and_edge_shapes(pt, oracle):
         assert_same_state(g, o, "shape L=%d q=%d" % (L, q))
 
 
+@pytest.mark.parametrize("L,q,sigma,n_rep,force", [
+    (256, 3, 0.4, 5, "2"), (256, 3, 0.4, 5, "4"), (512, 5, 0.8, 4, "8"), (448, 20, 0.5, 3, "4"), (1184, 7, 0.3, 3, "2"),
+    (8192, 8, 0.3, 3, None),      # 256 KB of local fields: does not fit in one SM, cluster of 2
+    (3072, 33, 0.5, 2, None),     # byte-wide spins, 396 KB of local fields: cluster of 2
+    (16384, 6, 0.6, 2, None),     # beyond the direct variant's L <= 10240: 384 KB (+ 32 KB of couplings per CTA), cluster of 4
+    (4096, 40, 0.4, 2, None),     # 640 KB: cluster of 4
+])
+def test_local_fields_over_a_thread_block_cluster(pt, oracle, monkeypatch, L, q, sigma, n_rep, force):
+    """SURVEY.md 8(f) NEXT-2 (L*q*4 bytes beyond one SM's shared memory; north_star (3): "cluster ... DSMEM"):
+    sweep_field_cluster_kernel spreads the local fields of a replica over the shared memory of 2, 4 or 8 CTAs of a
+    thread-block cluster.  Forced on small shapes (PT_FIELD_CLUSTER) and taken by itself where one SM is too small;
+    spins, energies and accumulators bit-identical to the oracle, across swap events and launches."""
+    if force:
+        monkeypatch.setenv("PT_FIELD_CLUSTER", force)
+    else:
+        monkeypatch.delenv("PT_FIELD_CLUSTER", raising=False)
+    b = inputs.geometric_betas(0.6, 2.5, n_rep)
+    g = pt.PT(L, q, sigma, 1, n_rep, b, 4242, variant="field")
+    o = oracle.Oracle(L, q, sigma, 1, n_rep, b, 4242)
+    assert g.get_variant() == "field"
+    assert_same_state(g, o, "cluster start")
+    n_small = 3 if L >= 4096 else 12
+    for k, every in ((1, 1), (n_small, 1), (4, 3)):
+        g.sweeps(k, every)
+        o.sweeps(k, every, field=True, threads=THREADS)
+        assert_same_state(g, o, "cluster L=%d q=%d after +%d" % (L, q, k))
+    if not force:   # what one CTA cannot hold stays refused where no cluster code exists: random site order
+        with pytest.raises(pt.PTError):
+            g.set_site_order("random")
+    g.close()
+
+
 @pytest.mark.parametrize("L,q,sigma,n_ens,n_rep", [(64, 17, 0.5, 2, 5), (200, 33, 0.45, 1, 4), (512, 64, 0.8, 1, 3),
                                                   (1024, 24, 0.3, 1, 6)])
 def test_more_than_16_colours(pt, oracle, L, q, sigma, n_ens, n_rep):
