@@ -369,9 +369,10 @@ def run_cfg4(args):
 
     def steps(n):
         launches = 0
-        for _ in range(n):           # interleaved, so that all 40 streams hold work from the start
+        c = max(1, args.sweeps_per_call)
+        for k in range(0, n, c):     # interleaved, so that all 40 streams hold work from the start
             for g in gs:
-                launches += g.sweeps_async(1, 1)
+                launches += g.sweeps_async(min(c, n - k), 1)
         return launches
 
     steps(W_)
@@ -510,6 +511,8 @@ def main():
     ap.add_argument("--sharded", action="store_true", help="one ensemble with its slots sharded over the GPUs (SURVEY.md 8(e)(2))")
     ap.add_argument("--peaks", action="store_true", help="print the instruction-rate micro-benchmarks (pt_measure_peaks) and exit")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweeps-per-call", type=int, default=1,
+                    help="cfg4: sweeps per pt_sweeps_async call and handle (swap event after every sweep either way)")
     ap.add_argument("--workload", default="cfg3", help="cfg3 (BASELINE.json's headline config, default), cfg4, paper:L or paper:L:R")
     args = ap.parse_args()
     if args.warmup < 3:

@@ -29,8 +29,9 @@
 // two-way dot products), all integer, exact.  The HIGH halves Jq[r] >> 16 are
 // non-zero only for r <= r_hi (71 at L=4096, sigma=0.3): with NEARQ != 0 the
 // main loop sums the low halves only (0.5 IDP.2A per pair term) and each thread
-// adds the high halves of NEARQ of the 56 quads of sites within distance 95 of
-// the block (NEAR); NEARQ = 0 keeps both halves everywhere (small L or sigma).
+// adds the high halves of NEARQ of the quads of sites within distance off - 1
+// of the block (NEAR; off = 96, 160 or 224, the smallest above r_hi: 56, 88 or
+// 120 quads); NEARQ = 0 keeps both halves everywhere (rings shorter than 2 off + 64).
 // Block sums: a transpose-shuffle reduction leaves one site's partial sum per
 // lane, then one shared-memory atomic per lane; every bulk warp then arrives on
 // full[k&1].  Before block k a bulk warp waits on
@@ -86,8 +87,11 @@ constexpr int DIRECT_BIG_THREADS = DIRECT_BIG_BULK + 32 * DIRECT_CHAIN_WARPS;
 constexpr int DIRECT_STATIC_SMEM = 14 * 1024;   // upper bound of the sweep kernel's static shared memory (13568 B)
 constexpr int DIRECT_NPAIR = 39;   // packed coupling pairs per thread and half: 64 + 2*7 couplings
 constexpr int ENERGY_MAX_THREADS = 512, ENERGY_NPAIR = 35;   // energy_direct_kernel: 4 sites x 64 j per thread
-constexpr int DIRECT_NEAR_R = 95;  // NEAR covers |i-j| <= 95: the 224 sites (56 quads) around a block
-constexpr int DIRECT_NEAR_QUADS = 56;
+// NEAR covers |i-j| < off, off = 96, 160 or 224 (the smallest that is > r_hi): the off/2 + 8 quads of sites from off
+// sites before the block to off sites behind it (56 quads for off = 96: sigma >= 0.22 at scale 2^24; 88 for sigma >=
+// 0.1; 120 for sigma >= 0.03, below which sum_r Jq[r] >= 2^30 rules the direct variant out anyway).  0: r_hi is beyond
+// every window.
+__host__ __device__ inline int direct_near_off(int r_hi) { return r_hi < 96 ? 96 : r_hi < 160 ? 160 : r_hi < 224 ? 224 : 0; }
 constexpr int DIRECT_MAX_PERSIST_REP = 512;   // replicas per ensemble in a persistent launch (static shared arrays)
 
 __host__ __device__ inline size_t direct_smem_bytes(int L, int q);
@@ -110,9 +114,9 @@ __host__ __device__ inline int energy_threads(int L) {
 __host__ __device__ inline int direct_threads(int L) { return direct_bulk_threads(L) + 32 * DIRECT_CHAIN_WARPS; }
 // Near quads per bulk thread (template parameter NEARQ): 0 = the bulk warps sum both halves everywhere.
 __host__ __device__ inline int direct_nearq(int L, int r_hi) {
-    const int njr = L / 64;
-    const int nq = (DIRECT_NEAR_QUADS + njr - 1) / njr;
-    if (r_hi > DIRECT_NEAR_R || L < 256 || nq > 4) return 0;
+    const int njr = L / 64, off = direct_near_off(r_hi);
+    const int nq = (off / 2 + 8 + njr - 1) / njr;
+    if (off == 0 || L < 2 * off + 64 || nq > 4) return 0;
     return nq == 3 ? 4 : nq;
 }
 // dynamic smem (32-bit words): theta[L] | lut[2L] | lutb[2L] (q > 8 only) | sp[W] | sp0[W] | bq[W] | selb[L/4] | part[64] | Jz[96]
@@ -374,13 +378,16 @@ __device__ __forceinline__ void recount_block(const uint32_t* sp, uint2* cnt8, i
 }
 
 // NEARQ = 0: the bulk warps sum both 16-bit halves of every coupling.  NEARQ = 1, 2, 4: they sum the low halves
-// only, plus the high halves of NEARQ of the 56 quads of sites within distance 95 of the block (requires
-// r_hi <= 95 and NEARQ * L/64 >= 56).  NJR64: L == 4096 (64 j-ranges as a compile-time constant).
+// only, plus the high halves of NEARQ of the off/2 + 8 quads of sites within distance off - 1 of the block (requires
+// r_hi < off = direct_near_off(r_hi) and NEARQ * L/64 >= off/2 + 8).  NJR64: L == 4096 (64 j-ranges as a compile-time
+// constant).
 // MINB: minimum CTAs per SM the register allocation must allow (1: up to 168 registers, for large L; 2: 80 registers,
 // so that several hundred small replicas can be co-resident for persistent launches); 3 stands for the L > 4096
 // build: one CTA of up to DIRECT_BIG_THREADS threads per SM, 80 registers.
 // MINB = 4 stands for the L <= 2048 build: CTAs of at most DIRECT_MID_THREADS threads, two per SM, 128 registers.
-template <int NEARQ, bool NJR64, bool Q16, int MINB, bool FAR = false>
+// WIDE: the near window is direct_near_off(r_hi) = 160 or 224 sites (a run-time value); else 96 (compile-time: the
+// schedule of the headline instantiation is sensitive to every instruction).
+template <int NEARQ, bool NJR64, bool Q16, int MINB, bool FAR = false, bool WIDE = false>
 __global__ void __launch_bounds__(MINB == 3 ? DIRECT_BIG_THREADS : MINB == 4 ? DIRECT_MID_THREADS : DIRECT_MAX_THREADS,
                                   MINB == 3 ? 1 : MINB == 4 ? 2 : MINB)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi) {
@@ -522,9 +529,10 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             }
             if (!FULL_HI) PH[0] = 0u;
         }
-        // NEAR: high halves of quad n = jr + NJR*iq (sites i0 - 96 + 4n + {0..3}) for this thread's 4 sites:
-        // NP[iq][mm][0] = hi(|r|) | hi(|r-1|) << 16, [1] = hi(|r-2|) | hi(|r-3|) << 16, r = gbase + 2mm + 96 - 4n,
-        // hi(x) = Jq[x] >> 16 for 1 <= x <= r_hi, else 0.
+        // NEAR: high halves of quad n = jr + NJR*iq (sites i0 - NOFF + 4n + {0..3}) for this thread's 8 sites:
+        // NP[iq][mm][0] = hi(|r|) | hi(|r-1|) << 16, [1] = hi(|r-2|) | hi(|r-3|) << 16, r = gbase + 2mm + NOFF - 4n,
+        // hi(x) = Jq[x] >> 16 for 1 <= x <= r_hi, else 0.  NOFF = 96, 160 or 224 sites (direct_near_off), NQD quads.
+        const int NOFF = (NEARQ && WIDE) ? direct_near_off(r_hi) : 96, NQD = NOFF / 2 + 8;
         uint32_t NP[NQ][DIRECT_SITES][2];
         if (NEARQ) {
 #pragma unroll
@@ -535,9 +543,9 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                     uint32_t hv[4];
 #pragma unroll
                     for (int c = 0; c < 4; ++c) {
-                        int r = gbase + 2 * mm + 96 - 4 * n - c;
+                        int r = gbase + 2 * mm + NOFF - 4 * n - c;
                         r = r < 0 ? -r : r;
-                        hv[c] = (active && n < DIRECT_NEAR_QUADS && r >= 1 && r <= r_hi) ? ((uint32_t)__ldg(d.Jq + r) >> 16)
+                        hv[c] = (active && n < NQD && r >= 1 && r <= r_hi) ? ((uint32_t)__ldg(d.Jq + r) >> 16)
                                                                                         : 0u;
                     }
                     NP[iq][mm][0] = hv[0] | (hv[1] << 16);
@@ -573,7 +581,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             int wn[NQ];                                         // NEAR: word of quad n = jr + NJR*iq
 #pragma unroll
             for (int iq = 0; iq < NQ; ++iq) {
-                wn[iq] = ((jr + NJR * iq) >> 1) - 12;
+                wn[iq] = ((jr + NJR * iq) >> 1) - (NOFF >> 3);
                 wn[iq] += wn[iq] < 0 ? W : 0;
             }
             for (int kb = 0; kb < NB; ++kb) {
@@ -600,9 +608,9 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                     }
                     uint32_t nword[NQ];
 #pragma unroll
-                    for (int iq = 0; iq < NQ; ++iq) {   // quads 16..23 are block kb-1: sweep-start copy
+                    for (int iq = 0; iq < NQ; ++iq) {   // the 8 quads before quad NOFF/4 are block kb-1: sweep-start copy
                         const int n = jr + NJR * iq;
-                        nword[iq] = NEARQ ? ((n >= 16 && n < 24) ? m.sp0 : m.sp)[wn[iq]] : 0u;
+                        nword[iq] = NEARQ ? ((n >= (NOFF >> 2) - 8 && n < (NOFF >> 2)) ? m.sp0 : m.sp)[wn[iq]] : 0u;
                     }
                     // two accumulators per site (even / odd pair of j) keep the IDP.2A chains short
                     uint32_t alo[DIRECT_SITES], alo2[DIRECT_SITES], ahi[DIRECT_SITES];
@@ -1031,12 +1039,25 @@ typedef void (*direct_kernel_t)(Dev, long long, int, int, int, int);
 
 // r_hi = largest r <= L/2 with Jq[r] >= 2^16 (0 if none).
 // minb = 1: up to 168 registers per thread (fastest block sums); minb = 2: 80 registers, twice the CTAs per SM.
-inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb) {
+// wide4: a window wider than 96 sites may take four near quads per thread (else: both halves everywhere).
+inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb, bool wide4 = true) {
 #ifdef PT_ONLY_HEADLINE   // development builds: only the configs[3] instantiation (fast to compile)
     return d.far ? sweep_direct_kernel<1, true, false, 1, true> : sweep_direct_kernel<1, true, false, 1>;
 #else
     const bool l4096 = d.L == 4096;
-    const int nq = direct_nearq(d.L, r_hi);
+    int nq = direct_nearq(d.L, r_hi);
+    if (nq && direct_near_off(r_hi) > 96) {   // the wide windows: their own instantiations
+        const bool big = d.L > 64 * (DIRECT_MAX_BULK / 4);
+        if (big && nq == 1)
+            return d.q <= 8 ? sweep_direct_kernel<1, false, false, 3, false, true> : sweep_direct_kernel<1, false, true, 3, false, true>;
+        if (!big && minb == 1 && nq == 2)
+            return d.q <= 8 ? sweep_direct_kernel<2, false, false, 1, false, true> : sweep_direct_kernel<2, false, true, 1, false, true>;
+        if (!big && minb == 1 && nq == 4 && wide4)
+            return d.q <= 8 ? sweep_direct_kernel<4, false, false, 1, false, true> : sweep_direct_kernel<4, false, true, 1, false, true>;
+        if (!big && minb == 4 && nq == 4 && wide4)
+            return d.q <= 8 ? sweep_direct_kernel<4, false, false, 4, false, true> : sweep_direct_kernel<4, false, true, 4, false, true>;
+        nq = 0;   // no instantiation for this combination: both halves everywhere
+    }
     if (d.L > 64 * (DIRECT_MAX_BULK / 4)) {   // more than 64 j-ranges: every near quad has a thread of its own
         if (d.q <= 8) return nq == 1 ? sweep_direct_kernel<1, false, false, 3> : sweep_direct_kernel<0, false, false, 3>;
         return nq == 1 ? sweep_direct_kernel<1, false, true, 3> : sweep_direct_kernel<0, false, true, 3>;
@@ -1112,6 +1133,15 @@ inline direct_kernel_t select_direct_kernel(const Dev& d, int r_hi, int device, 
     const int R = d.n_ens * d.n_rep;
     int n_sm = 0;
     if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) n_sm = 0;
+    // One wave: a block's time is the latency of the bulk -> chain hand-off, not the instruction count.  Four near
+    // quads per thread for a window of 160 or 224 sites (sigma around 0.2 at L <= 3008) lengthen the tail of every
+    // block and the set-up of every launch: measured equal to both halves everywhere for a lone context (0.0722
+    // against 0.0730 ms at L = 2048, q = 5, sigma = 0.2, 32 replicas) and 2 % slower on configs[4]; with several
+    // waves (two CTAs per SM, issue-bound) 13 % faster (0.178 against 0.204 ms at L = 2048, sigma = 0.2, 400 replicas).
+    if (R <= c1) {
+        k1 = direct_kernel_variant(d, r_hi, 1, false);
+        c1 = direct_coresident(k1, d, device);   // (also sets the kernel's shared-memory attribute)
+    }
     if (force1 || c1 <= 0) {
     } else if (force2) {
         k1 = direct_kernel_variant(d, r_hi, 2);

@@ -196,6 +196,33 @@ def test_ragged_and_edge_shapes(pt, oracle):
         assert_same_state(g, o, "shape L=%d q=%d" % (L, q))
 
 
+@pytest.mark.parametrize("L,q,sigma,n_rep,minb", [
+    (2048, 3, 0.1, 4, None), (2048, 9, 0.2, 3, None), (2048, 9, 0.2, 3, "4"), (2048, 5, 0.2, 150, None),
+    (4096, 8, 0.2, 3, None), (4096, 8, 0.1, 3, None), (4096, 5, 0.04, 2, None), (1024, 7, 0.15, 4, None),
+    (512, 3, 0.05, 3, None), (384, 4, 0.12, 3, None), (6144, 3, 0.12, 2, None), (8192, 6, 0.2, 2, None),
+    (1536, 12, 0.21, 3, None), (1536, 12, 0.21, 3, "4"), (1536, 4, 0.21, 3, "2"), (320, 3, 0.1, 3, None)])
+def test_wide_near_window_for_small_sigma(pt, oracle, monkeypatch, L, q, sigma, n_rep, minb):
+    """The couplings' high 16-bit halves reach r_hi = 101 (sigma = 0.2), 154 (0.1), 205 (0.04): the bulk warps sum the
+    low halves everywhere and the high halves inside a window of 96, 160 or 224 sites around the block
+    (direct_near_off), both halves everywhere only where the ring is too short for the window (L = 320; a smaller
+    sigma than 0.035 the direct variant refuses anyway: sum_r Jq[r] >= 2^30).  Every window, with one to four near
+    quads per thread, q <= 8 and q > 8, against the oracle: bit-identical.  Four near quads per thread in a wide
+    window are taken only by contexts of more than one wave (here: forced through PT_MINB, and 150 replicas)."""
+    if minb:
+        monkeypatch.setenv("PT_MINB", minb)
+    else:
+        monkeypatch.delenv("PT_MINB", raising=False)
+    b = inputs.geometric_betas(0.8, 6.0, n_rep)     # small sigma: transitions at higher temperatures
+    g = pt.PT(L, q, sigma, 1, n_rep, b, 977, variant="direct")
+    o = oracle.Oracle(L, q, sigma, 1, n_rep, b, 977)
+    assert_same_state(g, o, "sigma=%g start" % sigma)
+    for k, every in ((1, 1), (5, 1), (3, 2)):
+        g.sweeps(k, every)
+        o.sweeps(k, every, field=True, threads=THREADS)
+        assert_same_state(g, o, "L=%d q=%d sigma=%g after +%d" % (L, q, sigma, k))
+    g.close()
+
+
 @pytest.mark.parametrize("L,q,sigma,n_rep,force", [
     (256, 3, 0.4, 5, "2"), (256, 3, 0.4, 5, "4"), (512, 5, 0.8, 4, "8"), (448, 20, 0.5, 3, "4"), (1184, 7, 0.3, 3, "2"),
     (8192, 8, 0.3, 3, None),      # 256 KB of local fields: does not fit in one SM, cluster of 2
