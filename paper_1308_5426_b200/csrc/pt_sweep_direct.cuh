@@ -30,8 +30,8 @@
 // non-zero only for r <= r_hi (71 at L=4096, sigma=0.3): with NEARQ != 0 the
 // main loop sums the low halves only (0.5 IDP.2A per pair term) and each thread
 // adds the high halves of NEARQ of the quads of sites within distance off - 1
-// of the block (NEAR; off = 96, 160 or 224, the smallest above r_hi: 56, 88 or
-// 120 quads); NEARQ = 0 keeps both halves everywhere (rings shorter than 2 off + 64).
+// of the block (NEAR; off = 96, 160, .., 352, the smallest above r_hi: 56, 88, ..,
+// 184 quads); NEARQ = 0 keeps both halves everywhere (rings shorter than 2 off + 64).
 // Block sums: a transpose-shuffle reduction leaves one site's partial sum per
 // lane, then one shared-memory atomic per lane; every bulk warp then arrives on
 // full[k&1].  Before block k a bulk warp waits on
@@ -87,11 +87,13 @@ constexpr int DIRECT_BIG_THREADS = DIRECT_BIG_BULK + 32 * DIRECT_CHAIN_WARPS;
 constexpr int DIRECT_STATIC_SMEM = 14 * 1024;   // upper bound of the sweep kernel's static shared memory (13568 B)
 constexpr int DIRECT_NPAIR = 39;   // packed coupling pairs per thread and half: 64 + 2*7 couplings
 constexpr int ENERGY_MAX_THREADS = 512, ENERGY_NPAIR = 35;   // energy_direct_kernel: 4 sites x 64 j per thread
-// NEAR covers |i-j| < off, off = 96, 160 or 224 (the smallest that is > r_hi): the off/2 + 8 quads of sites from off
-// sites before the block to off sites behind it (56 quads for off = 96: sigma >= 0.22 at scale 2^24; 88 for sigma >=
-// 0.1; 120 for sigma >= 0.03, below which sum_r Jq[r] >= 2^30 rules the direct variant out anyway).  0: r_hi is beyond
-// every window.
-__host__ __device__ inline int direct_near_off(int r_hi) { return r_hi < 96 ? 96 : r_hi < 160 ? 160 : r_hi < 224 ? 224 : 0; }
+// NEAR covers |i-j| < off, off = 96, 160, .., 352 (the smallest that is > r_hi): the off/2 + 8 quads of sites from
+// off sites before the block to off sites behind it (56 quads for off = 96: r_hi = 71 at L = 4096, sigma = 0.3; 88
+// for 160: sigma = 0.2; 184 for 352: r_hi = 337 at L = 4096, sigma = 0.1 -- the periodic images add to every coupling,
+// so r_hi grows as the ring shrinks).  0: r_hi is beyond every window.
+__host__ __device__ inline int direct_near_off(int r_hi) {
+    return r_hi < 96 ? 96 : r_hi < 160 ? 160 : r_hi < 224 ? 224 : r_hi < 288 ? 288 : r_hi < 352 ? 352 : 0;
+}
 constexpr int DIRECT_MAX_PERSIST_REP = 512;   // replicas per ensemble in a persistent launch (static shared arrays)
 
 __host__ __device__ inline size_t direct_smem_bytes(int L, int q);
@@ -385,7 +387,7 @@ __device__ __forceinline__ void recount_block(const uint32_t* sp, uint2* cnt8, i
 // so that several hundred small replicas can be co-resident for persistent launches); 3 stands for the L > 4096
 // build: one CTA of up to DIRECT_BIG_THREADS threads per SM, 80 registers.
 // MINB = 4 stands for the L <= 2048 build: CTAs of at most DIRECT_MID_THREADS threads, two per SM, 128 registers.
-// WIDE: the near window is direct_near_off(r_hi) = 160 or 224 sites (a run-time value); else 96 (compile-time: the
+// WIDE: the near window is direct_near_off(r_hi) = 160 .. 352 sites (a run-time value); else 96 (compile-time: the
 // schedule of the headline instantiation is sensitive to every instruction).
 template <int NEARQ, bool NJR64, bool Q16, int MINB, bool FAR = false, bool WIDE = false>
 __global__ void __launch_bounds__(MINB == 3 ? DIRECT_BIG_THREADS : MINB == 4 ? DIRECT_MID_THREADS : DIRECT_MAX_THREADS,
@@ -531,7 +533,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         }
         // NEAR: high halves of quad n = jr + NJR*iq (sites i0 - NOFF + 4n + {0..3}) for this thread's 8 sites:
         // NP[iq][mm][0] = hi(|r|) | hi(|r-1|) << 16, [1] = hi(|r-2|) | hi(|r-3|) << 16, r = gbase + 2mm + NOFF - 4n,
-        // hi(x) = Jq[x] >> 16 for 1 <= x <= r_hi, else 0.  NOFF = 96, 160 or 224 sites (direct_near_off), NQD quads.
+        // hi(x) = Jq[x] >> 16 for 1 <= x <= r_hi, else 0.  NOFF = 96 .. 352 sites (direct_near_off), NQD quads.
         const int NOFF = (NEARQ && WIDE) ? direct_near_off(r_hi) : 96, NQD = NOFF / 2 + 8;
         uint32_t NP[NQ][DIRECT_SITES][2];
         if (NEARQ) {
@@ -1050,6 +1052,8 @@ inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb, b
         const bool big = d.L > 64 * (DIRECT_MAX_BULK / 4);
         if (big && nq == 1)
             return d.q <= 8 ? sweep_direct_kernel<1, false, false, 3, false, true> : sweep_direct_kernel<1, false, true, 3, false, true>;
+        if (big && nq == 2)
+            return d.q <= 8 ? sweep_direct_kernel<2, false, false, 3, false, true> : sweep_direct_kernel<2, false, true, 3, false, true>;
         if (!big && minb == 1 && nq == 2)
             return d.q <= 8 ? sweep_direct_kernel<2, false, false, 1, false, true> : sweep_direct_kernel<2, false, true, 1, false, true>;
         if (!big && minb == 1 && nq == 4 && wide4)
@@ -1133,12 +1137,12 @@ inline direct_kernel_t select_direct_kernel(const Dev& d, int r_hi, int device, 
     const int R = d.n_ens * d.n_rep;
     int n_sm = 0;
     if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) n_sm = 0;
-    // One wave: a block's time is the latency of the bulk -> chain hand-off, not the instruction count.  Four near
-    // quads per thread for a window of 160 or 224 sites (sigma around 0.2 at L <= 3008) lengthen the tail of every
+    // One wave at L <= 2048 (one bulk warp per sub-partition): a block's time is the latency of the bulk -> chain
+    // hand-off, not the instruction count.  Four near quads per thread for a wide window lengthen the tail of every
     // block and the set-up of every launch: measured equal to both halves everywhere for a lone context (0.0722
     // against 0.0730 ms at L = 2048, q = 5, sigma = 0.2, 32 replicas) and 2 % slower on configs[4]; with several
     // waves (two CTAs per SM, issue-bound) 13 % faster (0.178 against 0.204 ms at L = 2048, sigma = 0.2, 400 replicas).
-    if (R <= c1) {
+    if (R <= c1 && d.L <= 2048) {
         k1 = direct_kernel_variant(d, r_hi, 1, false);
         c1 = direct_coresident(k1, d, device);   // (also sets the kernel's shared-memory attribute)
     }

@@ -200,10 +200,11 @@ def test_ragged_and_edge_shapes(pt, oracle):
     (2048, 3, 0.1, 4, None), (2048, 9, 0.2, 3, None), (2048, 9, 0.2, 3, "4"), (2048, 5, 0.2, 150, None),
     (4096, 8, 0.2, 3, None), (4096, 8, 0.1, 3, None), (4096, 5, 0.04, 2, None), (1024, 7, 0.15, 4, None),
     (512, 3, 0.05, 3, None), (384, 4, 0.12, 3, None), (6144, 3, 0.12, 2, None), (8192, 6, 0.2, 2, None),
-    (1536, 12, 0.21, 3, None), (1536, 12, 0.21, 3, "4"), (1536, 4, 0.21, 3, "2"), (320, 3, 0.1, 3, None)])
+    (1536, 12, 0.21, 3, None), (1536, 12, 0.21, 3, "4"), (1536, 4, 0.21, 3, "2"), (320, 3, 0.1, 3, None),
+    (4096, 8, 0.1, 150, None), (6144, 5, 0.1, 2, None), (6144, 11, 0.1, 2, None), (2048, 3, 0.15, 3, "4")])
 def test_wide_near_window_for_small_sigma(pt, oracle, monkeypatch, L, q, sigma, n_rep, minb):
-    """The couplings' high 16-bit halves reach r_hi = 101 (sigma = 0.2), 154 (0.1), 205 (0.04): the bulk warps sum the
-    low halves everywhere and the high halves inside a window of 96, 160 or 224 sites around the block
+    """The couplings' high 16-bit halves reach r_hi = 114 (L = 4096, sigma = 0.2), 234 (6144, 0.1), 337 (4096, 0.1): the
+    bulk warps sum the low halves everywhere and the high halves inside a window of 96, 160, .., 352 sites around the block
     (direct_near_off), both halves everywhere only where the ring is too short for the window (L = 320; a smaller
     sigma than 0.035 the direct variant refuses anyway: sum_r Jq[r] >= 2^30).  Every window, with one to four near
     quads per thread, q <= 8 and q > 8, against the oracle: bit-identical.  Four near quads per thread in a wide
