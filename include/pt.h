@@ -74,6 +74,7 @@ typedef enum {
  * PT_MINB=1|2|4 forces the 168-, the 80- or (1024 < L <= 2048) the 128-register build of the direct sweep kernel
  * (experiments; default: by size and replica count).  PT_FIELD_CLUSTER=2|4|8 runs the field variant on clusters of
  * that size also where one CTA would hold the replica (tests, measurements).
+ * PT_CW=2 (L = 4096, q <= 8): two chain warps instead of four (bit-identical, measured slower: an experiment).
  * PT_FAR=1 (L = 4096, q <= 8) selects the far form of the bulk sum (8-bit coupling residuals beyond 1000 sites;
  * bit-identical results, measured slower than the default form: an experiment kept for reference). */
 enum { PT_VARIANT_AUTO = 0, PT_VARIANT_FIELD = 1, PT_VARIANT_DIRECT = 2, PT_VARIANT_FP32 = 3, PT_VARIANT_FP64 = 4 };

@@ -113,7 +113,7 @@ __host__ __device__ inline int energy_threads(int L) {
     const int t = 8 * (L / 64);
     return t < 32 ? 32 : (t + 31) / 32 * 32;
 }
-__host__ __device__ inline int direct_threads(int L) { return direct_bulk_threads(L) + 32 * DIRECT_CHAIN_WARPS; }
+__host__ __device__ inline int direct_threads(int L, int cw = DIRECT_CHAIN_WARPS) { return direct_bulk_threads(L) + 32 * cw; }
 // Near quads per bulk thread (template parameter NEARQ): 0 = the bulk warps sum both halves everywhere.
 __host__ __device__ inline int direct_nearq(int L, int r_hi) {
     const int njr = L / 64, off = direct_near_off(r_hi);
@@ -389,8 +389,16 @@ __device__ __forceinline__ void recount_block(const uint32_t* sp, uint2* cnt8, i
 // MINB = 4 stands for the L <= 2048 build: CTAs of at most DIRECT_MID_THREADS threads, two per SM, 128 registers.
 // WIDE: the near window is direct_near_off(r_hi) = 160 .. 352 sites (a run-time value); else 96 (compile-time: the
 // schedule of the headline instantiation is sensitive to every instruction).
-template <int NEARQ, bool NJR64, bool Q16, int MINB, bool FAR = false, bool WIDE = false>
-__global__ void __launch_bounds__(MINB == 3 ? DIRECT_BIG_THREADS : MINB == 4 ? DIRECT_MID_THREADS : DIRECT_MAX_THREADS,
+// CW: chain warps (4: one per SM sub-partition, 8 correction rows each; 2: 16 rows each -- 25 % fewer chain
+// instructions per block but longer fixed-point rounds).  Measured (profiles/r2_f_two_ctas_per_sm.md): two chain
+// warps are slower wherever tried -- configs[3] 0.1667 against 0.1419 ms per sweep, configs[4] 0.71 against 0.54 with
+// two 192-thread CTAs per SM at 168 registers, L = 2048 x 296..1200 replicas +0.5..+7 % -- the chain's serial latency,
+// not its instruction count, is what a block waits for.  Kept as an opt-in experiment of the headline instantiation
+// (PT_CW=2, bit-identical results).
+template <int NEARQ, bool NJR64, bool Q16, int MINB, bool FAR = false, bool WIDE = false, int CW = DIRECT_CHAIN_WARPS>
+__global__ void __launch_bounds__(MINB == 3 ? DIRECT_BIG_THREADS
+                                  : MINB == 4 ? DIRECT_MID_THREADS - 32 * (DIRECT_CHAIN_WARPS - CW)
+                                              : DIRECT_MAX_THREADS - 32 * (DIRECT_CHAIN_WARPS - CW),
                                   MINB == 3 ? 1 : MINB == 4 ? 2 : MINB)
 sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int swap_every, int r_hi) {
     // swap_mode 0: no swap event; 1: one event at the end of the launch (last-arriving CTA, nobody waits);
@@ -401,7 +409,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
     constexpr int NQ = NEARQ ? NEARQ : 1;
     extern __shared__ uint32_t smem_d[];
     const int L = d.L, W = d.W, q = d.q;
-    const int NT = blockDim.x, NTB = NT - 32 * DIRECT_CHAIN_WARPS;
+    const int NT = blockDim.x, NTB = NT - 32 * CW;
     const int NB = L >> 5;
     DirectSmem m;
     m.theta = (int32_t*)smem_d;
@@ -756,10 +764,11 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
         // CORR: this warp's correction rows for lane = site l.  If site f of the previous block (rows f = 8cw+j)
         // or of the own block (rows 32 + 8cw + j) accepts a_f -> b_f, dE_l changes by
         //   Jq[dist] (s'_l(b_f) - s'_l(a_f)),   dist = l + 32 - f  resp.  l - f  (nothing for dist <= 0).
-        int Jp[8], Jo[8];
+        constexpr int ROWS = 32 / CW, RG = ROWS / 4;   // correction rows per chain warp, in groups of four
+        int Jp[ROWS], Jo[ROWS];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const int dp = lane + 32 - (8 * cw + j), dn = lane - (8 * cw + j);
+        for (int j = 0; j < ROWS; ++j) {
+            const int dp = lane + 32 - (ROWS * cw + j), dn = lane - (ROWS * cw + j);
             Jp[j] = __ldg(d.Jq + dp);               // 1 <= dp <= 63 < L
             Jo[j] = dn > 0 ? __ldg(d.Jq + dn) : 0;
         }
@@ -792,28 +801,42 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 const uint32_t w_old = m.sp[wsp], w_new = m.bq[wsp];
                 const uint2 tab = m.lut[i0 + lane];
                 const uint2 tabb = Q16 ? m.lutb[i0 + lane] : make_uint2(0u, 0u);
-                int ipv = i0 - 32 + 8 * cw;
+                int ipv = i0 - 32 + ROWS * cw;
                 ipv += ipv < 0 ? L : 0;
-                const uint2 sfp = *reinterpret_cast<const uint2*>(m.selb + ipv);            // a | b << 4 of 8 sites
-                const uint2 sfo = *reinterpret_cast<const uint2*>(m.selb + i0 + 8 * cw);
-                int cp[8], co[8];
+                uint32_t sfp[RG], sfo[RG];                                                   // a | b << 4 of ROWS sites
+                if (CW == 4) {
+                    const uint2 vp = *reinterpret_cast<const uint2*>(m.selb + ipv);
+                    const uint2 vo = *reinterpret_cast<const uint2*>(m.selb + i0 + ROWS * cw);
+                    sfp[0] = vp.x; sfp[1] = vp.y; sfo[0] = vo.x; sfo[1] = vo.y;
+                } else {
+                    const uint4 vp = *reinterpret_cast<const uint4*>(m.selb + ipv);
+                    const uint4 vo = *reinterpret_cast<const uint4*>(m.selb + i0 + ROWS * cw);
+                    sfp[0] = vp.x; sfp[1] = vp.y; sfp[RG - 2] = vp.z; sfp[RG - 1] = vp.w;
+                    sfo[0] = vo.x; sfo[1] = vo.y; sfo[RG - 2] = vo.z; sfo[RG - 1] = vo.w;
+                }
+                int cp[ROWS], co[ROWS];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const uint32_t wp = j < 4 ? sfp.x : sfp.y, wo = j < 4 ? sfo.x : sfo.y;
+                for (int j = 0; j < ROWS; ++j) {
+                    const uint32_t wp = sfp[j >> 2], wo = sfo[j >> 2];
                     // selector byte j: nibble 0 = a_f, nibble 1 = b_f (the two higher nibbles pick bytes that the
                     // dot product weights with 0); byte 0 of the result = s'_l(a_f), byte 1 = s'_l(b_f)
                     const uint32_t sp_ = wp >> (8 * (j & 3)), so_ = wo >> (8 * (j & 3));
                     cp[j] = Jp[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, sp_, sp_ ^ 0x8888u), 0);
                     co[j] = Jo[j] * dp4a_s32_u32(0x000001ff, tab_lookup<Q16>(tab, tabb, so_, so_ ^ 0x8888u), 0);
                 }
-                const int4 cp0 = make_int4(cp[0], cp[1], cp[2], cp[3]), cp1 = make_int4(cp[4], cp[5], cp[6], cp[7]);
-                const int4 co0 = make_int4(co[0], co[1], co[2], co[3]), co1 = make_int4(co[4], co[5], co[6], co[7]);
+                int4 cpv[RG], cov[RG];
+#pragma unroll
+                for (int gq = 0; gq < RG; ++gq) {
+                    cpv[gq] = make_int4(cp[4 * gq], cp[4 * gq + 1], cp[4 * gq + 2], cp[4 * gq + 3]);
+                    cov[gq] = make_int4(co[4 * gq], co[4 * gq + 1], co[4 * gq + 2], co[4 * gq + 3]);
+                }
                 // changes accepted in block k-1, which the bulk sum saw as it was before: this warp's rows, known
                 // before the wait; they ride along with the first round below (one exchange less per block)
                 int pc = 0;
                 if (mp) {
-                    const unsigned mv = (mp >> (8 * cw)) ^ lz;
-                    pc = masked_add4(masked_add4(0, mv, 0, cp0), mv, 4, cp1);
+                    const unsigned mv = (mp >> (ROWS * cw)) ^ lz;
+#pragma unroll
+                    for (int gq = 0; gq < RG; ++gq) pc = masked_add4(pc, mv, 4 * gq, cpv[gq]);
                 }
                 mbar_wait(&s_full[k & 1], (uint32_t)(phase0 + (k >> 1)) & 1u);
                 PT_T0(t_c);
@@ -831,13 +854,20 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 int yy = y;
                 if (mask | mp) {   // nothing accepted here or in block k-1: nothing to correct
                     for (int it = 0; it < 33; ++it) {
-                        const unsigned mv = (mask >> (8 * cw)) ^ lz;
-                        const int part = masked_add4(masked_add4(pc, mv, 0, co0), mv, 4, co1);
+                        const unsigned mv = (mask >> (ROWS * cw)) ^ lz;
+                        int part = pc;
+#pragma unroll
+                        for (int gq = 0; gq < RG; ++gq) part = masked_add4(part, mv, 4 * gq, cov[gq]);
                         s_xch[xb][lane][cw] = part;
-                        asm volatile("bar.sync 1, 128;" ::: "memory");
-                        const int4 pv = *reinterpret_cast<const int4*>(&s_xch[xb][lane][0]);
+                        asm volatile("bar.sync 1, %0;" ::"n"(32 * CW) : "memory");
+                        if (CW == 4) {
+                            const int4 pv = *reinterpret_cast<const int4*>(&s_xch[xb][lane][0]);
+                            yy = y - ((pv.x + pv.y) + (pv.z + pv.w));
+                        } else {
+                            const int2 pv = *reinterpret_cast<const int2*>(&s_xch[xb][lane][0]);
+                            yy = y - (pv.x + pv.y);
+                        }
                         xb ^= 1;
-                        yy = y - ((pv.x + pv.y) + (pv.z + pv.w));
                         const unsigned m2 = __ballot_sync(0xffffffffu, yy >= 0);
 #ifdef PT_TIMING
                         tacc[5] += 1;
@@ -854,12 +884,16 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 {
                     unsigned seq = 0u;
                     for (int l = 0; l < 32; ++l) {
-                        const unsigned mv = (seq >> (8 * cw)) ^ lz;
-                        s_xch[xb][lane][cw] = masked_add4(masked_add4(pc, mv, 0, co0), mv, 4, co1);
-                        asm volatile("bar.sync 1, 128;" ::: "memory");
-                        const int4 pv = *reinterpret_cast<const int4*>(&s_xch[xb][lane][0]);
+                        const unsigned mv = (seq >> (ROWS * cw)) ^ lz;
+                        int part = pc;
+#pragma unroll
+                        for (int gq = 0; gq < RG; ++gq) part = masked_add4(part, mv, 4 * gq, cov[gq]);
+                        s_xch[xb][lane][cw] = part;
+                        asm volatile("bar.sync 1, %0;" ::"n"(32 * CW) : "memory");
+                        int ys = y;
+#pragma unroll
+                        for (int c2 = 0; c2 < CW; ++c2) ys -= s_xch[xb][lane][c2];
                         xb ^= 1;
-                        const int ys = y - ((pv.x + pv.y) + (pv.z + pv.w));
                         seq |= (unsigned)__shfl_sync(0xffffffffu, ys >= 0 ? 1 : 0, l) << l;   // site l, all before it decided
                     }
                     if (seq != mask && lane == 0) *(volatile int*)d.err = 2;
@@ -871,7 +905,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
                 }
                 // every chain warp has read the block sums of buffer k&1 (without rounds there is no other barrier
                 // between a slow warp's read and this point) before they are cleared and the buffer is handed back
-                asm volatile("bar.sync 1, 128;" ::: "memory");
+                asm volatile("bar.sync 1, %0;" ::"n"(32 * CW) : "memory");
                 if (cw == 0) {
                     m.part[(k & 1) * 32 + lane] = 0u;
                     __syncwarp();
@@ -1076,8 +1110,11 @@ inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb, b
     if (d.q <= 8) {
         if (minb == 1) {
             switch (nq) {
-                case 1: return l4096 ? (d.far ? sweep_direct_kernel<1, true, false, 1, true> : sweep_direct_kernel<1, true, false, 1>)
-                                     : sweep_direct_kernel<1, false, false, 1>;
+                case 1:
+                    if (l4096 && !d.far && getenv("PT_CW") && getenv("PT_CW")[0] == '2')   // experiment: two chain warps
+                        return sweep_direct_kernel<1, true, false, 1, false, false, 2>;
+                    return l4096 ? (d.far ? sweep_direct_kernel<1, true, false, 1, true> : sweep_direct_kernel<1, true, false, 1>)
+                                 : sweep_direct_kernel<1, false, false, 1>;
                 case 2: return sweep_direct_kernel<2, false, false, 1>;
                 case 4: return sweep_direct_kernel<4, false, false, 1>;
                 default: return l4096 ? sweep_direct_kernel<0, true, false, 1> : sweep_direct_kernel<0, false, false, 1>;
@@ -1097,12 +1134,20 @@ inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb, b
 #endif
 }
 
+// Chain warps of a kernel variant (its block size is direct_threads(L, cw)).
+inline int direct_chain_warps_of(direct_kernel_t k) {
+    const direct_kernel_t two[] = {sweep_direct_kernel<1, true, false, 1, false, false, 2>};
+    for (direct_kernel_t t : two)
+        if (k == t) return 2;
+    return DIRECT_CHAIN_WARPS;
+}
+
 // CTAs of a sweep kernel variant that can be resident on the device at once (0 on error).
 inline int direct_coresident(direct_kernel_t kern, const Dev& d, int device) {
     const size_t smem = direct_smem_bytes(d.L, d.q);
     if (allow_max_dynamic_smem((const void*)kern, DIRECT_STATIC_SMEM) != 0) return 0;
     int per_sm = 0, n_sm = 0, coop = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, direct_threads(d.L), smem) != cudaSuccess) return 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, direct_threads(d.L, direct_chain_warps_of(kern)), smem) != cudaSuccess) return 0;
     if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return 0;
     if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device) != cudaSuccess || !coop) return 0;
     return per_sm * n_sm;
@@ -1196,7 +1241,7 @@ inline int launch_sweep_direct(direct_kernel_t kern, const Dev& d, long long swe
     cudaError_t err = cudaSuccess;   // (the shared-memory attribute was set once, in direct_coresident)
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)(swap_mode == 3 ? d.n_local : d.n_ens * d.n_rep));
-    cfg.blockDim = dim3((unsigned)direct_threads(d.L));
+    cfg.blockDim = dim3((unsigned)direct_threads(d.L, direct_chain_warps_of(kern)));
     cfg.dynamicSmemBytes = smem;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];

@@ -312,10 +312,21 @@ def test_more_than_16_colours(pt, oracle, L, q, sigma, n_ens, n_rep):
         h.close()
 
 
-def test_field_table_capacity_beyond_16_colours(pt):
-    """L*q*4 bytes of local fields must fit in shared memory: q = 64 at L = 1024 does not (PT_ECAPACITY)."""
+def test_field_table_capacity_beyond_16_colours(pt, oracle):
+    """L*q*4 bytes of local fields must fit in the shared memory of one SM or of a cluster of up to 8: q = 64 at
+    L = 1024 (256 KB) takes a cluster of 2 and equals the oracle; q = 64 at L = 8192 (2 MB) does not fit
+    (PT_ECAPACITY), nor does a ring whose length the cluster sizes do not divide."""
+    g = pt.PT(1024, 64, 0.5, 1, 2, [0.5, 1.0], 1)
+    o = oracle.Oracle(1024, 64, 0.5, 1, 2, [0.5, 1.0], 1)
+    assert g.get_variant() == "field"
+    g.sweeps(6, 2)
+    o.sweeps(6, 2, field=True, threads=THREADS)
+    assert_same_state(g, o, "L=1024 q=64 on a cluster")
+    g.close()
     with pytest.raises(pt.PTError):
-        pt.PT(1024, 64, 0.5, 1, 2, [0.5, 1.0], 1)
+        pt.PT(8192, 64, 0.5, 1, 2, [0.5, 1.0], 1)
+    with pytest.raises(pt.PTError):
+        pt.PT(8 * 1031, 40, 0.5, 1, 2, [0.5, 1.0], 1)     # 1.3 MB of fields, L/8 prime: no cluster size divides it
 
 
 def test_ens_base_shards_ensembles(pt, oracle):
@@ -555,6 +566,18 @@ def test_far_form_of_the_bulk_sum_is_bit_exact(pt, oracle, monkeypatch):
         g.sweeps(n, w.swap_every)
         o.sweeps(n, w.swap_every, field=True, threads=THREADS)
         assert_same_state(g, o, "cfg3, far form, %d more sweeps" % n)
+
+
+def test_two_chain_warps_are_bit_exact(pt, oracle, monkeypatch):
+    """PT_CW=2 (an experiment kept in the tree, slower than four chain warps: profiles/r2_f): two chain warps with 16
+    correction rows each solve the block's accept system.  Integers: the trajectory must not change."""
+    monkeypatch.setenv("PT_CW", "2")
+    w = inputs.config(3)
+    g, o = make_pair(pt, oracle, w, "direct")
+    for n in (1, 2, 17):
+        g.sweeps(n, w.swap_every)
+        o.sweeps(n, w.swap_every, field=True, threads=THREADS)
+        assert_same_state(g, o, "cfg3, two chain warps, %d more sweeps" % n)
 
 
 @pytest.mark.parametrize("L,q,sigma", [(128, 16, 0.6), (256, 9, 0.2), (1024, 12, 0.9), (2048, 9, 0.5)])
