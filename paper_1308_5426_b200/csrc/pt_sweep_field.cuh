@@ -38,6 +38,51 @@ __host__ __device__ inline size_t field_smem_bytes(int L, int q, bool random_ord
     return (size_t)(2 * L + W + (random_order ? L + L / 4 : W) + q * L) * 4;
 }
 
+// a5, field variant: the columns of the old and the new colour after an accepted change at site fs,
+//   ha[j] -= Jq[|j0 + j - fs|],  hb[j] += Jq[|j0 + j - fs|]   for the n sites j0 .. j0 + n - 1 held in ha, hb
+// (distances folded to <= L/2 when FOLD: J then only needs the entries 0..L/2).  Each thread takes the sites
+// tid, tid + T, ..: four at a time, all twelve loads issued before the eight stores (the three arrays do not
+// overlap, a != b; written this way because the compiler must assume that they do and would serialise them).
+template <bool FOLD>
+__device__ __forceinline__ void field_column_update(int32_t* ha, int32_t* hb, const int32_t* J, int n, int j0, int fs,
+                                                    int L, int tid) {
+    constexpr int T = FIELD_THREADS;
+    if (n < 4 * T) {   // short columns: one site at a time
+        for (int j = tid; j < n; j += T) {
+            int dist = j0 + j - fs;
+            dist = dist < 0 ? -dist : dist;
+            if (FOLD) dist = dist > (L >> 1) ? L - dist : dist;
+            const int32_t Jv = J[dist];
+            ha[j] -= Jv;
+            hb[j] += Jv;
+        }
+        return;
+    }
+    for (int jb = tid; jb < n; jb += 4 * T) {
+        int32_t jv[4], av[4], bv[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int j = jb + u * T;
+            if (j < n) {
+                int dist = j0 + j - fs;
+                dist = dist < 0 ? -dist : dist;
+                if (FOLD) dist = dist > (L >> 1) ? L - dist : dist;
+                jv[u] = J[dist];   // J[0] = 0: the site's own field is unchanged
+                av[u] = ha[j];
+                bv[u] = hb[j];
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int j = jb + u * T;
+            if (j < n) {
+                ha[j] = av[u] - jv[u];
+                hb[j] = bv[u] + jv[u];
+            }
+        }
+    }
+}
+
 template <bool RANDOM, int BITS>
 __global__ void __launch_bounds__(FIELD_THREADS, 1)
 sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
@@ -132,14 +177,7 @@ sweep_field_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
             const int f = s_flip[0];
             if (f >= L) break;
             const int a = s_flip[1], b = s_flip[2], fs = s_flip[4];   // fs: the site of step f
-            int32_t* ha = h + a * L;
-            int32_t* hb = h + b * L;
-            for (int j = tid; j < L; j += FIELD_THREADS) {
-                const int dist = j > fs ? j - fs : fs - j;
-                const int32_t Jv = J[dist];  // J[0] = 0: the site's own field is unchanged
-                ha[j] -= Jv;
-                hb[j] += Jv;
-            }
+            field_column_update<false>(h + a * L, h + b * L, J, L, 0, fs, L, tid);
             if (tid == 0) {
                 const int sh = (fs % PER) * BITS;
                 sp[fs / PER] = (sp[fs / PER] & ~(CMASK << sh)) | ((uint32_t)b << sh);
@@ -307,16 +345,7 @@ sweep_field_cluster_kernel(Dev d, long long sweep0, int n_sweeps, int do_swap) {
             const int fs = rec.y;
             if (fs >= 0) {
                 const int a = rec.z & 255, b = rec.z >> 8;
-                int32_t* ha = h + a * Ls;
-                int32_t* hb = h + b * Ls;
-                for (int jj = tid; jj < Ls; jj += FIELD_THREADS) {
-                    int dist = lo + jj - fs;
-                    dist = dist < 0 ? -dist : dist;
-                    dist = dist > H ? L - dist : dist;
-                    const int32_t Jv = J[dist];   // J[0] = 0: the site's own field is unchanged
-                    ha[jj] -= Jv;
-                    hb[jj] += Jv;
-                }
+                field_column_update<true>(h + a * Ls, h + b * Ls, J, Ls, lo, fs, L, tid);
                 if (tid == 0) {
                     E += rec.w;
                     oa.acc += 1;
