@@ -241,8 +241,9 @@ def test_local_fields_over_a_thread_block_cluster(pt, oracle, monkeypatch, L, q,
     else:
         monkeypatch.delenv("PT_FIELD_CLUSTER", raising=False)
     b = inputs.geometric_betas(0.6, 2.5, n_rep)
-    g = pt.PT(L, q, sigma, 1, n_rep, b, 4242, variant="field")
-    o = oracle.Oracle(L, q, sigma, 1, n_rep, b, 4242)
+    n_ens = 2 if force else 1          # several ensembles: cluster -> (ensemble, slot) and one swap event per ensemble
+    g = pt.PT(L, q, sigma, n_ens, n_rep, b, 4242, variant="field")
+    o = oracle.Oracle(L, q, sigma, n_ens, n_rep, b, 4242)
     assert g.get_variant() == "field"
     assert_same_state(g, o, "cluster start")
     n_small = 3 if L >= 4096 else 12
