@@ -324,7 +324,7 @@ def run_ours(args):
         line = {"metric": metric_name(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W_,
                 "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": {"fp32": "f32", "fp64": "f64"}.get(variant, "int32"), "data": "synthetic",
-                "config": workload_config(w, variant, world), "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+                "config": dict(workload_config(w, variant, world), launch_plan=g.describe()), "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
                 "flip_acceptance": acc, "pair_evaluations_per_s": value * (w.L - 1)}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline_leg(w)
@@ -429,7 +429,8 @@ def run_cfg4(args):
                                    "40 handles x 32 replicas, T geometric in [0.4,3.0], hot start, swap every sweep, "
                                    "40 CUDA streams", "variant": gs[0].get_variant(),
                        "step": "1 sweep + swap event of all 1280 replicas = %d attempts" % (attempts // K),
-                       "l2": "not flushed: the per-step state (1.3 MB of packed spins) is resident by design"},
+                       "l2": "not flushed: the per-step state (1.3 MB of packed spins) is resident by design",
+                       "launch_plans": {p: n for p, n in sorted(__import__("collections").Counter(g.describe() for g in gs).items())}},
             "clocks": clocks,
             "e2e": {"value": attempts / e2e_s, "unit": UNIT, "h2d_bytes_per_step": sum(s0.nbytes for s0 in starts) / K,
                     "d2h_bytes_per_step": d2h / K,

@@ -220,6 +220,14 @@ int64_t pt_sweep_counter(pt_ctx* ctx);
 int pt_set_variant(pt_ctx* ctx, int variant);
 int pt_get_variant(pt_ctx* ctx); /* the variant that pt_sweeps runs (FIELD or DIRECT) */
 
+/* The launch plan of the context as one line of text (what pt_sweeps would launch now), e.g.
+ *   "direct: threads=384 regs=155 resident_ctas=148 near_window=96 near_quads=1 chain_warps=4 persistent=1"
+ *   "field: cluster=4 threads=512 smem=186400"
+ * out: caller's buffer of n bytes (host), NUL-terminated on return; a longer line is truncated.  Returns PT_OK,
+ * PT_EINVAL (NULL arguments, n < 1) or PT_ECUDA.  For logs, bench lines and tests of the launch policy
+ * (DESIGN.md sections 6.1b, 6.2); nothing of the path depends on it. */
+int pt_describe(pt_ctx* ctx, char* out, int n);
+
 /* Site order of a sweep (reading A5 of DESIGN.md).  PT_ORDER_SEQUENTIAL (default, BASELINE configs): sites 0..L-1
  * in order.  PT_ORDER_RANDOM ("L Metropolis steps ... an average of one Monte Carlo step per
  * spin"): step n = 0..L-1 of a sweep visits site mulhi32(w3, L) of the Philox draw keyed by (n, sweep, slot), which

@@ -748,6 +748,39 @@ int pt_set_variant(pt_ctx* c, int variant) {
 
 int pt_get_variant(pt_ctx* c) { return c ? c->variant : PT_EINVAL; }
 
+int pt_describe(pt_ctx* c, char* out, int n) {
+    if (!c || !out || n < 1) return fail(PT_EINVAL, "ctx or out is NULL, or n < 1");
+    DeviceGuard guard(c->device);
+    char line[256];
+    if (c->variant == PT_VARIANT_DIRECT) {
+        if (!c->direct_kern) c->direct_kern = ptk::select_direct_kernel(c->dev(), c->r_hi, c->device, &c->coresident);
+        cudaFuncAttributes fa;
+        PT_CUDA(cudaFuncGetAttributes(&fa, (const void*)c->direct_kern));
+        const int cw = ptk::direct_chain_warps_of(c->direct_kern);
+        // near quads per thread of the build in use: find the (build, wide) combination that gives this kernel
+        int nq = -1;
+        const ptk::Dev d = c->dev();
+        for (int minb : {1, 4, 2})
+            for (int wide4 = 1; wide4 >= 0 && nq < 0; --wide4)
+                if (c->direct_kern == ptk::direct_kernel_variant(d, c->r_hi, minb, wide4 != 0))
+                    nq = ptk::direct_effective_nearq(d, c->r_hi, minb, wide4 != 0);
+        if (nq < 0) nq = 0;
+        snprintf(line, sizeof line,
+                 "direct: threads=%d regs=%d resident_ctas=%d near_window=%d near_quads=%d chain_warps=%d persistent=%d",
+                 ptk::direct_threads(c->L, cw), fa.numRegs, c->coresident, nq ? ptk::direct_near_off(c->r_hi) : 0, nq, cw,
+                 persistent_ok(c) ? 1 : 0);
+    } else if (c->variant == PT_VARIANT_FIELD) {
+        const int C = field_cluster_of(c);
+        const size_t smem = C ? ptk::field_cluster_smem_bytes(c->L, c->q, C)
+                              : ptk::field_smem_bytes(c->L, c->q, c->site_order == PT_ORDER_RANDOM);
+        snprintf(line, sizeof line, "field: cluster=%d threads=%d smem=%zu", C, ptk::FIELD_THREADS, smem);
+    } else {
+        snprintf(line, sizeof line, "%s: threads=%d", c->variant == PT_VARIANT_FP32 ? "fp32" : "fp64", ptk::FLOAT_THREADS);
+    }
+    snprintf(out, (size_t)n, "%s", line);
+    return PT_OK;
+}
+
 int pt_set_site_order(pt_ctx* c, int order) {
     if (!c) return fail(PT_EINVAL, "ctx is NULL");
     if (order != PT_ORDER_SEQUENTIAL && order != PT_ORDER_RANDOM) return fail(PT_EINVAL, "unknown site order");

@@ -1134,6 +1134,23 @@ inline direct_kernel_t direct_kernel_variant(const Dev& d, int r_hi, int minb, b
 #endif
 }
 
+// Near quads per thread of the instantiation direct_kernel_variant(d, r_hi, minb, wide4) returns (0: both halves
+// everywhere): not every (window, quads, build) combination has an instantiation.  For pt_describe.
+inline int direct_effective_nearq(const Dev& d, int r_hi, int minb, bool wide4) {
+    const int nq = direct_nearq(d.L, r_hi);
+    const bool big = d.L > 64 * (DIRECT_MAX_BULK / 4);
+    if (nq && direct_near_off(r_hi) > 96) {
+        if (big) return nq <= 2 ? nq : 0;
+        if (minb == 1) return nq == 2 || (nq == 4 && wide4) ? nq : 0;
+        if (minb == 4) return nq == 4 && wide4 ? nq : 0;
+        return 0;
+    }
+    if (big) return nq == 1 ? 1 : 0;
+    if (minb == 4) return nq == 2 || nq == 4 ? nq : 0;
+    if (minb == 1) return nq == 1 || nq == 2 || nq == 4 ? nq : 0;
+    return nq == 4 ? 4 : 0;
+}
+
 // Chain warps of a kernel variant (its block size is direct_threads(L, cw)).
 inline int direct_chain_warps_of(direct_kernel_t k) {
     const direct_kernel_t two[] = {sweep_direct_kernel<1, true, false, 1, false, false, 2>};
@@ -1215,7 +1232,7 @@ inline direct_kernel_t select_direct_kernel(const Dev& d, int r_hi, int device, 
             }
             k1 = kb;
             c1 = cb;
-        } else if (3 * R < n_sm && d.q <= 8 && nq == 2) {
+        } else if (3 * R < n_sm && d.q <= 8 && nq == 2) {   // (q > 8 at 128 registers: 22 % slower alone, 2 % slower on configs[4])
             direct_kernel_t k4 = direct_kernel_variant(d, r_hi, 4);
             const int c4 = direct_coresident(k4, d, device);
             if (c4 > c1) { k1 = k4; c1 = c4; }

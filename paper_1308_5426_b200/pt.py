@@ -25,7 +25,7 @@ SYMBOLS = ["pt_create", "pt_create_ex", "pt_destroy", "pt_sweeps", "pt_energy", 
            "pt_sweep_counter", "pt_set_variant", "pt_get_variant", "pt_set_stream", "pt_sweeps_async",
            "pt_sync", "pt_last_error", "pt_create_shard", "pt_energy_storage_dev", "pt_swap_external",
            "pt_get_perm", "pt_measure_peaks", "pt_get_state", "pt_set_state", "pt_set_site_order",
-           "pt_energy_storage_dev_async", "pt_swap_external_async", "pt_energy_static"]
+           "pt_energy_storage_dev_async", "pt_swap_external_async", "pt_energy_static", "pt_describe"]
 
 
 class PTError(RuntimeError):
@@ -75,6 +75,7 @@ _lib.pt_sweep_counter.argtypes = [_vp]
 _lib.pt_sweep_counter.restype = _i64
 _lib.pt_set_variant.argtypes = [_vp, _i32]
 _lib.pt_get_variant.argtypes = [_vp]
+_lib.pt_describe.argtypes = [_vp, ctypes.c_char_p, ctypes.c_int]
 _lib.pt_set_stream.argtypes = [_vp, _vp]
 _lib.pt_last_error.restype = ctypes.c_char_p
 _lib.pt_measure_peaks.argtypes = [_vp, _i32]
@@ -269,6 +270,12 @@ class PT:
     def get_variant(self):
         v = _lib.pt_get_variant(self._h)
         return {VARIANT_FIELD: "field", VARIANT_DIRECT: "direct", VARIANT_FP32: "fp32", VARIANT_FP64: "fp64"}.get(v, str(v))
+
+    def describe(self):
+        """pt_describe: the launch plan of the context as one line of text."""
+        buf = ctypes.create_string_buffer(256)
+        _check(_lib.pt_describe(self._h, buf, 256))
+        return buf.value.decode()
 
     def set_stream(self, cuda_stream_ptr):
         _check(_lib.pt_set_stream(self._h, ctypes.c_void_p(int(cuda_stream_ptr) if cuda_stream_ptr else None)))

@@ -569,6 +569,52 @@ def test_far_form_of_the_bulk_sum_is_bit_exact(pt, oracle, monkeypatch):
         assert_same_state(g, o, "cfg3, far form, %d more sweeps" % n)
 
 
+def test_launch_policy_as_pt_describe_reports_it(pt, monkeypatch):
+    """The builds select_direct_kernel picks and the cluster size of the local-field sweep (6.2),
+    read back through pt_describe: the headline config on one 155..168-register CTA per SM with persistent launches;
+    more than one wave at L = 2048 on two 128-register CTAs per SM; a small context there as well where that is free;
+    wide near windows for small sigma; local fields beyond one SM on a cluster."""
+    for name in ("PT_MINB", "PT_FIELD_CLUSTER", "PT_CW", "PT_FAR", "PT_PERSISTENT", "PT_VARIANT"):
+        monkeypatch.delenv(name, raising=False)
+
+    def plan(L, q, sigma, n_rep, variant="auto"):
+        g = pt.PT(L, q, sigma, 1, n_rep, inputs.geometric_betas(0.6, 2.5, n_rep), 3, variant=variant)
+        txt = g.describe()
+        g.close()
+        head, _, rest = txt.partition(": ")
+        return head, {k: int(v) for k, v in (kv.split("=") for kv in rest.split())}
+
+    v, p = plan(4096, 8, 0.3, 128)
+    assert v == "direct" and p["threads"] == 384 and 150 <= p["regs"] <= 168 and p["resident_ctas"] == 148
+    assert p["near_window"] == 96 and p["near_quads"] == 1 and p["chain_warps"] == 4 and p["persistent"] == 1
+    v, p = plan(2048, 3, 0.5, 400)
+    assert p["threads"] == 256 and p["regs"] <= 128 and p["resident_ctas"] == 296 and p["persistent"] == 0
+    v, p = plan(2048, 3, 0.5, 296)
+    assert p["regs"] <= 128 and p["persistent"] == 1
+    v, p = plan(2048, 3, 0.5, 148)
+    assert p["regs"] > 128 and p["resident_ctas"] == 148
+    v, p = plan(2048, 3, 0.5, 32)
+    assert p["regs"] <= 128 and p["persistent"] == 0          # small context: shares the GPU, two CTAs per SM
+    v, p = plan(2048, 5, 0.2, 32)
+    assert p["regs"] > 128 and p["near_quads"] == 0           # one wave, wide window with 4 quads: both halves
+    v, p = plan(2048, 5, 0.2, 400)
+    assert p["regs"] <= 128 and p["near_window"] == 160 and p["near_quads"] == 4
+    v, p = plan(4096, 8, 0.2, 128)
+    assert p["near_window"] == 160 and p["near_quads"] == 2
+    v, p = plan(6144, 8, 0.1, 16)
+    assert p["threads"] == 512 and p["near_window"] == 288 and p["near_quads"] == 2
+    v, p = plan(1536, 3, 0.5, 400)
+    assert p["regs"] <= 80 and p["resident_ctas"] == 444      # three 80-register CTAs per SM: one wave
+    v, p = plan(1536, 3, 0.5, 1200)
+    assert 80 < p["regs"] <= 128 and p["resident_ctas"] == 296
+    v, p = plan(1000, 3, 0.5, 8)
+    assert v == "field" and p["cluster"] == 0
+    v, p = plan(16384, 6, 0.6, 2)
+    assert v == "field" and p["cluster"] == 4
+    v, p = plan(8192, 8, 0.3, 2, variant="field")
+    assert v == "field" and p["cluster"] == 2 and p["smem"] <= 227 * 1024
+
+
 def test_two_chain_warps_are_bit_exact(pt, oracle, monkeypatch):
     """PT_CW=2 (an experiment kept in the tree, slower than four chain warps: profiles/r2_f): two chain warps with 16
     correction rows each solve the block's accept system.  Integers: the trajectory must not change."""
