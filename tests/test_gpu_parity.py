@@ -767,13 +767,16 @@ def test_more_replicas_than_sms(pt, oracle, policy, monkeypatch):
         g.close()
 
 
-def test_binder_crossing_reproduces_the_papers_critical_temperature(pt):
+@pytest.mark.parametrize("sigma,T_lo,T_hi,Tc,tol", [(0.4, 1.95, 2.25, 2.085, 0.01), (0.2, 3.70, 4.25, 3.955, 0.015),
+                                                    (0.6, 1.30, 1.52, 1.4125, 0.0125)])
+def test_binder_crossing_reproduces_the_papers_critical_temperature(pt, sigma, T_lo, T_hi, Tc, tol):
     """Physics check of the whole path (not parity): the Binder cumulants V_M (Eq. 12) of two sizes cross at the
-    critical temperature; the paper's Table 1 gives T_c = 2.085(5) for q=3, sigma=0.4.  64 replicas on
-    a uniform ladder T in [1.95, 2.25], 2e4 + 6e4 sweeps, swap every sweep, L = 256 and 512 (about 3 s of GPU time)."""
+    critical temperature; the paper's Table 1 gives, for q=3, T_c = 3.955(5) at sigma=0.2, 2.085(5) at 0.4 and
+    1.4125(75) at 0.6.  64 replicas on a uniform ladder around T_c, 2e4 + 6e4 sweeps, swap every
+    sweep, L = 256 and 512 (about 3 s of GPU time per sigma); tolerance = the paper's error bar + 0.005."""
     from paper_1308_5426_b200 import pt_math
-    q, sigma, n_rep = 3, 0.4, 64
-    T = np.linspace(1.95, 2.25, n_rep)
+    q, n_rep = 3, 64
+    T = np.linspace(T_lo, T_hi, n_rep)
     V = {}
     for L in (256, 512):
         g = pt.PT(L, q, sigma, 1, n_rep, 1.0 / T, 1234 + L)
@@ -787,8 +790,8 @@ def test_binder_crossing_reproduces_the_papers_critical_temperature(pt):
     idx = np.where(np.sign(d[:-1]) != np.sign(d[1:]))[0]
     crossings = [T[i] + (T[i + 1] - T[i]) * d[i] / (d[i] - d[i + 1]) for i in idx]
     assert crossings, "the cumulants of L=256 and L=512 do not cross"
-    best = min(crossings, key=lambda x: abs(x - 2.085))
-    assert abs(best - 2.085) < 0.01, crossings
+    best = min(crossings, key=lambda x: abs(x - Tc))
+    assert abs(best - Tc) < tol, crossings
 
 
 @pytest.mark.parametrize("L,sweeps", [(512, 12), (1024, 6), (2048, 3)])
