@@ -46,6 +46,10 @@ class Obs(ctypes.Structure):  # pt_obs
 
 
 OBS_FIELDS = [f[0] for f in Obs._fields_]
+# the same 144-byte record as a numpy structured type (argument marshalling without a Python loop per record)
+OBS_DTYPE = np.dtype([(n, (np.uint64, (4,)) if n == "sum_E4" else
+                      (np.uint64 if n in ("sum_E2_lo", "sum_Nmax4_lo") else np.int64)) for n in OBS_FIELDS])
+assert OBS_DTYPE.itemsize == ctypes.sizeof(Obs)
 
 if not os.path.exists(LIB_PATH):
     raise ImportError("libpt.so is not built (run `python -m paper_1308_5426_b200.build`); "
@@ -207,15 +211,12 @@ class PT:
         return perm
 
     def observables(self):
-        arr = (Obs * (self.n_ens * self.n_rep))()
-        _check(_lib.pt_observables(self._h, ctypes.byref(arr)))
+        rec = np.zeros(self.n_ens * self.n_rep, dtype=OBS_DTYPE)
+        _check(_lib.pt_observables(self._h, _p(rec)))
         out = {}
-        for name in OBS_FIELDS:
-            if name == "sum_E4":   # [n_ens, n_rep, 4] little-endian 64-bit limbs of a 256-bit integer
-                out[name] = np.array([list(o.sum_E4) for o in arr], dtype=np.uint64).reshape(self.n_ens, self.n_rep, 4)
-                continue
-            dt = np.uint64 if name in ("sum_E2_lo", "sum_Nmax4_lo") else np.int64
-            out[name] = np.array([getattr(o, name) for o in arr], dtype=dt).reshape(self.n_ens, self.n_rep)
+        for name in OBS_FIELDS:   # sum_E4: [n_ens, n_rep, 4] little-endian 64-bit limbs of a 256-bit integer
+            shape = (self.n_ens, self.n_rep, 4) if name == "sum_E4" else (self.n_ens, self.n_rep)
+            out[name] = np.ascontiguousarray(rec[name]).reshape(shape)
         return out
 
     def get_spins(self):
