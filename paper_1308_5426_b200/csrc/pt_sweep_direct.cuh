@@ -597,7 +597,21 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             for (int kb = 0; kb < NB; ++kb) {
                 // block kb is summed against: blocks < kb-1 final (the chain warp is done with block kb-2, which
                 // also frees buffer kb&1), block kb-1 as at the start of the sweep, blocks >= kb untouched
+#ifdef PT_TIMING
+                if (kb >= 2) {   // slot 5: try_waits that found the phase incomplete; slot 6 (below): clocks of the wait
+                    PT_T0(t_w);
+                    uint32_t ok = 0u;
+                    do {
+                        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                                     "selp.u32 %0, 1, 0, p;\n\t}"
+                                     : "=r"(ok) : "r"(smem_u32(&s_done[kb & 1])), "r"((uint32_t)(phase0 + (kb >> 1) - 1) & 1u) : "memory");
+                        tacc[5] += ok ? 0 : 1;
+                    } while (!ok);
+                    PT_ACC(7, t_w);
+                }
+#else
                 if (kb >= 2) mbar_wait(&s_done[kb & 1], (uint32_t)(phase0 + (kb >> 1) - 1) & 1u);
+#endif
                 PT_T0(t_b);
                 // FAR: block kb-2 is final: its colour counts (a far range reads them 30 blocks later at the earliest)
                 int rcv = 0;
@@ -740,7 +754,7 @@ sweep_direct_kernel(Dev d, long long sweep0, int n_sweeps, int swap_mode, int sw
             // a8 (the chain warps' owner thread samples the observables; every thread helps counting colours)
             direct_nmax(m.sp, W, q, s_cnt);
             cta_sync();
-            PT_ACC(7, t_nm);
+            PT_ACC(6, t_nm);   // (slot 6: the closing barrier and the colour count; slot 7 is the done wait)
             if (swap_mode == 2 && (sweep0 + s + 1) % swap_every == 0) {
                 t = direct_swap_in_kernel(d, ps, e, (uint32_t)(sweep0 + s + 1), st, &s_E, event++);
                 scale = s_scale[t];
